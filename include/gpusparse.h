@@ -1,0 +1,199 @@
+/*
+ * gpusparse.h — C ABI of the B200-native GPUSparse hot path (arxiv/paper_2606_26441).
+ *
+ * What the library computes (citations are PAPER.md line numbers):
+ *   exact batched top-k scoring of sparse query vectors against a sparse document collection,
+ *       score(q,d) = sum_i w_i * s_d(t_i)                            L106-111 §4.1 Eq. (4)
+ *   over a GPU-resident inverted index whose posting lists are doc-id sorted and padded to
+ *   32-entry warp blocks with (doc_id=-1, score=0) sentinels         L79-90  §3.2 Eq. (2)
+ *   and over a CSR forward index used by the document-parallel kernel L174    §5.3,
+ *   followed by top-k over ALL N documents                           L61, L125.
+ *   Result rows are sorted by score descending, ties broken by LOWER doc id
+ *   (BASELINE.json north_star; the paper leaves tie order open, L129/L396).
+ *
+ * Conventions
+ *   - Plain C: opaque handle, plain pointers and sizes, no C++/torch types.
+ *   - Every array pointer is a DEVICE pointer unless the name or comment says HOST.
+ *   - The caller owns inputs, outputs and workspaces; the library owns only what hangs off a
+ *     gs_index_t handle (allocated through the optional gs_alloc_t callbacks, default cudaMalloc).
+ *   - Document id = CSR row number (0-based int32, N < 2^31).  Term ids are int32 in [0, V).
+ *   - `gs_stream_t` is a cudaStream_t passed as void* (0 = default stream).
+ *   - Errors are return codes, never exceptions or aborts.  Host-checkable arguments are checked
+ *     before any launch.  There is NO CPU fallback: a device that is not sm_100 yields
+ *     GS_ERR_UNSUPPORTED_DEVICE.
+ *   - Two numeric modes: GS_W_F32 (fp32 weights, fp32 accumulate, fp32 scores) and GS_W_U8
+ *     (uint8 impacts, int32 accumulate, int32 scores; bit-exact by construction).
+ */
+#ifndef GPUSPARSE_H
+#define GPUSPARSE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GS_ABI_VERSION 1
+#if defined(__GNUC__)
+#define GS_API __attribute__((visibility("default")))
+#else
+#define GS_API
+#endif
+#define GS_MAX_K 4096          /* largest supported k (bitonic finish runs in shared memory)   */
+#define GS_WARP_BLOCK 32       /* posting-list padding granularity W of Eq. (2)        */
+
+typedef struct gs_index gs_index_t;   /* opaque, immutable after build (paper: no dynamic updates, L412) */
+typedef void* gs_stream_t;
+
+typedef enum gs_status {
+    GS_OK = 0,
+    GS_ERR_INVALID_ARG = 1,        /* null pointer, bad enum, indptr[0] != 0, host pointer where device expected */
+    GS_ERR_OUT_OF_RANGE = 2,       /* term id outside [0,V), k < 1 or k > GS_MAX_K, non-monotone indptr          */
+    GS_ERR_DUPLICATE_TERM = 3,     /* a term id occurs twice in one row                                          */
+    GS_ERR_NONFINITE = 4,          /* NaN/Inf weight (fp32 mode)                                                 */
+    GS_ERR_OOM = 5,                /* allocation failed / workspace too small                                     */
+    GS_ERR_CUDA = 6,               /* a CUDA runtime call failed (see gs_last_cuda_error)                        */
+    GS_ERR_UNSUPPORTED_DEVICE = 7, /* not an sm_100 device                                                       */
+    GS_ERR_TYPE_MISMATCH = 8       /* query weight type differs from the index weight type                       */
+} gs_status_t;
+
+typedef enum gs_weight { GS_W_F32 = 0, GS_W_U8 = 1 } gs_weight_t;
+
+typedef enum gs_algo {
+    GS_ALGO_AUTO = 0,           /* term-parallel unless the work model of L176-181 favours doc-parallel */
+    GS_ALGO_TERM_PARALLEL = 1,  /* tiled scatter-add over the inverted index   (Eq. 5, §5.2)   */
+    GS_ALGO_DOC_PARALLEL = 2    /* CSR forward-index streaming, zero atomics   (L174)                    */
+} gs_algo_t;
+
+/* A batch of sparse rows in CSR form (documents for the build, queries for the search). */
+typedef struct gs_csr {
+    int64_t rows;             /* N (documents) or B (queries)                                          */
+    int64_t nnz;              /* total number of entries == indptr[rows] (the caller knows it)         */
+    const int64_t* indptr;    /* [rows+1], indptr[0] == 0, non-decreasing                              */
+    const int32_t* term_ids;  /* [nnz] in [0,V), unique within a row, any order within a row           */
+    const void* weights;      /* [nnz] float (GS_W_F32) or uint8_t (GS_W_U8); any finite value is legal */
+    int32_t wtype;            /* gs_weight_t                                                           */
+} gs_csr_t;
+
+/* Optional allocator for everything a handle owns (e.g. torch's caching allocator). */
+typedef struct gs_alloc {
+    void* (*alloc)(size_t bytes, gs_stream_t stream, void* user);   /* returns NULL on failure */
+    void (*free)(void* ptr, gs_stream_t stream, void* user);
+    void* user;
+} gs_alloc_t;
+
+/* Build options; pass NULL for defaults (fields set to 0 also mean "default"). */
+typedef struct gs_build_opts {
+    int32_t tile_docs;        /* doc-id range covered by one accumulator tile (multiple of 32; default 512)   */
+    int32_t head_max;         /* max number of posting lists additionally stored as dense strips (0..32;       */
+                              /* default 32; -1 disables).  A list qualifies when |PL(t)| >= head_density * N  */
+    float head_density;       /* default 0.5: the density at which 4 B/doc beats 8 B/posting                   */
+    int32_t validate;         /* default 1: reject out-of-range ids, duplicates, non-finite weights            */
+} gs_build_opts_t;
+
+typedef struct gs_info {
+    int64_t num_docs;          /* N                                                                   */
+    int32_t vocab_size;        /* V                                                                   */
+    int32_t wtype;
+    int64_t nnz;               /* P = number of postings                                              */
+    int64_t padded_nnz;        /* sum_t ceil(|PL(t)|/32)*32                        Eq. (2)            */
+    int64_t nonempty_terms;
+    int32_t tile_docs, num_tiles;
+    int32_t head_terms;        /* number of dense-strip posting lists                                 */
+    int64_t bytes_inverted;    /* doc_ids + weights of the padded lists            Eq. (3)            */
+    int64_t bytes_inverted_meta; /* offsets + lengths + tile-segment table                            */
+    int64_t bytes_forward;     /* CSR forward index: indptr + term ids + weights                      */
+    int64_t bytes_head;        /* dense strips                                                        */
+    int64_t bytes_total;
+} gs_info_t;
+
+/* Search options; pass NULL for defaults. */
+#define GS_FLAG_VALIDATE_QUERIES 1u   /* check query ids/dups/finite on device, synchronise, return the error   */
+#define GS_FLAG_FORCE_DENSE_TOPK 2u   /* materialise every score tile and select from it (no threshold filter) */
+#define GS_FLAG_NO_HEAD_STRIPS 4u     /* term-parallel: send every list through the scatter path               */
+typedef struct gs_search_opts {
+    int32_t algo;             /* gs_algo_t                                                              */
+    uint32_t flags;
+    int32_t query_group;      /* term-parallel: queries per accumulator tile (0 = auto)                 */
+    int32_t doc_query_tile;   /* doc-parallel: queries per pass over the forward index (0 = auto)       */
+    int32_t sample_shift;     /* threshold sample = 1/2^shift of the doc tiles (0 = auto)               */
+} gs_search_opts_t;
+
+/* Counters of the last search that used a workspace (read back with gs_search_stats). */
+typedef struct gs_stats {
+    int64_t candidates;        /* (query, doc) cells that passed the threshold filter                  */
+    int32_t overflow_queries;  /* queries re-run through the dense fallback                            */
+    int32_t launches;          /* kernels launched by the call (host-side count)                       */
+    int32_t algo_used;         /* gs_algo_t actually run                                               */
+    int32_t sample_tiles;      /* doc tiles scored densely to obtain the thresholds                    */
+} gs_stats_t;
+
+/* ------------------------------------------------------------------------------------------------
+ * Index (§3).
+ * gs_index_build: docs->indptr/term_ids/weights are DEVICE pointers; they may be released once the
+ * call returns (the call synchronises `stream`).  Builds (i) the inverted index: per-term posting
+ * lists sorted by doc id, padded to 32 with (-1, 0) sentinels, plus offsets/lengths; (ii) the CSR
+ * forward index; (iii) the per-(term, doc-tile) segment table; (iv) dense strips for the densest
+ * lists.  Errors: see gs_status_t; on error *out is NULL and nothing is leaked.
+ * ---------------------------------------------------------------------------------------------- */
+GS_API gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_build_opts_t* opts,
+                           const gs_alloc_t* alloc, gs_stream_t stream, gs_index_t** out);
+GS_API gs_status_t gs_index_info(const gs_index_t* index, gs_info_t* out);
+GS_API void gs_index_free(gs_index_t* index);
+
+/* Inspection (tests of Eq. 2/3): copy per-term metadata / one padded posting list to HOST buffers.
+ * host_offsets [V+1] int64 (padded start of each list), host_lengths [V] int32 (true |PL(t)|). */
+GS_API gs_status_t gs_index_copy_meta(const gs_index_t* index, int64_t* host_offsets, int32_t* host_lengths);
+/* Copies min(capacity, padded_length(term)) entries; host_weights is float[] or uint8_t[] per wtype. */
+GS_API gs_status_t gs_index_copy_list(const gs_index_t* index, int32_t term, int64_t capacity,
+                               int32_t* host_doc_ids, void* host_weights, int64_t* out_padded_length);
+
+/* ------------------------------------------------------------------------------------------------
+ * Search (§4-§5).
+ * gs_search: queries and outputs are DEVICE pointers.  Asynchronous on `stream` (unless
+ * GS_FLAG_VALIDATE_QUERIES), never allocates, re-entrant on different streams with different
+ * workspaces.  out_doc_ids [B*k] int32, out_scores [B*k] float (GS_W_F32) or int32_t (GS_W_U8),
+ * row-major, each row sorted by (score desc, doc id asc).  If k > N, slots >= N hold id -1 and
+ * score -inf / INT32_MIN.  Query term ids outside [0,V) are ignored unless validation is on.
+ * workspace: >= gs_search_workspace_bytes(...) bytes, 256-byte aligned.
+ * ---------------------------------------------------------------------------------------------- */
+GS_API gs_status_t gs_search_workspace_bytes(const gs_index_t* index, int64_t num_queries, int64_t query_nnz,
+                                      int32_t k, const gs_search_opts_t* opts, size_t* out_bytes);
+GS_API gs_status_t gs_search(const gs_index_t* index, const gs_csr_t* queries, int32_t k,
+                      const gs_search_opts_t* opts, int32_t* out_doc_ids, void* out_scores,
+                      void* workspace, size_t workspace_bytes, gs_stream_t stream);
+
+/* Same search with HOST buffers: queries->* and the outputs are HOST pointers (pinned memory makes
+ * the copies asynchronous).  Copies H2D, searches, copies D2H, synchronises `stream`.  Uses a
+ * workspace owned by the handle (grown on demand, hence NOT re-entrant for one handle). */
+GS_API gs_status_t gs_search_host(gs_index_t* index, const gs_csr_t* host_queries, int32_t k,
+                           const gs_search_opts_t* opts, int32_t* host_doc_ids, void* host_scores,
+                           gs_stream_t stream);
+
+/* Synchronises `stream` and copies the counters of the last gs_search on `workspace` to *out. */
+GS_API gs_status_t gs_search_stats(const void* workspace, gs_stream_t stream, gs_stats_t* out);
+
+/* Scores only (no top-k): out_scores [B][ld] float|int32 DEVICE, ld >= N.  Element (b,d) is Eq. (4).
+ * Used for element-by-element parity of either scoring kernel (algo must not be AUTO). */
+GS_API gs_status_t gs_score_dense(const gs_index_t* index, const gs_csr_t* queries, const gs_search_opts_t* opts,
+                           void* out_scores, int64_t ld, void* workspace, size_t workspace_bytes,
+                           gs_stream_t stream);
+
+/* Top-k alone: rows of a dense DEVICE score matrix [B][ld] (float or int32 per
+ * wtype) -> the k best (score desc, id asc) of columns [0,N).  -0.0 ranks equal to +0.0. */
+GS_API gs_status_t gs_topk_workspace_bytes(int64_t num_rows, int64_t n, int32_t k, size_t* out_bytes);
+GS_API gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t num_rows, int64_t n, int64_t ld,
+                          int32_t k, int32_t* out_ids, void* out_scores, void* workspace,
+                          size_t workspace_bytes, gs_stream_t stream);
+
+GS_API const char* gs_strerror(gs_status_t status);
+GS_API const char* gs_version(void);
+GS_API int32_t gs_abi_version(void);
+GS_API int32_t gs_last_cuda_error(void);    /* cudaError_t of the last GS_ERR_CUDA on this thread */
+GS_API int32_t gs_last_launch_count(void);  /* kernels launched by the last search/score/topk call on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPUSPARSE_H */

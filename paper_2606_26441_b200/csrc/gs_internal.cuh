@@ -1,0 +1,161 @@
+// gs_internal.cuh — internal declarations shared by the CUDA translation units of libgpusparse.
+// Nothing here is visible through the C ABI (include/gpusparse.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gpusparse.h"
+
+#define GS_HEAD_MAX 32          // dense-strip posting lists kept in registers by the head pass
+#define GS_SEL_BINS 2048        // radix-select digit: 11 bits
+#define GS_SEL_BITS 11
+
+void gs_set_cuda_error(cudaError_t e);
+#define GS_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e__ = (call);                       \
+        if (e__ != cudaSuccess) {                       \
+            gs_set_cuda_error(e__);                     \
+            return GS_ERR_CUDA;                         \
+        }                                               \
+    } while (0)
+#define GS_TRY(call)                                    \
+    do {                                                \
+        gs_status_t s__ = (call);                       \
+        if (s__ != GS_OK) return s__;                   \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// The index handle.  All pointers are device pointers owned by the handle.
+// ------------------------------------------------------------------------------------------------
+struct gs_index {
+    int64_t N = 0;            // documents
+    int32_t V = 0;            // vocabulary
+    int32_t wtype = 0;        // gs_weight_t
+    int64_t P = 0;            // postings
+    int64_t P_pad = 0;        // sum of padded lengths (Eq. 2)
+    int64_t nonempty = 0;
+    int32_t Ts = 512;         // docs per accumulator tile
+    int32_t ntiles = 0;       // ceil(N / Ts)
+    int64_t N_pad = 0;        // ntiles * Ts
+    // forward (doc-major CSR) index — PAPER.md L174
+    int64_t* fwd_indptr = nullptr;   // [N+1]
+    int32_t* fwd_terms = nullptr;    // [P]
+    void* fwd_w = nullptr;           // [P] float | uint8
+    // inverted index — PAPER.md L79-90
+    int64_t* inv_off = nullptr;      // [V+1] start of each padded list (multiple of 32)
+    int32_t* inv_len = nullptr;      // [V]   true list length
+    int32_t* inv_doc = nullptr;      // [P_pad] doc ids, ascending within a list, -1 in the padding
+    void* inv_w = nullptr;           // [P_pad] float | uint8, 0 in the padding
+    // per-(term, tile) segment table: seg[t*(ntiles+1)+j] = number of postings of t with doc < j*Ts
+    uint32_t* seg = nullptr;         // [V][ntiles+1]
+    // dense strips of the densest lists ("head" terms)
+    int32_t H = 0;
+    int32_t head_terms_host[GS_HEAD_MAX];
+    int16_t* head_slot = nullptr;    // [V]: strip number of a term or -1
+    void* head_strip = nullptr;      // [H][N_pad] float | uint8 (0 where the doc is not in the list)
+    // allocator
+    gs_alloc_t alloc{};
+    bool has_alloc = false;
+    // workspace owned by the handle for gs_search_host
+    void* host_ws = nullptr;
+    size_t host_ws_bytes = 0;
+    void* host_stage = nullptr;      // device staging for queries and outputs
+    size_t host_stage_bytes = 0;
+    int64_t bytes_inverted = 0, bytes_meta = 0, bytes_forward = 0, bytes_head = 0;
+};
+
+void* gs_dev_alloc(const gs_index* ix, size_t bytes, cudaStream_t s);
+void gs_dev_free(const gs_index* ix, void* p, cudaStream_t s);
+
+// ------------------------------------------------------------------------------------------------
+// Order-preserving keys.  A 64-bit composite key makes the order (score desc, doc id asc) a strict
+// total order on distinct documents: key = ord(score) << 32 | (0xFFFFFFFF - doc id).
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ uint32_t gs_ord_f32(uint32_t bits) {
+    if (bits == 0x80000000u) bits = 0u;                      // -0.0 ranks equal to +0.0
+    return (bits & 0x80000000u) ? ~bits : (bits | 0x80000000u);
+}
+__host__ __device__ __forceinline__ uint32_t gs_unord_f32(uint32_t o) {
+    return (o & 0x80000000u) ? (o & 0x7FFFFFFFu) : ~o;
+}
+__host__ __device__ __forceinline__ uint32_t gs_ord_i32(uint32_t bits) { return bits ^ 0x80000000u; }
+__host__ __device__ __forceinline__ uint64_t gs_make_key(uint32_t ord, uint32_t doc) {
+    return ((uint64_t)ord << 32) | (uint64_t)(0xFFFFFFFFu - doc);
+}
+template <int WT>
+__device__ __forceinline__ uint32_t gs_ord_bits(uint32_t bits) {
+    return WT == GS_W_F32 ? gs_ord_f32(bits) : gs_ord_i32(bits);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Query batch after ingest (S1): per-query dense head weights + compacted tail term lists.
+// Accumulator type: float (GS_W_F32) or int32 (GS_W_U8), both 4 bytes, stored as uint32 bit patterns.
+// ------------------------------------------------------------------------------------------------
+struct gs_qbatch {
+    int64_t B = 0;
+    int64_t nnz = 0;
+    const int64_t* indptr = nullptr;   // caller's CSR indptr (device)
+    uint32_t* head_w = nullptr;        // [B][GS_HEAD_MAX] accumulator-typed weights, 0 if absent
+    int32_t* tail_term = nullptr;      // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]
+    uint32_t* tail_w = nullptr;        // [nnz] accumulator-typed
+    int32_t* tail_cnt = nullptr;       // [B]
+    int32_t* status = nullptr;         // device status word: first validation error (gs_status_t) or 0
+};
+
+// Where a scoring kernel puts its results.
+//   dense : scores[(b - q0) * ld + col] for the doc tiles it was given (col = compact tile index * Ts + d)
+//   filter: append key64 to cand[b * cand_cap + n] when key >= thr[b]
+struct gs_tileset {
+    int32_t first = 0;       // first doc tile
+    int32_t stride = 1;      // tile j of the set is doc tile first + j*stride
+    int32_t count = 0;       // number of tiles in the set
+};
+struct gs_sink {
+    uint32_t* dense = nullptr;
+    int64_t ld = 0;
+    const uint64_t* thr = nullptr;       // [B] threshold keys (filter mode when non-null)
+    uint64_t* cand = nullptr;            // [B][cand_cap]
+    uint32_t* cand_cnt = nullptr;        // [B]
+    int64_t cand_cap = 0;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Launchers (one per translation unit).  Each returns GS_OK or GS_ERR_CUDA and counts its launches.
+// ------------------------------------------------------------------------------------------------
+extern thread_local int32_t gs_tls_launches;
+
+gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head,
+                             gs_qbatch* qb, cudaStream_t s);
+
+gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
+                                 bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
+
+// doc-parallel: scratch holds the transposed query tile(s)
+size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, int64_t q_nnz);
+gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_qbatch& qb, int64_t q0, int64_t nq,
+                                int qtile, const gs_tileset& ts, const gs_sink& sink, void* scratch,
+                                cudaStream_t s);
+
+// top-k selection (S3).  Source = dense score rows or candidate key lists.
+struct gs_sel_src {
+    // dense
+    const uint32_t* dense = nullptr;
+    int64_t ld = 0;
+    int64_t n_cols = 0;        // columns per row (compact); column c maps to doc via tileset/Ts
+    int64_t n_docs = 0;        // columns whose doc id >= n_docs are ignored
+    gs_tileset ts{};
+    int32_t Ts = 0;            // 0: column == doc id
+    // list
+    const uint64_t* keys = nullptr;
+    int64_t cap = 0;
+    const uint32_t* counts = nullptr;
+    int32_t wtype = 0;
+};
+size_t gs_select_scratch_bytes(int64_t rows, int32_t k);
+// Selects the k best of every row; writes sorted results to out_ids/out_scores (row stride k) when
+// non-null, and the k-th key (threshold) of each row to out_thr when non-null.  When out_keys is
+// non-null the selected (unsorted) keys are ALSO appended to out_keys[b*out_cap + ..] / out_cnt[b].
+gs_status_t gs_launch_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* out_ids, void* out_scores,
+                             uint64_t* out_thr, uint64_t* out_keys, uint32_t* out_cnt, int64_t out_cap,
+                             void* scratch, cudaStream_t s);

@@ -1,0 +1,308 @@
+// index_build.cu — S0: doc CSR -> GPU-resident inverted index + forward index + tile segments + head strips.
+//
+// PAPER.md §3 (L67-100): two flat arrays doc_ids(int32)/scores(fp32) with per-term offsets/lengths
+// (L79-84); every list padded to a multiple of W=32 with (doc_id=-1, score=0) and sorted by doc id
+// (Eq. 2); no delta coding (L75).  Additions of this build: a per-(term, doc
+// tile) segment table so a kernel can find the slice of a list inside a doc-id range without
+// searching, and dense strips for the few lists that cover >= half the collection.
+//
+// Because CSR rows arrive in doc order, a STABLE sort of the postings by term id yields doc-id-sorted
+// lists directly.  The sort is cub::DeviceRadixSort (a library primitive; the build is not on the
+// timed path).
+#include <cub/device/device_radix_sort.cuh>
+
+#include <algorithm>
+#include <vector>
+
+#include "gs_internal.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+
+// err[0] = first error code seen
+__global__ void k_check_indptr(const int64_t* __restrict__ indptr, int64_t rows, int* err) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < rows && indptr[i + 1] < indptr[i]) atomicCAS(err, 0, (int)GS_ERR_OUT_OF_RANGE);
+}
+
+template <int WT>
+__global__ void k_check_entries(const int32_t* __restrict__ terms, const void* __restrict__ w, int64_t nnz, int32_t V,
+                                int* err) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= nnz) return;
+    int32_t t = terms[i];
+    if (t < 0 || t >= V) atomicCAS(err, 0, (int)GS_ERR_OUT_OF_RANGE);
+    if (WT == GS_W_F32) {
+        float x = ((const float*)w)[i];
+        if (!isfinite(x)) atomicCAS(err, 0, (int)GS_ERR_NONFINITE);
+    }
+}
+
+// term histogram with a full-vocabulary shared-memory privatised copy when it fits
+__global__ void k_term_hist(const int32_t* __restrict__ terms, int64_t nnz, int32_t V, int32_t* __restrict__ counts,
+                            int use_smem) {
+    extern __shared__ int32_t sh[];
+    if (use_smem) {
+        for (int i = threadIdx.x; i < V; i += blockDim.x) sh[i] = 0;
+        __syncthreads();
+    }
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nnz; i += (int64_t)gridDim.x * blockDim.x) {
+        int32_t t = terms[i];
+        if (t < 0 || t >= V) continue;
+        if (use_smem) atomicAdd(&sh[t], 1);
+        else atomicAdd(&counts[t], 1);
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < V; i += blockDim.x)
+            if (sh[i]) atomicAdd(&counts[i], sh[i]);
+    }
+}
+
+__global__ void k_iota(uint32_t* __restrict__ v, int64_t n) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) v[i] = (uint32_t)i;
+}
+
+// one warp per document: write the doc id over its posting range
+__global__ void k_expand_rows(const int64_t* __restrict__ indptr, int64_t rows, int32_t* __restrict__ rowid) {
+    int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (warp >= rows) return;
+    int64_t a = indptr[warp], b = indptr[warp + 1];
+    for (int64_t i = a + lane; i < b; i += 32) rowid[i] = (int32_t)warp;
+}
+
+// sorted position j (term-major, stable) -> padded slot
+template <typename W>
+__global__ void k_scatter_padded(const int32_t* __restrict__ sorted_terms, const uint32_t* __restrict__ sorted_src,
+                                 const int32_t* __restrict__ rowid, const W* __restrict__ w_in,
+                                 const int64_t* __restrict__ cnt_scan, const int64_t* __restrict__ inv_off,
+                                 int64_t nnz, int32_t* __restrict__ inv_doc, W* __restrict__ inv_w) {
+    int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (j >= nnz) return;
+    int32_t t = sorted_terms[j];
+    uint32_t src = sorted_src[j];
+    int64_t pos = inv_off[t] + (j - cnt_scan[t]);
+    inv_doc[pos] = rowid[src];
+    inv_w[pos] = w_in[src];
+}
+
+__device__ __forceinline__ int32_t term_of_slot(const int64_t* __restrict__ inv_off, int32_t V, int64_t pos) {
+    // largest t with inv_off[t] <= pos
+    int32_t lo = 0, hi = V;   // answer in [lo, hi)
+    while (hi - lo > 1) {
+        int32_t mid = (lo + hi) >> 1;
+        if (inv_off[mid] <= pos) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// Per padded slot: duplicate detection (equal neighbours inside a list) + the tile segment table.
+__global__ void k_segments(const int64_t* __restrict__ inv_off, const int32_t* __restrict__ inv_len,
+                           const int32_t* __restrict__ inv_doc, int32_t V, int64_t P_pad, int32_t Ts, int32_t ntiles,
+                           uint32_t* __restrict__ seg, int* err) {
+    int64_t pos = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (pos >= P_pad) return;
+    int32_t t = term_of_slot(inv_off, V, pos);
+    int32_t i = (int32_t)(pos - inv_off[t]);
+    int32_t len = inv_len[t];
+    if (i >= len) return;                       // padding slot
+    int32_t doc = inv_doc[pos];
+    int32_t tile_cur = doc / Ts;
+    int32_t tile_prev = -1;
+    if (i > 0) {
+        int32_t prev = inv_doc[pos - 1];
+        if (prev == doc) atomicCAS(err, 0, (int)GS_ERR_DUPLICATE_TERM);
+        tile_prev = prev / Ts;
+    }
+    uint32_t* row = seg + (size_t)t * (ntiles + 1);
+    for (int32_t j = tile_prev + 1; j <= tile_cur; ++j) row[j] = (uint32_t)i;
+    if (i == len - 1)
+        for (int32_t j = tile_cur + 1; j <= ntiles; ++j) row[j] = (uint32_t)len;
+}
+
+template <typename W>
+__global__ void k_fill_strip(const int32_t* __restrict__ inv_doc, const W* __restrict__ inv_w, int64_t off, int32_t len,
+                             W* __restrict__ strip) {
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < len) strip[inv_doc[off + i]] = inv_w[off + i];
+}
+
+inline unsigned grid_for(int64_t n, int threads = kThreads) { return (unsigned)((n + threads - 1) / threads); }
+
+}  // namespace
+
+void* gs_dev_alloc(const gs_index* ix, size_t bytes, cudaStream_t s) {
+    if (bytes == 0) bytes = 256;
+    if (ix && ix->has_alloc) return ix->alloc.alloc(bytes, (gs_stream_t)s, ix->alloc.user);
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return p;
+}
+void gs_dev_free(const gs_index* ix, void* p, cudaStream_t s) {
+    if (!p) return;
+    if (ix && ix->has_alloc) ix->alloc.free(p, (gs_stream_t)s, ix->alloc.user);
+    else cudaFree(p);
+}
+
+namespace {
+struct Temp {   // frees build temporaries on every exit path
+    const gs_index* ix; cudaStream_t s; std::vector<void*> ptrs;
+    void* get(size_t bytes) { void* p = gs_dev_alloc(ix, bytes, s); if (p) ptrs.push_back(p); return p; }
+    ~Temp() { cudaStreamSynchronize(s); for (void* p : ptrs) gs_dev_free(ix, p, s); }
+};
+
+template <typename W>
+gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_t& o, cudaStream_t s) {
+    const int64_t N = ix->N, P = ix->P;
+    const int32_t V = ix->V;
+    constexpr int WT = sizeof(W) == 4 ? GS_W_F32 : GS_W_U8;
+    Temp tmp{ix, s, {}};
+    int* d_err = (int*)tmp.get(sizeof(int));
+    if (!d_err) return GS_ERR_OOM;
+    GS_CUDA(cudaMemsetAsync(d_err, 0, sizeof(int), s));
+
+    if (N > 0) k_check_indptr<<<grid_for(N), kThreads, 0, s>>>(docs->indptr, N, d_err);
+    if (o.validate && P > 0)
+        k_check_entries<WT><<<grid_for(P), kThreads, 0, s>>>(docs->term_ids, docs->weights, P, V, d_err);
+    int h_err = 0;
+    GS_CUDA(cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
+    GS_CUDA(cudaStreamSynchronize(s));
+    if (h_err) return (gs_status_t)h_err;
+
+    // ---- forward index: a private copy of the CSR (inputs may be released after the call)
+    ix->fwd_indptr = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(N + 1), s);
+    ix->fwd_terms = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)P, s);
+    ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)P, s);
+    if (!ix->fwd_indptr || !ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
+    GS_CUDA(cudaMemcpyAsync(ix->fwd_indptr, docs->indptr, sizeof(int64_t) * (size_t)(N + 1), cudaMemcpyDeviceToDevice, s));
+    if (P > 0) {
+        GS_CUDA(cudaMemcpyAsync(ix->fwd_terms, docs->term_ids, sizeof(int32_t) * (size_t)P, cudaMemcpyDeviceToDevice, s));
+        GS_CUDA(cudaMemcpyAsync(ix->fwd_w, docs->weights, sizeof(W) * (size_t)P, cudaMemcpyDeviceToDevice, s));
+    }
+    ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(N + 1) + (sizeof(int32_t) + sizeof(W)) * (size_t)P);
+
+    // ---- list lengths
+    ix->inv_len = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)V, s);
+    ix->inv_off = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(V + 1), s);
+    if (!ix->inv_len || !ix->inv_off) return GS_ERR_OOM;
+    GS_CUDA(cudaMemsetAsync(ix->inv_len, 0, sizeof(int32_t) * (size_t)V, s));
+    if (P > 0) {
+        int dev = 0, smem_max = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        size_t need = sizeof(int32_t) * (size_t)V;
+        int use_smem = need <= (size_t)smem_max;
+        if (use_smem) GS_CUDA(cudaFuncSetAttribute(k_term_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+        k_term_hist<<<sms * 2, 512, use_smem ? need : 0, s>>>(docs->term_ids, P, V, ix->inv_len, use_smem);
+    }
+    std::vector<int32_t> h_len(V);
+    GS_CUDA(cudaMemcpyAsync(h_len.data(), ix->inv_len, sizeof(int32_t) * (size_t)V, cudaMemcpyDeviceToHost, s));
+    GS_CUDA(cudaStreamSynchronize(s));
+
+    // ---- host: padded offsets (Eq. 2), unpadded scan, head selection
+    std::vector<int64_t> h_off(V + 1), h_scan(V + 1);
+    int64_t acc = 0, accp = 0, nonempty = 0;
+    for (int32_t t = 0; t < V; ++t) {
+        h_scan[t] = acc;
+        h_off[t] = accp;
+        acc += h_len[t];
+        accp += ((int64_t)h_len[t] + GS_WARP_BLOCK - 1) / GS_WARP_BLOCK * GS_WARP_BLOCK;
+        nonempty += h_len[t] > 0;
+    }
+    h_scan[V] = acc;
+    h_off[V] = accp;
+    if (acc != P) return GS_ERR_OUT_OF_RANGE;   // some term id was outside [0,V) (validate off)
+    ix->P_pad = accp;
+    ix->nonempty = nonempty;
+    GS_CUDA(cudaMemcpyAsync(ix->inv_off, h_off.data(), sizeof(int64_t) * (size_t)(V + 1), cudaMemcpyHostToDevice, s));
+
+    std::vector<int32_t> order;
+    int hmax = o.head_max < 0 ? 0 : (o.head_max == 0 ? GS_HEAD_MAX : std::min(o.head_max, GS_HEAD_MAX));
+    float dens = o.head_density > 0.f ? o.head_density : 0.5f;
+    for (int32_t t = 0; t < V; ++t)
+        if (N > 0 && (double)h_len[t] >= (double)dens * (double)N && h_len[t] > 0) order.push_back(t);
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return h_len[a] > h_len[b]; });
+    if ((int)order.size() > hmax) order.resize(hmax);
+    ix->H = (int32_t)order.size();
+    std::vector<int16_t> h_slot(V, (int16_t)-1);
+    for (int h = 0; h < GS_HEAD_MAX; ++h) ix->head_terms_host[h] = h < ix->H ? order[h] : -1;
+    for (int h = 0; h < ix->H; ++h) h_slot[order[h]] = (int16_t)h;
+    ix->head_slot = (int16_t*)gs_dev_alloc(ix, sizeof(int16_t) * (size_t)V, s);
+    if (!ix->head_slot) return GS_ERR_OOM;
+    GS_CUDA(cudaMemcpyAsync(ix->head_slot, h_slot.data(), sizeof(int16_t) * (size_t)V, cudaMemcpyHostToDevice, s));
+
+    // ---- padded inverted arrays, pre-filled with the sentinel (doc_id=-1, score=0), L90
+    ix->inv_doc = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)ix->P_pad, s);
+    ix->inv_w = gs_dev_alloc(ix, sizeof(W) * (size_t)ix->P_pad, s);
+    if (!ix->inv_doc || !ix->inv_w) return GS_ERR_OOM;
+    if (ix->P_pad > 0) {
+        GS_CUDA(cudaMemsetAsync(ix->inv_doc, 0xFF, sizeof(int32_t) * (size_t)ix->P_pad, s));
+        GS_CUDA(cudaMemsetAsync(ix->inv_w, 0, sizeof(W) * (size_t)ix->P_pad, s));
+    }
+    ix->bytes_inverted = (int64_t)((sizeof(int32_t) + sizeof(W)) * (size_t)ix->P_pad);
+
+    // ---- segment table
+    const size_t seg_elems = (size_t)V * (size_t)(ix->ntiles + 1);
+    ix->seg = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * seg_elems, s);
+    if (!ix->seg) return GS_ERR_OOM;
+    GS_CUDA(cudaMemsetAsync(ix->seg, 0, sizeof(uint32_t) * seg_elems, s));
+    ix->bytes_meta = (int64_t)(sizeof(uint32_t) * seg_elems + sizeof(int64_t) * (size_t)(V + 1) +
+                               sizeof(int32_t) * (size_t)V + sizeof(int16_t) * (size_t)V);
+
+    if (P > 0) {
+        // ---- stable sort of (term, source position) by term
+        int32_t* d_sorted_terms = (int32_t*)tmp.get(sizeof(int32_t) * (size_t)P);
+        uint32_t* d_src_in = (uint32_t*)tmp.get(sizeof(uint32_t) * (size_t)P);
+        uint32_t* d_src_out = (uint32_t*)tmp.get(sizeof(uint32_t) * (size_t)P);
+        int32_t* d_rowid = (int32_t*)tmp.get(sizeof(int32_t) * (size_t)P);
+        int64_t* d_scan = (int64_t*)tmp.get(sizeof(int64_t) * (size_t)(V + 1));
+        if (!d_sorted_terms || !d_src_in || !d_src_out || !d_rowid || !d_scan) return GS_ERR_OOM;
+        GS_CUDA(cudaMemcpyAsync(d_scan, h_scan.data(), sizeof(int64_t) * (size_t)(V + 1), cudaMemcpyHostToDevice, s));
+        k_iota<<<grid_for(P), kThreads, 0, s>>>(d_src_in, P);
+        k_expand_rows<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, N, d_rowid);
+        int end_bit = 1;
+        while ((1 << end_bit) < V) ++end_bit;
+        size_t cub_bytes = 0;
+        if (P > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;   // cub item counts are int
+        GS_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, cub_bytes, docs->term_ids, d_sorted_terms, d_src_in, d_src_out,
+                                                (int)P, 0, end_bit, s));
+        void* d_cub = tmp.get(cub_bytes);
+        if (!d_cub) return GS_ERR_OOM;
+        GS_CUDA(cub::DeviceRadixSort::SortPairs(d_cub, cub_bytes, docs->term_ids, d_sorted_terms, d_src_in, d_src_out,
+                                                (int)P, 0, end_bit, s));
+        k_scatter_padded<W><<<grid_for(P), kThreads, 0, s>>>(d_sorted_terms, d_src_out, d_rowid, (const W*)docs->weights,
+                                                            d_scan, ix->inv_off, P, ix->inv_doc, (W*)ix->inv_w);
+        k_segments<<<grid_for(ix->P_pad), kThreads, 0, s>>>(ix->inv_off, ix->inv_len, ix->inv_doc, V, ix->P_pad, ix->Ts,
+                                                            ix->ntiles, ix->seg, d_err);
+        GS_CUDA(cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaStreamSynchronize(s));
+        GS_CUDA(cudaGetLastError());
+        if (h_err && o.validate) return (gs_status_t)h_err;
+    }
+
+    // ---- dense strips of the head lists
+    if (ix->H > 0) {
+        size_t strip_bytes = sizeof(W) * (size_t)ix->H * (size_t)ix->N_pad;
+        ix->head_strip = gs_dev_alloc(ix, strip_bytes, s);
+        if (!ix->head_strip) return GS_ERR_OOM;
+        GS_CUDA(cudaMemsetAsync(ix->head_strip, 0, strip_bytes, s));
+        for (int h = 0; h < ix->H; ++h) {
+            int32_t t = order[h];
+            k_fill_strip<W><<<grid_for(h_len[t]), kThreads, 0, s>>>(ix->inv_doc, (const W*)ix->inv_w, h_off[t], h_len[t],
+                                                                   (W*)ix->head_strip + (size_t)h * (size_t)ix->N_pad);
+        }
+        ix->bytes_head = (int64_t)strip_bytes;
+    }
+    GS_CUDA(cudaStreamSynchronize(s));
+    GS_CUDA(cudaGetLastError());
+    return GS_OK;
+}
+}  // namespace
+
+gs_status_t gs_build_index_impl(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_t& o, cudaStream_t s) {
+    return ix->wtype == GS_W_F32 ? build_typed<float>(ix, docs, o, s) : build_typed<uint8_t>(ix, docs, o, s);
+}

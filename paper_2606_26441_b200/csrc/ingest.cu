@@ -1,0 +1,82 @@
+// ingest.cu — S1: validate and reorganise the CSR query batch for the scoring kernels.
+//
+// The paper pads queries to a [B, M] matrix of (term id, weight) in Python (PAPER.md L120-123,
+// L146-152).  Here one warp per query splits its terms into
+//   * head terms (lists kept as dense strips): weights go into a dense row head_w[b][32];
+//   * tail terms: compacted (row b starts at indptr[b]) into tail_term/tail_w, weights converted to the
+//     accumulator type (float, or int32 for uint8 impacts).
+// Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
+// (out of range / duplicate / non-finite) is recorded in a status word the host reads back.
+#include "gs_internal.cuh"
+
+namespace {
+
+template <int WT>
+__global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
+                         const void* __restrict__ weights, int64_t B, int32_t V, const int16_t* __restrict__ head_slot,
+                         int use_head, int validate, uint32_t* __restrict__ head_w, int32_t* __restrict__ tail_term,
+                         uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, int32_t* __restrict__ status) {
+    const int lane = threadIdx.x & 31;
+    const int64_t b = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (b >= B) return;
+    const int64_t a = indptr[b], e = indptr[b + 1];
+    head_w[b * GS_HEAD_MAX + lane] = 0u;
+    __syncwarp();
+    int32_t n_tail = 0;
+    for (int64_t i0 = a; i0 < e; i0 += 32) {
+        const int64_t i = i0 + lane;
+        int32_t t = -1;
+        uint32_t w = 0;
+        bool ok = false;
+        if (i < e) {
+            t = terms[i];
+            ok = t >= 0 && t < V;
+            if (WT == GS_W_F32) {
+                float x = ((const float*)weights)[i];
+                w = __float_as_uint(x);
+                if (validate && !isfinite(x)) atomicCAS(status, 0, (int)GS_ERR_NONFINITE);
+            } else {
+                w = (uint32_t)((const uint8_t*)weights)[i];
+            }
+            if (validate && !ok) atomicCAS(status, 0, (int)GS_ERR_OUT_OF_RANGE);
+            if (validate && ok) {   // duplicates: compare with every earlier entry of the row
+                for (int64_t j = a; j < i; ++j)
+                    if (terms[j] == t) { atomicCAS(status, 0, (int)GS_ERR_DUPLICATE_TERM); break; }
+            }
+        }
+        int slot = (ok && use_head) ? (int)head_slot[t] : -1;
+        if (ok && slot >= 0) head_w[b * GS_HEAD_MAX + slot] = w;
+        const bool is_tail = ok && slot < 0;
+        const unsigned m = __ballot_sync(0xFFFFFFFFu, is_tail);
+        if (is_tail) {
+            const int64_t dst = a + n_tail + __popc(m & ((1u << lane) - 1u));
+            tail_term[dst] = t;
+            tail_w[dst] = w;
+        }
+        n_tail += __popc(m);
+        __syncwarp();
+    }
+    if (lane == 0) tail_cnt[b] = n_tail;
+}
+
+}  // namespace
+
+gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head, gs_qbatch* qb,
+                             cudaStream_t s) {
+    const int64_t B = q->rows;
+    GS_CUDA(cudaMemsetAsync(qb->status, 0, sizeof(int32_t), s));
+    if (B == 0) return GS_OK;
+    const int threads = 128;
+    const unsigned grid = (unsigned)((B * 32 + threads - 1) / threads);
+    if (ix->wtype == GS_W_F32)
+        k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
+                                                   use_head && ix->H > 0, validate, qb->head_w, qb->tail_term,
+                                                   qb->tail_w, qb->tail_cnt, qb->status);
+    else
+        k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
+                                                  use_head && ix->H > 0, validate, qb->head_w, qb->tail_term,
+                                                  qb->tail_w, qb->tail_cnt, qb->status);
+    ++gs_tls_launches;
+    GS_CUDA(cudaGetLastError());
+    return GS_OK;
+}

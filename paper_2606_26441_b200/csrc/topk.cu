@@ -1,0 +1,270 @@
+// topk.cu — S3: exact per-query top-k under the strict order (score desc, doc id asc) (kernel K3').
+//
+// The paper takes torch.topk over the whole [B,N] score buffer
+// and attributes its recall < 1 to unspecified tie order (L129, L396).  Here every candidate is a
+// 64-bit composite key ord(score)<<32 | ~doc, so all keys of a query are distinct and the order is
+// total: an MSD radix select (11-bit digits, shared-memory histograms) finds the exact k-th key,
+// one pass collects the k keys >= it, and a bitonic network (warp shuffles for the short strides,
+// shared memory for the long ones) sorts them.  The select runs either over dense score rows
+// (fallback / threshold sample) or over the candidate key lists the scoring kernels emit.
+#include <algorithm>
+
+#include "gs_internal.cuh"
+
+namespace {
+
+constexpr int kSelThreads = 512;
+constexpr int kItemsPerCta = 16384;
+
+struct SelState {
+    unsigned long long prefix;   // key bits decided so far (undecided low bits are 0)
+    unsigned int k_rem;          // how many of the items matching `prefix` are still wanted
+    int shift;                   // bit position of the next digit (+width); <= 0 when all bits are decided
+    int done;
+    unsigned int n_items;
+    unsigned int out_cnt;
+    unsigned int pad[2];
+};
+
+__device__ __forceinline__ int64_t src_count(const gs_sel_src& s, int64_t b) {
+    return s.keys ? (int64_t)min((uint64_t)s.counts[b], (uint64_t)s.cap) : s.n_cols;
+}
+// key of item i of row b, or 0 when the item does not exist (column beyond the last document)
+template <int WT>
+__device__ __forceinline__ uint64_t src_key(const gs_sel_src& s, int64_t b, int64_t i) {
+    if (s.keys) return s.keys[b * s.cap + i];
+    int64_t doc = i;
+    if (s.Ts > 0) doc = ((int64_t)s.ts.first + (i / s.Ts) * s.ts.stride) * s.Ts + (i % s.Ts);
+    if (doc >= s.n_docs) return 0ull;
+    return gs_make_key(gs_ord_bits<WT>(s.dense[b * s.ld + i]), (uint32_t)doc);
+}
+
+__global__ void k_sel_init(gs_sel_src src, int64_t rows, int32_t k, SelState* st, uint32_t* hist) {
+    const int64_t b = blockIdx.x;
+    if (threadIdx.x == 0) {
+        int64_t n = src_count(src, b);
+        if (!src.keys) {   // dense: number of live documents among the columns
+            int64_t live = 0;
+            if (src.Ts > 0) {
+                for (int64_t j = 0; j < src.ts.count; ++j) {
+                    int64_t d0 = ((int64_t)src.ts.first + j * src.ts.stride) * src.Ts;
+                    live += max((int64_t)0, min((int64_t)src.Ts, src.n_docs - d0));
+                }
+            } else live = min(n, src.n_docs);
+            n = live;
+        }
+        SelState s;
+        s.prefix = 0ull;
+        s.k_rem = (unsigned)min((int64_t)k, n);
+        s.shift = 64;
+        s.done = (n <= k) ? 1 : 0;     // everything is selected: threshold key 0 (no live key is 0)
+        s.n_items = (unsigned)n;
+        s.out_cnt = 0;
+        st[b] = s;
+    }
+    for (int i = threadIdx.x; i < GS_SEL_BINS; i += blockDim.x) hist[b * GS_SEL_BINS + i] = 0;
+}
+
+// histogram of the next digit over the items whose decided bits equal the prefix
+template <int WT>
+__global__ void __launch_bounds__(kSelThreads) k_sel_hist(gs_sel_src src, const SelState* __restrict__ st,
+                                                          uint32_t* __restrict__ hist) {
+    const int64_t b = blockIdx.y;
+    const SelState s = st[b];
+    if (s.done) return;
+    const int64_t n = src_count(src, b);
+    const int64_t i0 = (int64_t)blockIdx.x * kItemsPerCta;
+    if (i0 >= n) return;
+    __shared__ uint32_t sh[GS_SEL_BINS];
+    for (int i = threadIdx.x; i < GS_SEL_BINS; i += kSelThreads) sh[i] = 0;
+    __syncthreads();
+    const int width = min(GS_SEL_BITS, s.shift);
+    const int lo = s.shift - width;                          // digit = bits [lo, lo+width)
+    const uint64_t himask = s.shift >= 64 ? 0ull : ~((1ull << s.shift) - 1ull);
+    const int64_t i1 = min(n, i0 + kItemsPerCta);
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += kSelThreads) {
+        const uint64_t key = src_key<WT>(src, b, i);
+        if (key != 0ull && (key & himask) == s.prefix) atomicAdd(&sh[(key >> lo) & ((1u << width) - 1u)], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < GS_SEL_BINS; i += kSelThreads)
+        if (sh[i]) atomicAdd(&hist[b * GS_SEL_BINS + i], sh[i]);
+}
+
+// pick the digit value that contains the k_rem-th largest item, update the state, clear the histogram
+__global__ void __launch_bounds__(GS_SEL_BINS / 4) k_sel_scan(SelState* __restrict__ st, uint32_t* __restrict__ hist) {
+    const int64_t b = blockIdx.x;
+    SelState s = st[b];
+    if (s.done) return;
+    uint32_t* h = hist + b * GS_SEL_BINS;
+    __shared__ uint32_t part[GS_SEL_BINS / 4];
+    __shared__ int sel_bin;
+    __shared__ uint32_t sel_above, sel_cnt;
+    const int tid = threadIdx.x;               // thread tid owns bins [4*tid, 4*tid+4), scanned from the TOP
+    uint32_t c[4], tot = 0;
+    for (int j = 0; j < 4; ++j) { c[j] = h[4 * tid + j]; tot += c[j]; }
+    part[tid] = tot;
+    __syncthreads();
+    // suffix sums over threads (512 partials): simple log-step scan in shared memory
+    for (int o = 1; o < GS_SEL_BINS / 4; o <<= 1) {
+        uint32_t v = (tid + o < GS_SEL_BINS / 4) ? part[tid + o] : 0;
+        __syncthreads();
+        part[tid] += v;
+        __syncthreads();
+    }
+    uint32_t above = part[tid] - tot;          // items in bins strictly above this thread's bins
+    for (int j = 3; j >= 0; --j) {
+        if (above < s.k_rem && above + c[j] >= s.k_rem) { sel_bin = 4 * tid + j; sel_above = above; sel_cnt = c[j]; }
+        above += c[j];
+    }
+    __syncthreads();
+    for (int j = 0; j < 4; ++j) h[4 * tid + j] = 0;
+    if (tid == 0) {
+        const int width = min(GS_SEL_BITS, s.shift);
+        const int lo = s.shift - width;
+        s.prefix |= (unsigned long long)sel_bin << lo;
+        s.k_rem -= sel_above;
+        s.shift = lo;
+        // every item of the chosen bin is wanted, or no bits are left: the threshold is decided
+        if (sel_cnt == s.k_rem || lo == 0) s.done = 1;
+        st[b] = s;
+    }
+}
+
+// collect the items with key >= threshold: exactly k_total of them (all keys are distinct)
+template <int WT>
+__global__ void __launch_bounds__(kSelThreads) k_sel_collect(gs_sel_src src, SelState* __restrict__ st, int32_t k,
+                                                             uint64_t* __restrict__ sel) {
+    const int64_t b = blockIdx.y;
+    const int64_t n = src_count(src, b);
+    const int64_t i0 = (int64_t)blockIdx.x * kItemsPerCta;
+    if (i0 >= n) return;
+    const uint64_t thr = st[b].prefix;
+    const int64_t i1 = min(n, i0 + kItemsPerCta);
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += kSelThreads) {
+        const uint64_t key = src_key<WT>(src, b, i);
+        if (key != 0ull && key >= thr) {
+            const unsigned pos = atomicAdd(&st[b].out_cnt, 1u);
+            if (pos < (unsigned)k) sel[b * k + pos] = key;
+        }
+    }
+}
+
+// bitonic sort (descending) of the selected keys, then decode (id, score); also the k-th key
+template <int WT>
+__global__ void k_sel_sort(const SelState* __restrict__ st, const uint64_t* __restrict__ sel, int32_t k, int kp2,
+                           int32_t* __restrict__ out_ids, uint32_t* __restrict__ out_scores,
+                           uint64_t* __restrict__ out_thr, uint64_t* __restrict__ out_keys,
+                           uint32_t* __restrict__ out_cnt, int64_t out_cap) {
+    extern __shared__ uint64_t sk[];
+    const int64_t b = blockIdx.x;
+    const unsigned cnt = min(st[b].out_cnt, (unsigned)k);
+    for (int i = threadIdx.x; i < kp2; i += blockDim.x) sk[i] = (unsigned)i < cnt ? sel[b * k + i] : 0ull;
+    __syncthreads();
+    for (int size = 2; size <= kp2; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            if (stride >= 32) {
+                for (int i = threadIdx.x; i < kp2 / 2; i += blockDim.x) {
+                    const int lo = 2 * i - (i & (stride - 1));
+                    const int hi = lo + stride;
+                    const bool desc = (lo & size) == 0;
+                    const uint64_t x = sk[lo], y = sk[hi];
+                    if ((x < y) == desc) { sk[lo] = y; sk[hi] = x; }
+                }
+                __syncthreads();
+            } else {
+                // strides < 32: finish this merge step inside warps with shuffles
+                for (int base = 0; base < kp2; base += blockDim.x) {
+                    const int i = base + threadIdx.x;
+                    uint64_t v = i < kp2 ? sk[i] : 0ull;
+                    for (int st2 = stride; st2 > 0; st2 >>= 1) {
+                        const uint64_t o = __shfl_xor_sync(0xFFFFFFFFu, v, st2);
+                        const bool lower = (i & st2) == 0;
+                        const bool desc = (i & size) == 0;
+                        const bool take_max = lower == desc;
+                        v = take_max ? (v > o ? v : o) : (v < o ? v : o);
+                    }
+                    if (i < kp2) sk[i] = v;
+                }
+                __syncthreads();
+                break;
+            }
+        }
+    }
+    for (int i = threadIdx.x; i < k; i += blockDim.x) {
+        const uint64_t key = sk[i];
+        if (out_ids) {
+            if (key == 0ull) {
+                out_ids[b * k + i] = -1;
+                out_scores[b * k + i] = WT == GS_W_F32 ? 0xFF800000u : 0x80000000u;   // -inf | INT32_MIN
+            } else {
+                out_ids[b * k + i] = (int32_t)(0xFFFFFFFFu - (uint32_t)key);
+                const uint32_t o = (uint32_t)(key >> 32);
+                out_scores[b * k + i] = WT == GS_W_F32 ? gs_unord_f32(o) : (o ^ 0x80000000u);
+            }
+        }
+        if (out_keys && key != 0ull) out_keys[b * out_cap + i] = key;
+    }
+    if (threadIdx.x == 0) {
+        // threshold for the filter phase: the k-th best key seen so far, or 0 when fewer than k exist
+        if (out_thr) out_thr[b] = cnt >= (unsigned)k ? sk[k - 1] : 0ull;
+        if (out_cnt) out_cnt[b] = cnt;
+    }
+}
+
+struct Scratch { SelState* st; uint32_t* hist; uint64_t* sel; };
+Scratch carve(void* scratch, int64_t rows, int32_t k) {
+    unsigned char* p = (unsigned char*)scratch;
+    Scratch s;
+    s.st = (SelState*)p;
+    p += ((size_t)rows * sizeof(SelState) + 255) / 256 * 256;
+    s.hist = (uint32_t*)p;
+    p += ((size_t)rows * GS_SEL_BINS * 4 + 255) / 256 * 256;
+    s.sel = (uint64_t*)p;
+    (void)k;
+    return s;
+}
+
+template <int WT>
+gs_status_t run_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* out_ids, void* out_scores,
+                       uint64_t* out_thr, uint64_t* out_keys, uint32_t* out_cnt, int64_t out_cap, void* scratch,
+                       cudaStream_t s) {
+    Scratch sc = carve(scratch, rows, k);
+    const int64_t max_items = src.keys ? src.cap : src.n_cols;
+    const unsigned chunks = (unsigned)std::max<int64_t>(1, (max_items + kItemsPerCta - 1) / kItemsPerCta);
+    if (rows > 65535) return GS_ERR_OUT_OF_RANGE;
+    k_sel_init<<<(unsigned)rows, 256, 0, s>>>(src, rows, k, sc.st, sc.hist);
+    ++gs_tls_launches;
+    for (int shift = 64; shift > 0; shift -= GS_SEL_BITS) {
+        k_sel_hist<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, sc.hist);
+        k_sel_scan<<<(unsigned)rows, GS_SEL_BINS / 4, 0, s>>>(sc.st, sc.hist);
+        gs_tls_launches += 2;
+    }
+    k_sel_collect<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, k, sc.sel);
+    int kp2 = 32;
+    while (kp2 < k) kp2 <<= 1;
+    const int threads = std::min(1024, std::max(32, kp2));
+    k_sel_sort<WT><<<(unsigned)rows, threads, (size_t)kp2 * 8, s>>>(sc.st, sc.sel, k, kp2, out_ids, (uint32_t*)out_scores,
+                                                                   out_thr, out_keys, out_cnt, out_cap);
+    gs_tls_launches += 2;
+    GS_CUDA(cudaGetLastError());
+    return GS_OK;
+}
+
+}  // namespace
+
+size_t gs_select_scratch_bytes(int64_t rows, int32_t k) {
+    size_t b = ((size_t)rows * sizeof(SelState) + 255) / 256 * 256;
+    b += ((size_t)rows * GS_SEL_BINS * 4 + 255) / 256 * 256;
+    b += ((size_t)rows * (size_t)k * 8 + 255) / 256 * 256;
+    return b;
+}
+
+gs_status_t gs_launch_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* out_ids, void* out_scores,
+                             uint64_t* out_thr, uint64_t* out_keys, uint32_t* out_cnt, int64_t out_cap, void* scratch,
+                             cudaStream_t s) {
+    if (rows <= 0) return GS_OK;
+    return src.wtype == GS_W_F32
+               ? run_select<GS_W_F32>(src, rows, k, out_ids, out_scores, out_thr, out_keys, out_cnt, out_cap, scratch, s)
+               : run_select<GS_W_U8>(src, rows, k, out_ids, out_scores, out_thr, out_keys, out_cnt, out_cap, scratch, s);
+}
