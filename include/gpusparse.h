@@ -156,6 +156,7 @@ GS_API gs_status_t gs_index_copy_list(const gs_index_t* index, int32_t term, int
  * workspaces.  out_doc_ids [B*k] int32, out_scores [B*k] float (GS_W_F32) or int32_t (GS_W_U8),
  * row-major, each row sorted by (score desc, doc id asc).  If k > N, slots >= N hold id -1 and
  * score -inf / INT32_MIN.  Query term ids outside [0,V) are ignored unless validation is on.
+ * B == 0 is legal (nothing is written; the output pointers may then be NULL).
  * workspace: >= gs_search_workspace_bytes(...) bytes, 256-byte aligned.
  * ---------------------------------------------------------------------------------------------- */
 GS_API gs_status_t gs_search_workspace_bytes(const gs_index_t* index, int64_t num_queries, int64_t query_nnz,

@@ -366,12 +366,14 @@ gs_status_t gs_search_workspace_bytes(const gs_index_t* ix, int64_t B, int64_t n
 
 gs_status_t gs_search(const gs_index_t* ix, const gs_csr_t* q, int32_t k, const gs_search_opts_t* opts, int32_t* out_ids,
                       void* out_scores, void* ws, size_t ws_bytes, gs_stream_t stream) {
-    if (!ix || !out_ids || !out_scores || !ws) return GS_ERR_INVALID_ARG;
+    if (!ix || !ws) return GS_ERR_INVALID_ARG;
     GS_TRY(check_csr_host(q, true));
     if (k < 1 || k > GS_MAX_K) return GS_ERR_OUT_OF_RANGE;
     if (q->wtype != ix->wtype) return GS_ERR_TYPE_MISMATCH;
     if (q->rows > 65535) return GS_ERR_OUT_OF_RANGE;
-    if (!is_device_ptr(out_ids) || !is_device_ptr(out_scores) || !is_device_ptr(ws)) return GS_ERR_INVALID_ARG;
+    if (!is_device_ptr(ws)) return GS_ERR_INVALID_ARG;
+    // an empty batch has empty outputs: their pointers may be null
+    if (q->rows > 0 && (!is_device_ptr(out_ids) || !is_device_ptr(out_scores))) return GS_ERR_INVALID_ARG;
     if (opts && (opts->algo < GS_ALGO_AUTO || opts->algo > GS_ALGO_DOC_PARALLEL)) return GS_ERR_INVALID_ARG;
     if (((uintptr_t)ws & 255) != 0) return GS_ERR_INVALID_ARG;
     gs_search_opts_t tmp;

@@ -1,0 +1,372 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle — `-m gpu`, run on the B200 box.
+
+Integer-impact mode must be bit-exact; fp32 mode within tol(x) = max(1e-5*|x|, 1e-6) with the set/order
+rules of tests/parity.py (BASELINE.json north_star).  Inputs come from the seeded generator
+(paper_2606_26441_b200.workload) or are built by hand here; expected values come from `oracle/` only.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_26441_b200 import workload as wl
+import parity  # tests/parity.py (pytest puts tests/ on sys.path)
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+ALGOS = ["term", "doc"]
+
+
+@pytest.fixture(scope="module")
+def gs():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (run through gpurun)")
+    from paper_2606_26441_b200 import binding
+    binding.lib()
+    return binding
+
+
+def dev(csr):
+    import torch
+    d = torch.device("cuda:0")
+    return (torch.from_numpy(np.ascontiguousarray(csr.indptr)).to(d), torch.from_numpy(np.ascontiguousarray(csr.terms)).to(d),
+            torch.from_numpy(np.ascontiguousarray(csr.weights)).to(d))
+
+
+def csr_from_dicts(rows, dtype):
+    indptr, terms, weights = [0], [], []
+    for r in rows:
+        for t, w in r.items():
+            terms.append(int(t))
+            weights.append(w)
+        indptr.append(len(terms))
+    return wl.Csr(np.array(indptr, np.int64), np.array(terms, np.int32), np.array(weights, dtype))
+
+
+def gpu_search(gs, ix, queries, k, **opt):
+    ids, sc = ix.search(*dev(queries), k, **opt)
+    return ids.cpu().numpy(), sc.cpu().numpy()
+
+
+def compare(gs, docs, queries, vocab, k, g_ids, g_sc):
+    """Full comparison of a GPU result against the oracle's exhaustive search."""
+    R_d, R_q = oracle.as_rows(docs, vocab), oracle.as_rows(queries, vocab)
+    o_ids, o_sc = oracle.search(R_q, R_d, k)
+    if docs.weights.dtype == np.uint8:
+        parity.check_int_exact(g_ids, g_sc, o_ids, o_sc)
+        return 0.0, 0
+    def true_scores(b, ids):
+        return oracle.score_pairs(R_q, R_d, np.full(len(ids), b, np.int64), ids.astype(np.int64))
+    return parity.check_f32(g_ids, g_sc, o_ids, o_sc, true_scores, docs.rows)
+
+
+# ----------------------------------------------------------------------------------------------------
+# hand-worked example (tests/golden/handworked_3doc.json) and the index layout of Eq. 2
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+def test_handworked_three_docs(gs, mode, algo):
+    g = json.load(open(os.path.join(GOLD, "handworked_3doc.json")))
+    c = g[mode]
+    dt = np.float32 if mode == "f32" else np.uint8
+    docs, queries = csr_from_dicts(c["docs"], dt), csr_from_dicts(c["queries"], dt)
+    ix = gs.Index.from_numpy(docs, g["vocab"])
+    ids, sc = gpu_search(gs, ix, queries, c["k"], algo=algo)
+    assert ids.tolist() == c["expect_ids"]
+    assert sc.tolist() == c["expect_scores"]
+    ix.close()
+
+
+def test_index_layout_eq2(gs):
+    g = json.load(open(os.path.join(GOLD, "handworked_3doc.json")))
+    docs = csr_from_dicts(g["f32"]["docs"], np.float32)
+    ix = gs.Index.from_numpy(docs, g["vocab"])
+    inf, lay = ix.info(), g["index_layout"]
+    assert inf["nnz"] == lay["postings"] and inf["nonempty_terms"] == lay["nonempty_terms"]
+    assert inf["padded_nnz"] == lay["padded_slots"]
+    ids, w = ix.posting_list(3)
+    assert len(ids) == 32
+    assert [[int(i), float(x)] for i, x in zip(ids[:2], w[:2])] == lay["term3_list"]
+    assert np.all(ids[2:] == -1) and np.all(w[2:] == 0)          # sentinel (doc_id=-1, score=0), L90
+    off, ln = ix.meta()
+    assert np.all(off % 32 == 0) and off[-1] == lay["padded_slots"]
+    assert np.array_equal(np.diff(off), (ln.astype(np.int64) + 31) // 32 * 32)
+    ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# BASELINE.json configs[0] (tiny): element-by-element score parity + top-k parity, both kernels
+# ----------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def tiny():
+    w = wl.make_workload("tiny")
+    return w
+
+
+def _dense_parity(gs, docs, queries, vocab, algo, **build_kw):
+    ix = gs.Index.from_numpy(docs, vocab, **build_kw)
+    S = ix.score_dense(*dev(queries), algo=algo).cpu().numpy()[:, :docs.rows]
+    R_d, R_q = oracle.as_rows(docs, vocab), oracle.as_rows(queries, vocab)
+    _, _, A = oracle.search(R_q, R_d, 1, all_scores=True)
+    if docs.weights.dtype == np.uint8:
+        assert np.array_equal(S.astype(np.int64), A.astype(np.int64))
+    else:
+        err = np.abs(S.astype(np.float64) - A)
+        assert np.all(err <= parity.tol(A)), f"max err {err.max()}"
+        assert np.all(S[A == 0.0] == 0.0)             # a doc with no shared term scores exactly 0
+    ix.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+@pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=-1), dict(tile_docs=2048, head_max=5)])
+def test_tiny_all_scores(gs, tiny, mode, algo, build_kw):
+    docs = tiny.docs if mode == "f32" else tiny.docs.to_u8()
+    queries = tiny.queries if mode == "f32" else tiny.queries.to_u8()
+    _dense_parity(gs, docs, queries, tiny.vocab, algo, **build_kw)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+@pytest.mark.parametrize("k", [1, 10, 33, 1000])
+def test_tiny_topk(gs, tiny, mode, algo, k):
+    docs = tiny.docs if mode == "f32" else tiny.docs.to_u8()
+    queries = tiny.queries if mode == "f32" else tiny.queries.to_u8()
+    ix = gs.Index.from_numpy(docs, tiny.vocab)
+    for flags in (0, gs.GS_FLAG_FORCE_DENSE_TOPK, gs.GS_FLAG_NO_HEAD_STRIPS | gs.GS_FLAG_VALIDATE_QUERIES):
+        ids, sc = gpu_search(gs, ix, queries, k, algo=algo, flags=flags)
+        compare(gs, docs, queries, tiny.vocab, k, ids, sc)
+    ix.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("n_docs", [1, 31, 33, 1000, 4097, 10_007])
+def test_ragged_collection_sizes(gs, algo, n_docs):
+    """N not a multiple of the warp block / tile; includes collections smaller than one tile."""
+    docs = wl.make_docs("tiny", n_docs=n_docs, seed=3)
+    queries = wl.make_queries("tiny", n_queries=7, seed=3)
+    for d, q in ((docs, queries), (docs.to_u8(), queries.to_u8())):
+        ix = gs.Index.from_numpy(d, wl.VOCAB, tile_docs=256)
+        for k in (1, 10, 50):
+            ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+            compare(gs, d, q, wl.VOCAB, k, ids, sc)
+        ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# degenerate cases and closed forms (SURVEY §8c pins, here applied to the CUDA path)
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("algo", ALGOS)
+def test_empty_query_empty_batch_and_k_gt_n(gs, algo):
+    import torch
+    docs = wl.make_docs("tiny", n_docs=40, seed=5)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    # query 1 is empty: all scores 0 -> ids ascending; k > N -> (-1, -inf) padding
+    q = wl.make_queries("tiny", n_queries=3, seed=5)
+    a, b = int(q.indptr[1]), int(q.indptr[2])
+    q = wl.Csr(np.array([0, a, a, a + int(q.indptr[3]) - b], np.int64), np.delete(q.terms, slice(a, b)),
+               np.delete(q.weights, slice(a, b)))
+    ids, sc = gpu_search(gs, ix, q, 64, algo=algo)
+    compare(gs, docs, q, wl.VOCAB, 64, ids, sc)
+    assert ids[1, :40].tolist() == list(range(40)) and np.all(sc[1, :40] == 0)
+    assert np.all(ids[:, 40:] == -1) and np.all(np.isneginf(sc[:, 40:]))
+    # B = 0
+    e = wl.Csr(np.zeros(1, np.int64), np.zeros(0, np.int32), np.zeros(0, np.float32))
+    d = torch.device("cuda:0")
+    ids0, sc0 = ix.search(torch.zeros(1, dtype=torch.int64, device=d), torch.zeros(0, dtype=torch.int32, device=d),
+                          torch.zeros(0, dtype=torch.float32, device=d), 5, algo=algo)
+    assert tuple(ids0.shape) == (0, 5) and tuple(sc0.shape) == (0, 5)
+    ix.close()
+    # integer twin of the padding rule
+    du, qu = docs.to_u8(), q.to_u8()
+    ixu = gs.Index.from_numpy(du, wl.VOCAB)
+    ids, sc = gpu_search(gs, ixu, qu, 64, algo=algo)
+    compare(gs, du, qu, wl.VOCAB, 64, ids, sc)
+    assert np.all(sc[:, 40:] == np.iinfo(np.int32).min)
+    ixu.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("N,k,tile", [(5000, 100, 64), (70_001, 1000, 512), (70_001, 4096, 512)])
+def test_closed_form_ties_across_tiles(gs, algo, N, k, tile):
+    """Every doc holds only term 0 with weight floor(d/2): ranking known in closed form, pairs tie -> lower id first."""
+    indptr = np.arange(N + 1, dtype=np.int64)
+    docs = wl.Csr(indptr, np.zeros(N, np.int32), (np.arange(N) // 2).astype(np.float32))
+    q = csr_from_dicts([{0: 1.0}, {0: 0.5}], np.float32)
+    ix = gs.Index.from_numpy(docs, 4, tile_docs=tile)
+    ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+    # descending score = descending floor(d/2); inside a pair (2j, 2j+1) the lower id comes first
+    order = sorted(range(N), key=lambda d: (-(d // 2), d))[:k]
+    assert ids[0].tolist() == order and ids[1].tolist() == order
+    assert sc[0].tolist() == [float(d // 2) for d in order]
+    assert sc[1].tolist() == [0.5 * (d // 2) for d in order]
+    ix.close()
+    # u8 twin: weight (d mod 7)+1, query impact 3
+    du = wl.Csr(indptr, np.zeros(N, np.int32), ((np.arange(N) % 7) + 1).astype(np.uint8))
+    qu = csr_from_dicts([{0: 3}], np.uint8)
+    ixu = gs.Index.from_numpy(du, 4, tile_docs=tile)
+    ids, sc = gpu_search(gs, ixu, qu, k, algo=algo)
+    order = sorted(range(N), key=lambda d: (-((d % 7) + 1), d))[:k]
+    assert ids[0].tolist() == order and sc[0].tolist() == [3 * ((d % 7) + 1) for d in order]
+    ixu.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_padding_sentinel_never_surfaces(gs, algo):
+    """A list of length 33 (== 1 mod 32); k > 33: the remaining slots are real zero-score docs in id order, never -1."""
+    N, V = 300, 16
+    rows = [{1: 1.0} for _ in range(N)]
+    hit = list(range(5, 5 + 33 * 7, 7))
+    for j, d in enumerate(hit):
+        rows[d][7] = 1.0 + j
+    docs = csr_from_dicts(rows, np.float32)
+    ix = gs.Index.from_numpy(docs, V, tile_docs=32, head_max=-1)
+    lids, _ = ix.posting_list(7)
+    assert len(lids) == 64 and lids[:33].tolist() == hit and np.all(lids[33:] == -1)
+    q = csr_from_dicts([{7: 2.0}], np.float32)
+    ids, sc = gpu_search(gs, ix, q, 50, algo=algo)
+    assert ids[0, :33].tolist() == hit[::-1]
+    rest = [d for d in range(N) if d not in set(hit)][:17]
+    assert ids[0, 33:].tolist() == rest and np.all(sc[0, 33:] == 0) and np.all(ids >= 0)
+    ix.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_signed_weights_and_negative_zero(gs, algo):
+    """Any finite weight is legal: negative scores rank below zero-score docs; -0.0 ties with +0.0."""
+    rng = np.random.default_rng(11)
+    N, V = 3000, 200
+    rows = []
+    for _ in range(N):
+        t = rng.choice(V, size=int(rng.integers(1, 30)), replace=False)
+        rows.append({int(x): float(np.float32(rng.normal())) for x in t})
+    rows[10] = {3: -0.0}
+    docs = csr_from_dicts(rows, np.float32)
+    qs = []
+    for _ in range(9):
+        t = rng.choice(V, size=int(rng.integers(1, 12)), replace=False)
+        qs.append({int(x): float(np.float32(rng.normal())) for x in t})
+    qs.append({3: 1.0})
+    q = csr_from_dicts(qs, np.float32)
+    ix = gs.Index.from_numpy(docs, V, tile_docs=128)
+    for k in (10, 2999, 3000):
+        ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+        R_d, R_q = oracle.as_rows(docs, V), oracle.as_rows(q, V)
+        o_ids, o_sc = oracle.search(R_q, R_d, k)
+        # cancellation makes |score| small relative to the summands: compare with an absolute bound from the summand sizes
+        for b in range(q.rows):
+            t = oracle.score_pairs(R_q, R_d, np.full(k, b, np.int64), ids[b].astype(np.int64))
+            assert np.all(np.abs(sc[b] - t) <= 1e-5 * 30 * 16), "score error"
+            assert np.all(np.diff(sc[b]) <= 0) and len(set(ids[b].tolist())) == k
+            eq = np.nonzero(np.diff(sc[b]) == 0)[0]
+            assert np.all(ids[b][eq] < ids[b][eq + 1])
+    ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# top-k selection alone (S3) on synthetic score arrays vs a host full sort
+# ----------------------------------------------------------------------------------------------------
+def host_topk(row, k):
+    """(score desc, id asc) by a stable full sort; -0.0 ranks equal to +0.0."""
+    n = len(row)
+    key = row.astype(np.float64) + 0.0
+    order = np.lexsort((np.arange(n), -key))[:k]
+    return order
+
+
+@pytest.mark.parametrize("n,k", [(1, 1), (100, 100), (5000, 10), (100_000, 1000), (300_001, 4096)])
+def test_topk_dense_synthetic_f32(gs, n, k):
+    import torch
+    rng = np.random.default_rng(n + k)
+    rows = [
+        np.zeros(n, np.float32),                                             # all equal
+        np.arange(n, 0, -1).astype(np.float32),                              # strictly descending
+        np.arange(n).astype(np.float32),                                     # strictly ascending
+        rng.lognormal(0, 0.5, n).astype(np.float32),
+        np.where(rng.random(n) < 0.5, 1.5, rng.random(n)).astype(np.float32),   # k-th value massively repeated
+        (rng.integers(0, 3, n) * np.float32(1e-45)).astype(np.float32),      # denormals
+        np.where(rng.random(n) < 0.5, -0.0, 0.0).astype(np.float32),         # +-0
+        rng.normal(size=n).astype(np.float32),                               # signed
+    ]
+    S = np.stack(rows)
+    k = min(k, gs.GS_MAX_K)
+    ids, sc = gs.topk_dense(torch.from_numpy(S).cuda(), k)
+    ids, sc = ids.cpu().numpy(), sc.cpu().numpy()
+    for r in range(S.shape[0]):
+        want = host_topk(S[r], k)
+        assert np.array_equal(ids[r, :len(want)], want), f"row {r}"
+        assert np.array_equal(sc[r, :len(want)] + 0.0, S[r][want] + 0.0)
+
+
+def test_topk_dense_synthetic_i32(gs):
+    import torch
+    rng = np.random.default_rng(2)
+    n, k = 77_777, 500
+    S = np.stack([rng.integers(0, 50, n), rng.integers(-2**31, 2**31 - 1, n), np.full(n, 7)]).astype(np.int32)
+    ids, sc = gs.topk_dense(torch.from_numpy(S).cuda(), k)
+    for r in range(3):
+        want = np.lexsort((np.arange(n), -S[r].astype(np.int64)))[:k]
+        assert np.array_equal(ids[r].cpu().numpy(), want) and np.array_equal(sc[r].cpu().numpy(), S[r][want])
+
+
+# ----------------------------------------------------------------------------------------------------
+# host-buffer entry point, error codes, mid-scale sampled parity
+# ----------------------------------------------------------------------------------------------------
+def test_search_host_matches_device_search(gs, tiny):
+    ix = gs.Index.from_numpy(tiny.docs, tiny.vocab)
+    q = tiny.queries
+    ids_h, sc_h = ix.search_host(q.indptr, q.terms, q.weights, 10, algo="term")
+    ids_d, sc_d = gpu_search(gs, ix, q, 10, algo="term")
+    assert np.array_equal(ids_h, ids_d) and np.array_equal(sc_h, sc_d)
+    compare(gs, tiny.docs, q, tiny.vocab, 10, ids_h, sc_h)
+    ix.close()
+
+
+def test_error_codes(gs, tiny):
+    import torch
+    d = tiny.docs
+    bad = wl.Csr(d.indptr[:11].copy(), d.terms[:int(d.indptr[10])].copy(), d.weights[:int(d.indptr[10])].copy())
+    t = bad.terms.copy(); t[3] = wl.VOCAB
+    with pytest.raises(gs.GsError) as e:
+        gs.Index.from_numpy(wl.Csr(bad.indptr, t, bad.weights), wl.VOCAB)
+    assert e.value.code == 2
+    t = bad.terms.copy(); t[1] = t[0]
+    with pytest.raises(gs.GsError) as e:
+        gs.Index.from_numpy(wl.Csr(bad.indptr, t, bad.weights), wl.VOCAB)
+    assert e.value.code == 3
+    w = bad.weights.copy(); w[5] = np.nan
+    with pytest.raises(gs.GsError) as e:
+        gs.Index.from_numpy(wl.Csr(bad.indptr, bad.terms, w), wl.VOCAB)
+    assert e.value.code == 4
+    ix = gs.Index.from_numpy(bad, wl.VOCAB)
+    q = tiny.queries
+    with pytest.raises(gs.GsError) as e:
+        gpu_search(gs, ix, q, 0)
+    assert e.value.code == 2
+    with pytest.raises(gs.GsError) as e:
+        gpu_search(gs, ix, q.to_u8(), 5)
+    assert e.value.code == 8
+    qt = q.terms.copy(); qt[1] = qt[0]
+    with pytest.raises(gs.GsError) as e:
+        gpu_search(gs, ix, wl.Csr(q.indptr, qt, q.weights), 5, flags=gs.GS_FLAG_VALIDATE_QUERIES)
+    assert e.value.code == 3
+    ix.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+def test_mid_prefix_full_compare(gs, mode, algo):
+    """First 200K docs of the 8.8M collection (several hundred tiles, ragged tail), 8 queries, k=1000: full oracle compare."""
+    docs = wl.make_docs("mid", n_docs=200_003)
+    queries = wl.make_queries("mid", n_queries=8)
+    if mode == "u8":
+        docs, queries = docs.to_u8(), queries.to_u8()
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    ids, sc = gpu_search(gs, ix, queries, 1000, algo=algo)
+    worst, subs = compare(gs, docs, queries, wl.VOCAB, 1000, ids, sc)
+    st = ix.stats()
+    assert st["overflow_queries"] == 0
+    ix.close()
