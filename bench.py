@@ -1,0 +1,381 @@
+#!/usr/bin/env python
+"""bench.py — QPS of exact batched sparse top-k search on the seeded synthetic stand-in for BASELINE.json's
+paper-scale config (8.8M docs, batch 500, top-1000, fp32), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config paper] [--docs N] [--queries B] [--k K] [--algo auto|term|doc]
+
+A "step" is one gs_search call (S1 ingest -> S2 scoring -> S3 top-k -> S4 output) over one batch
+of B queries.  `value` is measured with queries/outputs resident in HBM (CUDA events on the launching
+stream, barrier + synchronize on both sides, max over ranks); `e2e` goes through gs_search_host with pinned
+HOST buffers (H2D + D2H inside the timed region).  Inputs (index 8.45 GB per layout) are far larger than
+the 126 MB L2, so no explicit flush is needed between iterations (stated in config.l2).
+The forward and inverted index are built once before the timed region (the paper does not time the build
+either).
+
+--gpus N > 1 (torchrun): the path does not shard (BASELINE.json north_star: one GPU, no collectives), so
+every rank is an independent replica with its own index and its own query batch ("replicas only",
+DESIGN.md §8); value = all ranks' queries / max-over-ranks time.
+
+--impl reference: times the CPU oracle (oracle/) as it stands on the host cores, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "QPS @8.8M docs batch 500 top-1000"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="paper")
+    ap.add_argument("--docs", type=int, default=None, help="use the first N docs of the collection (debug)")
+    ap.add_argument("--queries", type=int, default=None)
+    ap.add_argument("--k", type=int, default=None)
+    ap.add_argument("--algo", default="auto", choices=["auto", "term", "doc"])
+    ap.add_argument("--also", default="term,doc", help="extra algos timed after the main one ('' = none)")
+    ap.add_argument("--doc-query-tile", type=int, default=0)
+    ap.add_argument("--query-group", type=int, default=0)
+    ap.add_argument("--tile-docs", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-sample-queries", type=int, default=0, help="oracle sample size (0 = one per core)")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# clocks: sample nvidia-smi DURING the timed region
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.samples, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=10)
+
+    def summary(self) -> dict:
+        sm, mx, reasons, pw = [], [], set(), []
+        for s in self.samples:
+            try:
+                sm.append(float(s[0])); mx.append(float(s[1])); pw.append(float(s[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), s[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)",
+                "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0))}
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)", "sm_max_mhz": 1965.0}
+
+
+def workload_for(args, rank: int):
+    from paper_2606_26441_b200 import workload as wl
+    c = wl.CONFIGS[args.config]
+    n_docs = args.docs or c["N"]
+    B = args.queries or c["B"]
+    k = args.k or c["k"]
+    return wl, c, n_docs, B, k
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the oracle timed on the host cores (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------------
+def time_oracle(docs, queries, vocab, k, n_sample: int, steps: int = 1, warmup: int = 0, R_d=None):
+    import oracle
+    cores = oracle.max_threads()
+    n = n_sample or cores
+    n = max(1, min(n, queries.rows))
+    t0 = time.perf_counter()
+    if R_d is None:
+        R_d = oracle.as_rows(docs, vocab)
+    t_rows = time.perf_counter() - t0
+    R_q = oracle.as_rows(queries.slice_rows(0, n), vocab)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle.search(R_q, R_d, k, nthreads=0)
+        if it >= warmup:
+            times.append(time.perf_counter() - t0)
+    dt = float(np.mean(times))
+    return {"value": n / dt, "unit": "queries/s", "cores": min(cores, n), "kind": "oracle",
+            "sample": f"first {n} of {queries.rows} queries against all {docs.rows} docs, exhaustive merge scoring + full sort "
+                      f"(oracle.search, OpenMP over queries); {dt:.2f} s per pass; doc canonicalisation {t_rows:.1f} s not counted",
+            "ms_per_query": 1e3 * dt / n * min(cores, n), "seconds_per_pass": dt}, R_d
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl, c, n_docs, B, k = workload_for(args, 0)
+    docs = wl.make_docs(args.config, n_docs=n_docs)
+    queries = wl.make_queries(args.config, n_queries=B)
+    base, _ = time_oracle(docs, queries, wl.VOCAB, k, args.cpu_sample_queries, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    dt = base["seconds_per_pass"]
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": "queries/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if c["wtype"] == "f32" else "int64", "data": "synthetic",
+            "config": config_dict(args, c, n_docs, B, k, "oracle"),
+            "cpu_baseline": {k_: base[k_] for k_ in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": base["value"], "unit": "queries/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(args, c, n_docs, B, k, algo):
+    return {"workload": f"BASELINE.json configs[2] '{args.config}': V=30522, N={n_docs} docs (nnz~N(120,40) clip [20,400], Zipf s={c['s']}, "
+                        f"LogNormal(0,0.5) {c['wtype']} weights), B={B} queries (nnz~N(25,8) clip [5,64]), top-k={k}, seed 0",
+            "num_docs": n_docs, "batch": B, "k": k, "vocab": 30522, "wtype": c["wtype"], "algo": algo,
+            "l2": "index arrays (GBs) exceed the 126 MB L2; no explicit flush between iterations",
+            "parallelism": "replicas only (no sharding, no collectives)"}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------------
+def timed_steps(torch, dist, fn, steps, warmup, world):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    s = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s)
+    for _ in range(steps):
+        fn()
+    e1.record(s)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback for the hot path"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    from paper_2606_26441_b200 import binding as gs
+    from paper_2606_26441_b200 import build as gsbuild
+    if rank == 0 and not os.path.exists(gs.LIB_PATH):
+        gsbuild.build_all()
+    if world > 1:
+        dist.barrier()
+    gs.lib()
+    wl, c, n_docs, B, k = workload_for(args, rank)
+    dev = torch.device(f"cuda:{local}")
+    peaks = measured_peaks()
+
+    t0 = time.perf_counter()
+    docs = wl.make_docs(args.config, n_docs=n_docs)                  # every replica indexes the same collection
+    queries = wl.make_queries(args.config, n_queries=B, row0=rank * B)   # ... and searches its own batch
+    t_gen = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs)
+    torch.cuda.synchronize()
+    t_build = time.perf_counter() - t0
+    info = ix.info()
+    lens = ix.meta()[1].astype(np.int64)
+    q_dev = [torch.from_numpy(a).to(dev) for a in (queries.indptr, queries.terms, queries.weights)]
+    sdt = torch.float32 if c["wtype"] == "f32" else torch.int32
+    out_ids = torch.empty((B, k), dtype=torch.int32, device=dev)
+    out_sc = torch.empty((B, k), dtype=sdt, device=dev)
+    opt_common = dict(doc_query_tile=args.doc_query_tile, query_group=args.query_group)
+
+    def measure(algo):
+        ws_bytes = ix.workspace_bytes(B, queries.nnz, k, algo=algo, **opt_common)
+        ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+
+        def step():
+            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, **opt_common)
+
+        with ClockSampler(local) as cs:
+            ms = timed_steps(torch, dist, step, args.steps, args.warmup, world)
+        launches = gs.last_launch_count()
+        st = ix.stats(ws)
+        # per-kernel device time, measured live with CUDA events on the launching stream (same K steps again)
+        gs.profile_enable(True)
+        torch.cuda.synchronize()
+        for _ in range(args.steps):
+            step()
+        torch.cuda.synchronize()
+        prof = gs.profile_read()
+        gs.profile_enable(False)
+        res = {"algo": algo, "algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"), "ms_per_step": ms / args.steps,
+               "qps": world * B * args.steps / (ms * 1e-3), "ms_per_query": ms / args.steps / B,
+               "launches_per_step": launches, "candidates_per_query": st["candidates"] / max(B, 1),
+               "overflow_queries": st["overflow_queries"], "workspace_bytes": ws_bytes, "clocks": cs.summary(),
+               "kernels": {n: {"launches_per_step": v["launches"] / args.steps, "ms_per_step": v["ms"] / args.steps}
+                           for n, v in prof.items()}}
+        res["roofline"] = roofline(res, st, info, lens, queries, B, k, peaks, c["wtype"])
+        del ws
+        return res
+
+    main = measure(args.algo)
+    others = {}
+    for a in [x for x in args.also.split(",") if x]:
+        if a != args.algo and a != main["algo_used"]:
+            others[a] = measure(a)
+        elif a == main["algo_used"] and a != args.algo:
+            others[a] = "same as the main line (auto dispatch chose it)"
+
+    # ---- e2e: HOST buffers through gs_search_host (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = [torch.from_numpy(a).pin_memory() for a in (queries.indptr, queries.terms, queries.weights)]
+        h_ids = torch.empty((B, k), dtype=torch.int32).pin_memory()
+        h_sc = torch.empty((B, k), dtype=sdt).pin_memory()
+        pn = [t.numpy() for t in pin]
+
+        def step_host():
+            ix.search_host(pn[0], pn[1], pn[2], k, out_ids=h_ids.numpy(), out_scores=h_sc.numpy(), algo=args.algo, **opt_common)
+
+        for _ in range(args.warmup):
+            step_host()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_host()          # synchronous: returns after the D2H copy of the results
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * B * args.steps / dt, "unit": "queries/s", "ms_per_step": 1e3 * dt / args.steps,
+               "h2d_bytes_per_step": int(sum(a.nbytes for a in pn)), "d2h_bytes_per_step": int(h_ids.numel() * 4 + h_sc.numel() * 4),
+               "api": "gs_search_host (pinned host buffers; H2D + search + D2H + stream sync per step, host wall clock)"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        full, _ = time_oracle(docs, queries, wl.VOCAB, k, args.cpu_sample_queries)
+        cpu = {k_: full[k_] for k_ in ("value", "unit", "cores", "kind", "sample")}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": main["qps"], "unit": "queries/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32" if c["wtype"] == "f32" else "u8", "data": "synthetic",
+                "config": config_dict(args, c, n_docs, B, k, f"{args.algo}->{main['algo_used']}"),
+                "ms_per_query": main["ms_per_query"], "clocks": main["clocks"], "e2e": e2e,
+                "gpu_launches": int(main["launches_per_step"] * args.steps), "roofline": main["roofline"],
+                "cpu_baseline": cpu, "kernels": main["kernels"], "candidates_per_query": main["candidates_per_query"],
+                "overflow_queries": main["overflow_queries"], "other_algos": others,
+                "index": {"postings": info["nnz"], "padded_postings": info["padded_nnz"], "bytes_inverted": info["bytes_inverted"],
+                          "bytes_forward": info["bytes_forward"], "bytes_head": info["bytes_head"],
+                          "bytes_meta": info["bytes_inverted_meta"], "head_terms": info["head_terms"], "tile_docs": info["tile_docs"],
+                          "build_s": t_build, "generate_s": t_gen},
+                "context": {"paper_h100_qps": 787, "paper_h100_doc_parallel_hbm_frac": 0.626,
+                            "note": "paper numbers are H100 + MS MARCO/SPLADE (PAPER.md L292, L340): context, not a baseline"}}
+        print(json.dumps(line), flush=True)
+    ix.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def roofline(res, st, info, lens, queries, B, k, peaks, wtype):
+    """Roofline of the dominant scoring kernel of the step (SURVEY §8d byte models).
+
+    doc-parallel (bound hbm): algorithmic bytes per step = passes * bytes(forward index) * (1 + sample share):
+      the forward index is streamed once per tile of `doc_query_tile` queries (PAPER.md L174 streams it once
+      per QUERY: B*N*kbar*12 bytes); the threshold sample re-reads 1/2^shift of it.
+    term-parallel: algorithmic bytes per step = (4 + w) * U, U = postings of the batch's distinct terms
+      (each read once; the paper's model B*qbar*Lbar*8 of L172 counts them once per query: `bytes_paper_model`).
+      The kernel is bound by shared-memory read-modify-writes, so its `mac_per_s` is reported too.
+    """
+    kern = res["kernels"]
+    name = "score_doc" if res["algo_used"] == "doc" else "score_term"
+    if name not in kern:
+        return None
+    kms, nl = kern[name]["ms_per_step"], kern[name]["launches_per_step"]
+    wb = 4 if wtype == "f32" else 1
+    ntiles = max(info["num_tiles"], 1)
+    share = 1.0 + (st["sample_tiles"] / ntiles if st["sample_tiles"] < ntiles else 0.0)
+    qt = np.asarray(queries.terms)
+    distinct = np.unique(qt[(qt >= 0) & (qt < len(lens))])
+    U = int(lens[distinct].sum())
+    W = int(lens[qt[(qt >= 0) & (qt < len(lens))]].sum())
+    out = {"kernel": name, "kernel_ms_per_step": kms, "launches_per_step": nl, "share_of_step": kms / res["ms_per_step"],
+           "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": None,
+           "useful_mac_per_step": W, "mac_per_s": W / (kms * 1e-3)}
+    if name == "score_doc":
+        passes = st["doc_passes"]
+        alg = passes * info["bytes_forward"] * share
+        out.update({"doc_query_tile": st["doc_query_tile"], "passes": passes,
+                    "bytes_per_step": alg, "bytes_model": "passes*(8*(N+1)+(4+w)*P)*(1+sample share)",
+                    "bytes_one_pass": info["bytes_forward"], "frac_one_pass": info["bytes_forward"] / (kms * 1e-3) / 1e9 / peaks["hbm_gbs"]})
+    else:
+        alg = (4 + wb) * U * share
+        out.update({"query_group": st["query_group"], "bytes_per_step": alg, "bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
+                    "bytes_paper_model": (4 + wb) * W})
+    out["achieved"] = alg / (kms * 1e-3) / 1e9
+    out["frac"] = out["achieved"] / peaks["hbm_gbs"]
+    return out
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -127,6 +127,9 @@ typedef struct gs_stats {
     int32_t launches;          /* kernels launched by the call (host-side count)                       */
     int32_t algo_used;         /* gs_algo_t actually run                                               */
     int32_t sample_tiles;      /* doc tiles scored densely to obtain the thresholds                    */
+    int32_t doc_query_tile;    /* doc-parallel: queries per pass over the forward index (0 otherwise)  */
+    int32_t doc_passes;        /* doc-parallel: passes over the forward index per full-collection launch */
+    int32_t query_group;       /* term-parallel: queries sharing one CTA's accumulator tiles           */
 } gs_stats_t;
 
 /* ------------------------------------------------------------------------------------------------
@@ -187,6 +190,30 @@ GS_API gs_status_t gs_topk_workspace_bytes(int64_t num_rows, int64_t n, int32_t 
 GS_API gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t num_rows, int64_t n, int64_t ld,
                           int32_t k, int32_t* out_ids, void* out_scores, void* workspace,
                           size_t workspace_bytes, gs_stream_t stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Kernel timing (SURVEY §8d measurement): when enabled on the calling thread, every kernel launch of
+ * the following gs_search / gs_score_dense / gs_topk_dense calls is bracketed by CUDA events on the
+ * call's stream; gs_profile_read synchronises those events, returns launch counts and summed device
+ * milliseconds per kernel class, and clears the record.  Off by default (no events are recorded).
+ * ---------------------------------------------------------------------------------------------- */
+#define GS_PROF_CLASSES 8
+typedef enum gs_kclass {
+    GS_K_INGEST = 0,       /* S1  query ingest                                            */
+    GS_K_SCORE_TERM = 1,   /* S2a term-parallel tiled scatter-add (+ head strips)          */
+    GS_K_SCORE_DOC = 2,    /* S2b document-parallel forward-index streaming                */
+    GS_K_QTILE = 3,        /* S1  transposed query tiles of the document-parallel kernel   */
+    GS_K_SELECT = 4,       /* S3  radix select (histogram / scan / collect)                */
+    GS_K_SORT = 5,         /* S3  bitonic finish + decode                                  */
+    GS_K_MISC = 6          /* zeroing, statistics                                          */
+} gs_kclass_t;
+typedef struct gs_profile {
+    int32_t launches[GS_PROF_CLASSES];
+    float ms[GS_PROF_CLASSES];
+} gs_profile_t;
+GS_API void gs_profile_enable(int32_t on);
+GS_API gs_status_t gs_profile_read(gs_profile_t* out);
+GS_API const char* gs_kclass_name(int32_t kclass);
 
 GS_API const char* gs_strerror(gs_status_t status);
 GS_API const char* gs_version(void);

@@ -25,8 +25,9 @@ EXPORTS = [
     "gs_index_build", "gs_index_info", "gs_index_free", "gs_index_copy_meta", "gs_index_copy_list",
     "gs_search_workspace_bytes", "gs_search", "gs_search_host", "gs_search_stats", "gs_score_dense",
     "gs_topk_workspace_bytes", "gs_topk_dense", "gs_strerror", "gs_version", "gs_abi_version",
-    "gs_last_cuda_error", "gs_last_launch_count",
+    "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name",
 ]
+GS_PROF_CLASSES = 8
 
 
 class GsError(RuntimeError):
@@ -60,7 +61,12 @@ class gs_search_opts_t(ctypes.Structure):
 
 class gs_stats_t(ctypes.Structure):
     _fields_ = [("candidates", ctypes.c_int64), ("overflow_queries", ctypes.c_int32), ("launches", ctypes.c_int32),
-                ("algo_used", ctypes.c_int32), ("sample_tiles", ctypes.c_int32)]
+                ("algo_used", ctypes.c_int32), ("sample_tiles", ctypes.c_int32), ("doc_query_tile", ctypes.c_int32),
+                ("doc_passes", ctypes.c_int32), ("query_group", ctypes.c_int32)]
+
+
+class gs_profile_t(ctypes.Structure):
+    _fields_ = [("launches", ctypes.c_int32 * GS_PROF_CLASSES), ("ms", ctypes.c_float * GS_PROF_CLASSES)]
 
 
 _lib_handle = None
@@ -93,6 +99,11 @@ def lib():
         L.gs_strerror.argtypes = [ctypes.c_int]
         L.gs_strerror.restype = ctypes.c_char_p
         L.gs_version.restype = ctypes.c_char_p
+        L.gs_profile_enable.argtypes = [i32]
+        L.gs_profile_enable.restype = None
+        L.gs_profile_read.argtypes = [P(gs_profile_t)]
+        L.gs_kclass_name.argtypes = [i32]
+        L.gs_kclass_name.restype = ctypes.c_char_p
         for name in EXPORTS:
             getattr(L, name)            # every symbol the header declares must be exported
         _lib_handle = L
@@ -114,6 +125,24 @@ def version() -> str:
 
 def last_launch_count() -> int:
     return int(lib().gs_last_launch_count())
+
+
+def profile_enable(on: bool) -> None:
+    """gs_profile_enable: bracket every kernel launch of this thread's following calls with CUDA events."""
+    lib().gs_profile_enable(1 if on else 0)
+
+
+def profile_read() -> dict:
+    """gs_profile_read -> {kernel class: {"launches": n, "ms": summed device time}} (clears the record)."""
+    L = lib()
+    pr = gs_profile_t()
+    _check(L.gs_profile_read(ctypes.byref(pr)))
+    out = {}
+    for c in range(GS_PROF_CLASSES):
+        name = L.gs_kclass_name(c).decode()
+        if name and pr.launches[c]:
+            out[name] = {"launches": int(pr.launches[c]), "ms": float(pr.ms[c])}
+    return out
 
 
 def _torch():

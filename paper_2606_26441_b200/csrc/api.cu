@@ -26,6 +26,32 @@ thread_local int32_t gs_tls_launches = 0;
 static thread_local int32_t tls_cuda_error = 0;
 void gs_set_cuda_error(cudaError_t e) { tls_cuda_error = (int32_t)e; cudaGetLastError(); }
 
+// ---- kernel timing (gs_profile_*): thread-local list of event pairs
+namespace {
+struct ProfRec { int kclass; int n; cudaEvent_t a, b; };
+thread_local bool tls_prof_on = false;
+thread_local std::vector<ProfRec> tls_prof;
+thread_local std::vector<cudaEvent_t> tls_event_pool;
+cudaEvent_t prof_event() {
+    if (!tls_event_pool.empty()) { cudaEvent_t e = tls_event_pool.back(); tls_event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return e;
+}
+}  // namespace
+
+GsProfScope::GsProfScope(int kclass, cudaStream_t s, int n) : stream(s) {
+    if (!tls_prof_on) return;
+    ProfRec r{kclass, n, prof_event(), prof_event()};
+    if (!r.a || !r.b) return;
+    cudaEventRecord(r.a, s);
+    tls_prof.push_back(r);
+    slot = (int)tls_prof.size() - 1;
+}
+GsProfScope::~GsProfScope() {
+    if (slot >= 0) cudaEventRecord(tls_prof[slot].b, stream);
+}
+
 namespace {
 
 inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
@@ -62,8 +88,10 @@ gs_status_t check_csr_host(const gs_csr_t* c, bool device) {
 // device-side stats block at the start of every search workspace
 struct StatsBlock { gs_stats_t stats; int32_t status; int32_t n_overflow; };
 
+struct PlanStats { int32_t launches, algo, sample_tiles, qtile, passes, group; };
+
 __global__ void k_finalize_stats(StatsBlock* sb, const uint32_t* cand_cnt, int64_t B, int64_t cap, int32_t* overflow_list,
-                                 int32_t launches, int32_t algo, int32_t sample_tiles) {
+                                 PlanStats ps) {
     __shared__ unsigned long long tot;
     __shared__ int n_ov;
     if (threadIdx.x == 0) { tot = 0; n_ov = 0; }
@@ -79,9 +107,12 @@ __global__ void k_finalize_stats(StatsBlock* sb, const uint32_t* cand_cnt, int64
     if (threadIdx.x == 0) {
         sb->stats.candidates = (int64_t)tot;
         sb->stats.overflow_queries = n_ov;
-        sb->stats.launches = launches;
-        sb->stats.algo_used = algo;
-        sb->stats.sample_tiles = sample_tiles;
+        sb->stats.launches = ps.launches;
+        sb->stats.algo_used = ps.algo;
+        sb->stats.sample_tiles = ps.sample_tiles;
+        sb->stats.doc_query_tile = ps.qtile;
+        sb->stats.doc_passes = ps.passes;
+        sb->stats.query_group = ps.group;
         sb->n_overflow = n_ov;
     }
 }
@@ -123,6 +154,20 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
     }
     (void)B;
     return p;
+}
+
+PlanStats plan_stats(const gs_index* ix, const Plan& p, int64_t B, int32_t sample_tiles) {
+    PlanStats ps{};
+    ps.launches = gs_tls_launches + 1;
+    ps.algo = p.algo;
+    ps.sample_tiles = sample_tiles;
+    if (p.algo == GS_ALGO_DOC_PARALLEL) {
+        ps.qtile = gs_score_doc_qtile(p.qtile);
+        ps.passes = (int32_t)((B + ps.qtile - 1) / ps.qtile);
+    } else {
+        ps.group = gs_score_term_group(ix, B, p.group);
+    }
+    return ps;
 }
 
 struct Carve {
@@ -210,7 +255,10 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
 
     if (p.dense_only) {
         GS_TRY(dense_topk(ix, p, q, c, 0, B, k, out_ids, out_scores, s));
-        k_finalize_stats<<<1, 256, 0, s>>>(c.sb, nullptr, B, 0, c.overflow_list, gs_tls_launches + 1, p.algo, ix->ntiles);
+        {
+            GsProfScope ps(GS_K_MISC, s);
+            k_finalize_stats<<<1, 256, 0, s>>>(c.sb, nullptr, B, 0, c.overflow_list, plan_stats(ix, p, B, ix->ntiles));
+        }
         ++gs_tls_launches;
         GS_CUDA(cudaGetLastError());
         return GS_OK;
@@ -233,7 +281,10 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
         GS_TRY(gs_launch_select(src, n, k, nullptr, nullptr, c.thr + a, nullptr, nullptr, 0, c.sel_scratch, s));
     }
     // ---- 2. filter: all tiles, emit key >= bound
-    k_zero_u32<<<(unsigned)((B + 255) / 256), 256, 0, s>>>(c.cand_cnt, B);
+    {
+        GsProfScope ps(GS_K_MISC, s);
+        k_zero_u32<<<(unsigned)((B + 255) / 256), 256, 0, s>>>(c.cand_cnt, B);
+    }
     ++gs_tls_launches;
     {
         gs_tileset all{0, 1, ix->ntiles};
@@ -247,8 +298,11 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
         src.keys = c.cand; src.cap = p.cand_cap; src.counts = c.cand_cnt; src.wtype = ix->wtype;
         GS_TRY(gs_launch_select(src, B, k, out_ids, out_scores, nullptr, nullptr, nullptr, 0, c.sel_scratch, s));
     }
-    k_finalize_stats<<<1, 256, 0, s>>>(c.sb, c.cand_cnt, B, p.cand_cap, c.overflow_list, gs_tls_launches + 1, p.algo,
-                                       p.sample_tiles);
+    {
+        GsProfScope ps(GS_K_MISC, s);
+        k_finalize_stats<<<1, 256, 0, s>>>(c.sb, c.cand_cnt, B, p.cand_cap, c.overflow_list,
+                                           plan_stats(ix, p, B, p.sample_tiles));
+    }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     // ---- 4. overflowed candidate lists -> dense fallback for those queries (needs the count on the host)
@@ -481,6 +535,45 @@ gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t rows, int64
     gs_sel_src src{};
     src.dense = (const uint32_t*)scores; src.ld = ld; src.n_cols = n; src.n_docs = n; src.Ts = 0; src.wtype = wtype;
     return gs_launch_select(src, rows, k, out_ids, out_scores, nullptr, nullptr, nullptr, 0, ws, (cudaStream_t)stream);
+}
+
+void gs_profile_enable(int32_t on) {
+    tls_prof_on = on != 0;
+    for (ProfRec& r : tls_prof) { tls_event_pool.push_back(r.a); tls_event_pool.push_back(r.b); }
+    tls_prof.clear();
+}
+
+gs_status_t gs_profile_read(gs_profile_t* out) {
+    if (!out) return GS_ERR_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    gs_status_t st = GS_OK;
+    for (ProfRec& r : tls_prof) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess) {
+            gs_set_cuda_error(cudaGetLastError());
+            st = GS_ERR_CUDA;
+        } else if (r.kclass >= 0 && r.kclass < GS_PROF_CLASSES) {
+            out->launches[r.kclass] += r.n;
+            out->ms[r.kclass] += ms;
+        }
+        tls_event_pool.push_back(r.a);
+        tls_event_pool.push_back(r.b);
+    }
+    tls_prof.clear();
+    return st;
+}
+
+const char* gs_kclass_name(int32_t k) {
+    switch (k) {
+        case GS_K_INGEST: return "ingest";
+        case GS_K_SCORE_TERM: return "score_term";
+        case GS_K_SCORE_DOC: return "score_doc";
+        case GS_K_QTILE: return "build_qtile";
+        case GS_K_SELECT: return "radix_select";
+        case GS_K_SORT: return "bitonic_sort";
+        case GS_K_MISC: return "misc";
+    }
+    return "";
 }
 
 const char* gs_strerror(gs_status_t st) {

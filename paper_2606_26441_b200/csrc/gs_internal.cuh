@@ -125,11 +125,25 @@ struct gs_sink {
 // ------------------------------------------------------------------------------------------------
 extern thread_local int32_t gs_tls_launches;
 
+// Brackets the launches issued during its lifetime with CUDA events when gs_profile_enable(1) is set
+// on the calling thread (no-op otherwise).  `n` = kernels launched inside the scope.
+struct GsProfScope {
+    GsProfScope(int kclass, cudaStream_t s, int n = 1);
+    ~GsProfScope();
+    GsProfScope(const GsProfScope&) = delete;
+    GsProfScope& operator=(const GsProfScope&) = delete;
+    int slot = -1;
+    cudaStream_t stream = nullptr;
+};
+
 gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head,
                              gs_qbatch* qb, cudaStream_t s);
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
+
+int gs_score_term_group(const gs_index* ix, int64_t nq, int group);   // queries per CTA actually used
+int gs_score_doc_qtile(int qtile);                                    // queries per pass actually used
 
 // doc-parallel: scratch holds the transposed query tile(s)
 size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, int64_t q_nnz);

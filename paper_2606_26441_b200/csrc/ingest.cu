@@ -68,6 +68,7 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     if (B == 0) return GS_OK;
     const int threads = 128;
     const unsigned grid = (unsigned)((B * 32 + threads - 1) / threads);
+    GsProfScope ps(GS_K_INGEST, s);
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
                                                    use_head && ix->H > 0, validate, qb->head_w, qb->tail_term,

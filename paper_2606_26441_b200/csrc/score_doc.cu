@@ -240,7 +240,10 @@ int norm_qt(int qtile) {
 template <int WT, int QT>
 gs_status_t launch_doc(const DocParams& p, unsigned grid, size_t smem, cudaStream_t s) {
     GS_CUDA(cudaFuncSetAttribute(k_score_doc<WT, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_score_doc<WT, QT><<<grid, kThreads, smem, s>>>(p);
+    {
+        GsProfScope ps(GS_K_SCORE_DOC, s);
+        k_score_doc<WT, QT><<<grid, kThreads, smem, s>>>(p);
+    }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;
@@ -259,6 +262,8 @@ gs_status_t launch_doc_qt(int QT, const DocParams& p, unsigned grid, size_t smem
 
 // rows capacity of one scratch tile: every distinct term of the batch could fall in one tile
 static int64_t rows_cap_for(const gs_index* ix, int64_t q_nnz) { return std::min<int64_t>(ix->V, q_nnz) + 1; }
+
+int gs_score_doc_qtile(int qtile) { return norm_qt(qtile); }
 
 size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, int64_t q_nnz) {
     const int QT = norm_qt(qtile);
@@ -281,6 +286,7 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
     {   // build all query tiles of this chunk in one launch
         const size_t bsm = sizeof(uint32_t) * (size_t)ix->V;
         if (bsm > (size_t)smem_max) return GS_ERR_OUT_OF_RANGE;
+        GsProfScope ps(GS_K_QTILE, s);
         if (ix->wtype == GS_W_F32) {
             GS_CUDA(cudaFuncSetAttribute(k_build_qtile<GS_W_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
             k_build_qtile<GS_W_F32><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, q0, nq, QT, ix->V,

@@ -156,7 +156,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_score_term(const TermParams p) 
 template <int WT, bool HEAD>
 gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
     GS_CUDA(cudaFuncSetAttribute(k_score_term<WT, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_score_term<WT, HEAD><<<grid, kThreads, smem, s>>>(p);
+    {
+        GsProfScope ps(GS_K_SCORE_TERM, s);
+        k_score_term<WT, HEAD><<<grid, kThreads, smem, s>>>(p);
+    }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;
@@ -164,16 +167,23 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t
 
 }  // namespace
 
+static int max_cells_for(const gs_index* ix) {
+    const size_t budget = 200 * 1024;   // shared memory for accumulators + head weights
+    return (int)(budget / ((size_t)ix->Ts * 4 + GS_HEAD_MAX * 4));
+}
+int gs_score_term_group(const gs_index* ix, int64_t nq, int group) {
+    int G = group > 0 ? group : (int)std::min<int64_t>(nq, 1 << 20);
+    return (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(G, nq), max_cells_for(ix)));
+}
+
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     const bool head = use_head && ix->H > 0;
     // cells per CTA: bounded by shared memory (accumulators + head weights)
-    const size_t budget = 200 * 1024;
-    const int max_cells = (int)((budget) / ((size_t)ix->Ts * 4 + GS_HEAD_MAX * 4));
-    int G = group > 0 ? group : (int)nq;
-    G = (int)std::min<int64_t>(std::min<int64_t>(G, nq), max_cells);
-    if (G < 1) return GS_ERR_OOM;
+    const int max_cells = max_cells_for(ix);
+    if (max_cells < 1) return GS_ERR_OOM;
+    const int G = gs_score_term_group(ix, nq, group);
     int m = std::max(1, std::min(max_cells / G, kWarps / std::min(G, kWarps)));
     m = std::min(m, ts.count);
     TermParams p{};

@@ -233,20 +233,27 @@ gs_status_t run_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* 
     const int64_t max_items = src.keys ? src.cap : src.n_cols;
     const unsigned chunks = (unsigned)std::max<int64_t>(1, (max_items + kItemsPerCta - 1) / kItemsPerCta);
     if (rows > 65535) return GS_ERR_OUT_OF_RANGE;
-    k_sel_init<<<(unsigned)rows, 256, 0, s>>>(src, rows, k, sc.st, sc.hist);
-    ++gs_tls_launches;
-    for (int shift = 64; shift > 0; shift -= GS_SEL_BITS) {
-        k_sel_hist<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, sc.hist);
-        k_sel_scan<<<(unsigned)rows, GS_SEL_BINS / 4, 0, s>>>(sc.st, sc.hist);
-        gs_tls_launches += 2;
+    {
+        GsProfScope ps(GS_K_SELECT, s, 14);
+        k_sel_init<<<(unsigned)rows, 256, 0, s>>>(src, rows, k, sc.st, sc.hist);
+        ++gs_tls_launches;
+        for (int shift = 64; shift > 0; shift -= GS_SEL_BITS) {
+            k_sel_hist<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, sc.hist);
+            k_sel_scan<<<(unsigned)rows, GS_SEL_BINS / 4, 0, s>>>(sc.st, sc.hist);
+            gs_tls_launches += 2;
+        }
+        k_sel_collect<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, k, sc.sel);
+        ++gs_tls_launches;
     }
-    k_sel_collect<WT><<<dim3(chunks, (unsigned)rows), kSelThreads, 0, s>>>(src, sc.st, k, sc.sel);
     int kp2 = 32;
     while (kp2 < k) kp2 <<= 1;
     const int threads = std::min(1024, std::max(32, kp2));
-    k_sel_sort<WT><<<(unsigned)rows, threads, (size_t)kp2 * 8, s>>>(sc.st, sc.sel, k, kp2, out_ids, (uint32_t*)out_scores,
-                                                                   out_thr, out_keys, out_cnt, out_cap);
-    gs_tls_launches += 2;
+    {
+        GsProfScope ps(GS_K_SORT, s);
+        k_sel_sort<WT><<<(unsigned)rows, threads, (size_t)kp2 * 8, s>>>(sc.st, sc.sel, k, kp2, out_ids, (uint32_t*)out_scores,
+                                                                       out_thr, out_keys, out_cnt, out_cap);
+    }
+    ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;
 }
