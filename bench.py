@@ -339,32 +339,30 @@ def roofline(res, st, info, lens, queries, B, k, peaks, wtype):
       (each read once; the paper's model B*qbar*Lbar*8 of L172 counts them once per query: `bytes_paper_model`).
       The kernel is bound by shared-memory read-modify-writes, so its `mac_per_s` is reported too.
     """
+    from paper_2606_26441_b200 import roofline as rf
     kern = res["kernels"]
     name = "score_doc" if res["algo_used"] == "doc" else "score_term"
     if name not in kern:
         return None
     kms, nl = kern[name]["ms_per_step"], kern[name]["launches_per_step"]
-    wb = 4 if wtype == "f32" else 1
     ntiles = max(info["num_tiles"], 1)
-    share = 1.0 + (st["sample_tiles"] / ntiles if st["sample_tiles"] < ntiles else 0.0)
-    qt = np.asarray(queries.terms)
-    distinct = np.unique(qt[(qt >= 0) & (qt < len(lens))])
-    U = int(lens[distinct].sum())
-    W = int(lens[qt[(qt >= 0) & (qt < len(lens))]].sum())
+    share = st["sample_tiles"] / ntiles if st["sample_tiles"] < ntiles else 0.0
+    ts = rf.batch_term_stats(lens, queries.terms)
     out = {"kernel": name, "kernel_ms_per_step": kms, "launches_per_step": nl, "share_of_step": kms / res["ms_per_step"],
            "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": None,
-           "useful_mac_per_step": W, "mac_per_s": W / (kms * 1e-3)}
+           "useful_mac_per_step": ts["W"], "mac_per_s": ts["W"] / (kms * 1e-3)}
     if name == "score_doc":
-        passes = st["doc_passes"]
-        alg = passes * info["bytes_forward"] * share
-        out.update({"doc_query_tile": st["doc_query_tile"], "passes": passes,
-                    "bytes_per_step": alg, "bytes_model": "passes*(8*(N+1)+(4+w)*P)*(1+sample share)",
-                    "bytes_one_pass": info["bytes_forward"], "frac_one_pass": info["bytes_forward"] / (kms * 1e-3) / 1e9 / peaks["hbm_gbs"]})
+        alg = rf.doc_parallel_bytes(info["num_docs"], info["nnz"], wtype, B, st["doc_query_tile"], share)
+        one = rf.forward_index_bytes(info["num_docs"], info["nnz"], wtype)
+        out.update({"doc_query_tile": st["doc_query_tile"], "passes": st["doc_passes"], "bytes_per_step": alg,
+                    "bytes_model": "passes*(8*(N+1)+(4+w)*P)*(1+sample share)", "bytes_one_pass": one,
+                    "frac_one_pass": rf.effective_gbps(one, kms) / peaks["hbm_gbs"]})
     else:
-        alg = (4 + wb) * U * share
-        out.update({"query_group": st["query_group"], "bytes_per_step": alg, "bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
-                    "bytes_paper_model": (4 + wb) * W})
-    out["achieved"] = alg / (kms * 1e-3) / 1e9
+        alg = rf.term_parallel_bytes(ts["U"], wtype, share)
+        out.update({"query_group": st["query_group"], "bytes_per_step": alg,
+                    "bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
+                    "bytes_paper_model": rf.term_parallel_bytes(ts["W"], wtype)})
+    out["achieved"] = rf.effective_gbps(alg, kms)
     out["frac"] = out["achieved"] / peaks["hbm_gbs"]
     return out
 

@@ -1,0 +1,42 @@
+"""The byte-accounting conventions of paper_2606_26441_b200/roofline.py against the numbers the paper prints
+(tests/golden/paper_byte_models.json: PAPER.md L172-181 and Table 7).  CPU only."""
+import json
+import os
+
+import numpy as np
+
+from paper_2606_26441_b200 import roofline as rf
+
+G = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "paper_byte_models.json")))
+
+
+def test_paper_scatter_model():
+    assert abs(rf.paper_scatter_entries_per_query(G["q_bar"], G["L_bar"]) - G["scatter_entries_per_query"]) <= G["scatter_entries_tol"]
+    gb = rf.paper_scatter_bytes(G["B"], G["q_bar"], G["L_bar"]) / 1e9
+    assert abs(gb - G["scatter_bytes_GB"]) <= G["scatter_bytes_tol_GB"]
+    gbps = rf.effective_gbps(rf.paper_scatter_bytes(G["B"], G["q_bar"], G["L_bar"]), G["scatter_ms"])
+    assert abs(gbps - G["scatter_GBps"]) <= G["scatter_GBps_tol"]
+    assert abs(100 * gbps / G["h100_peak_GBps"] - G["scatter_pct"]) <= G["scatter_pct_tol"]
+
+
+def test_paper_doc_parallel_model():
+    assert rf.paper_doc_entries_per_query(G["N"], G["k_bar_model"]) == G["doc_entries_per_query"]
+    b = rf.paper_doc_bytes(G["B"], G["N"], G["k_bar_measured"])
+    assert abs(b / 1e9 - G["doc_bytes_GB"]) <= G["doc_bytes_tol_GB"]
+    gbps = rf.effective_gbps(b, G["doc_ms"])
+    assert abs(gbps - G["doc_GBps"]) <= G["doc_GBps_tol"]
+    assert abs(100 * gbps / G["h100_peak_GBps"] - G["doc_pct"]) <= G["doc_pct_tol"]
+    ratio = rf.paper_doc_entries_per_query(G["N"], G["k_bar_model"]) / rf.paper_scatter_entries_per_query(G["q_bar"], G["L_bar"])
+    assert abs(ratio - G["work_ratio"]) <= G["work_ratio_tol"]
+
+
+def test_our_models_closed_forms():
+    L = np.array([10, 0, 7, 3], np.int64)
+    q_terms = np.array([0, 2, 2, 3, 9, -1], np.int32)           # out-of-range ids contribute nothing
+    st = rf.batch_term_stats(L, q_terms)
+    assert st == {"U": 20, "W": 27, "distinct_terms": 3}
+    assert rf.term_parallel_bytes(20, "f32") == 160 and rf.term_parallel_bytes(20, "u8") == 100
+    assert rf.forward_index_bytes(3, 7, "f32") == 8 * 4 + 8 * 7
+    assert rf.forward_index_bytes(3, 7, "u8") == 8 * 4 + 5 * 7
+    assert rf.doc_parallel_bytes(3, 7, "f32", B=500, query_tile=16) == 32 * (32 + 56)
+    assert rf.doc_parallel_bytes(3, 7, "f32", B=1, query_tile=16, sample_share=0.5) == 1.5 * 88
