@@ -165,7 +165,7 @@ PlanStats plan_stats(const gs_index* ix, const Plan& p, int64_t B, int32_t sampl
         ps.qtile = gs_score_doc_qtile(p.qtile);
         ps.passes = (int32_t)((B + ps.qtile - 1) / ps.qtile);
     } else {
-        ps.group = gs_score_term_group(ix, B, p.group);
+        ps.group = gs_score_term_group(ix, B, p.group, p.use_head);
     }
     return ps;
 }
@@ -182,7 +182,8 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
     size_t off = 0;
     auto take = [&](size_t bytes) { void* r = base ? base + off : nullptr; off += up256(bytes); return r; };
     c.sb = (StatsBlock*)take(sizeof(StatsBlock));
-    c.qb.head_w = (uint32_t*)take((size_t)B * GS_HEAD_MAX * 4);
+    c.qb.head_pair = (uint2*)take((size_t)B * GS_HEAD_MAX * 8);
+    c.qb.head_cnt = (int32_t*)take((size_t)B * 4);
     c.qb.tail_term = (int32_t*)take((size_t)nnz * 4);
     c.qb.tail_w = (uint32_t*)take((size_t)nnz * 4);
     c.qb.tail_cnt = (int32_t*)take((size_t)B * 4);

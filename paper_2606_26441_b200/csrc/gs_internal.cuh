@@ -89,14 +89,15 @@ __device__ __forceinline__ uint32_t gs_ord_bits(uint32_t bits) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Query batch after ingest (S1): per-query dense head weights + compacted tail term lists.
+// Query batch after ingest (S1): per-query compact head-term lists + compacted tail term lists.
 // Accumulator type: float (GS_W_F32) or int32 (GS_W_U8), both 4 bytes, stored as uint32 bit patterns.
 // ------------------------------------------------------------------------------------------------
 struct gs_qbatch {
     int64_t B = 0;
     int64_t nnz = 0;
     const int64_t* indptr = nullptr;   // caller's CSR indptr (device)
-    uint32_t* head_w = nullptr;        // [B][GS_HEAD_MAX] accumulator-typed weights, 0 if absent
+    uint2* head_pair = nullptr;        // [B][GS_HEAD_MAX] compact (strip number, accumulator-typed weight bits)
+    int32_t* head_cnt = nullptr;       // [B] number of head terms of the query
     int32_t* tail_term = nullptr;      // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]
     uint32_t* tail_w = nullptr;        // [nnz] accumulator-typed
     int32_t* tail_cnt = nullptr;       // [B]
@@ -142,7 +143,7 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
 
-int gs_score_term_group(const gs_index* ix, int64_t nq, int group);   // queries per CTA actually used
+int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head);   // queries per CTA actually used
 int gs_score_doc_qtile(int qtile);                                    // queries per pass actually used
 
 // doc-parallel: scratch holds the transposed query tile(s)

@@ -222,6 +222,8 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
 
     std::vector<int32_t> order;
     int hmax = o.head_max < 0 ? 0 : (o.head_max == 0 ? GS_HEAD_MAX : std::min(o.head_max, GS_HEAD_MAX));
+    // the tile's strips are staged in shared memory next to the accumulator rows (score_term.cu)
+    hmax = std::max(0, std::min(hmax, (int)(200 * 1024 / (4 * (size_t)ix->Ts)) - 8));
     float dens = o.head_density > 0.f ? o.head_density : 0.5f;
     for (int32_t t = 0; t < V; ++t)
         if (N > 0 && (double)h_len[t] >= (double)dens * (double)N && h_len[t] > 0) order.push_back(t);

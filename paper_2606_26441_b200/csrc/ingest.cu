@@ -2,7 +2,7 @@
 //
 // The paper pads queries to a [B, M] matrix of (term id, weight) in Python (PAPER.md L120-123,
 // L146-152).  Here one warp per query splits its terms into
-//   * head terms (lists kept as dense strips): weights go into a dense row head_w[b][32];
+//   * head terms (lists kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
 //   * tail terms: compacted (row b starts at indptr[b]) into tail_term/tail_w, weights converted to the
 //     accumulator type (float, or int32 for uint8 impacts).
 // Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
@@ -14,15 +14,14 @@ namespace {
 template <int WT>
 __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
                          const void* __restrict__ weights, int64_t B, int32_t V, const int16_t* __restrict__ head_slot,
-                         int use_head, int validate, uint32_t* __restrict__ head_w, int32_t* __restrict__ tail_term,
+                         int use_head, int validate, uint2* __restrict__ head_pair, int32_t* __restrict__ head_cnt,
+                         int32_t* __restrict__ tail_term,
                          uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, int32_t* __restrict__ status) {
     const int lane = threadIdx.x & 31;
     const int64_t b = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     if (b >= B) return;
     const int64_t a = indptr[b], e = indptr[b + 1];
-    head_w[b * GS_HEAD_MAX + lane] = 0u;
-    __syncwarp();
-    int32_t n_tail = 0;
+    int32_t n_tail = 0, n_head = 0;
     for (int64_t i0 = a; i0 < e; i0 += 32) {
         const int64_t i = i0 + lane;
         int32_t t = -1;
@@ -45,7 +44,15 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
             }
         }
         int slot = (ok && use_head) ? (int)head_slot[t] : -1;
-        if (ok && slot >= 0) head_w[b * GS_HEAD_MAX + slot] = w;
+        const bool is_head = ok && slot >= 0;
+        const unsigned mh = __ballot_sync(0xFFFFFFFFu, is_head);
+        if (is_head) {
+            // a valid row holds each head term at most once, so the list never exceeds GS_HEAD_MAX entries;
+            // the bound only protects memory when a (non-validated) row repeats a term
+            const int dst = n_head + __popc(mh & ((1u << lane) - 1u));
+            if (dst < GS_HEAD_MAX) head_pair[b * GS_HEAD_MAX + dst] = make_uint2((uint32_t)slot, w);
+        }
+        n_head = min(GS_HEAD_MAX, n_head + __popc(mh));
         const bool is_tail = ok && slot < 0;
         const unsigned m = __ballot_sync(0xFFFFFFFFu, is_tail);
         if (is_tail) {
@@ -56,7 +63,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
         n_tail += __popc(m);
         __syncwarp();
     }
-    if (lane == 0) tail_cnt[b] = n_tail;
+    if (lane == 0) { tail_cnt[b] = n_tail; head_cnt[b] = n_head; }
 }
 
 }  // namespace
@@ -71,11 +78,11 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     GsProfScope ps(GS_K_INGEST, s);
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                   use_head && ix->H > 0, validate, qb->head_w, qb->tail_term,
+                                                   use_head && ix->H > 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                    qb->tail_w, qb->tail_cnt, qb->status);
     else
         k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                  use_head && ix->H > 0, validate, qb->head_w, qb->tail_term,
+                                                  use_head && ix->H > 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                   qb->tail_w, qb->tail_cnt, qb->status);
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());

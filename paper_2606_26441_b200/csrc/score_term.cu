@@ -3,38 +3,49 @@
 // PAPER.md Eq. (5): scores[d] += w_i * PL(t_i)[d] for all d in PL(t_i), one independent
 // scatter per query term; the paper launches one program per (query, term) that atomically adds
 // into a global [B,N] buffer (L118-125, L137-172) and names "scattered atomics" as the cost
-// (L172, L411).  Here the doc-id axis is cut into tiles of Ts docs; a CTA owns a block of
-// (query, doc-tile) cells whose accumulators live in SHARED memory; each cell is owned by exactly
-// one warp, so accumulation is plain LDS/FFMA/STS in a fixed order (no atomics, deterministic),
-// and the per-(term, tile) segment table turns "the part of PL(t) inside this tile" into two loads.
-// Posting slices are read with aligned, coalesced 128-byte warp loads (lists are padded to 32).
+// (L172, L411).  Here the doc-id axis is cut into tiles of Ts docs and a CTA owns one doc tile x a
+// group of G queries; its G x Ts accumulators live in SHARED memory.
 //
-// Lists stored as dense strips ("head" terms, >= half of all docs) are not scattered: thread d of
-// the epilogue keeps the strip values of its document in registers and adds the dot product with
-// the query's dense head weights (read through shared-memory broadcasts).
+//   phase 1 (scatter, "tail" lists): a warp takes whole accumulator rows (queries) off a shared
+//     counter, so a row is only ever touched by one warp: plain LDS/FFMA/STS, no atomics, fixed
+//     order.  The per-(term, tile) segment table turns "the part of PL(t) inside this tile" into two
+//     loads, probed for 32 query terms at once (one per lane); only non-empty segments are visited,
+//     and each is streamed with coalesced loads, several independent 32-posting chunks in flight.
+//   phase 2 (epilogue, "head" lists): the <= 32 densest lists are stored as dense strips; the tile's
+//     strips are staged in shared memory once per CTA and every thread owns 4 consecutive documents
+//     of one query: 128-bit shared loads of the accumulators and of the strip of every head term
+//     the query actually contains (per-query compact lists), then the finished cells go to the sink
+//     (dense score matrix, or threshold filter -> candidate list).
 #include <algorithm>
 
 #include "gs_internal.cuh"
 
 namespace {
 
-constexpr int kThreads = 512;
-constexpr int kWarps = kThreads / 32;
+constexpr int kMaxThreads = 1024;
 
 template <int WT> struct Num;
 template <> struct Num<GS_W_F32> {
     using W = float;
     using A = float;
     static __device__ __forceinline__ A qw(uint32_t bits) { return __uint_as_float(bits); }
-    static __device__ __forceinline__ A mac(A acc, A q, W w) { return fmaf(q, w, acc); }
+    static __device__ __forceinline__ A from_bits(int bits) { return __int_as_float(bits); }
+    static __device__ __forceinline__ A mac(A acc, A q, A w) { return fmaf(q, w, acc); }
+    static __device__ __forceinline__ A widen(W w) { return w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return __float_as_uint(a); }
+    static __device__ __forceinline__ bool below(A s, uint32_t thr_ord) {
+        return s < __uint_as_float(gs_unord_f32(thr_ord));      // false for a NaN threshold (thr_ord == 0: accept all)
+    }
 };
 template <> struct Num<GS_W_U8> {
     using W = uint8_t;
     using A = int32_t;
     static __device__ __forceinline__ A qw(uint32_t bits) { return (int32_t)bits; }
-    static __device__ __forceinline__ A mac(A acc, A q, W w) { return acc + q * (int32_t)w; }
+    static __device__ __forceinline__ A from_bits(int bits) { return bits; }
+    static __device__ __forceinline__ A mac(A acc, A q, A w) { return acc + q * w; }
+    static __device__ __forceinline__ A widen(W w) { return (int32_t)w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return (uint32_t)a; }
+    static __device__ __forceinline__ bool below(A s, uint32_t thr_ord) { return s < (int32_t)(thr_ord ^ 0x80000000u); }
 };
 
 struct TermParams {
@@ -42,123 +53,212 @@ struct TermParams {
     const int64_t* inv_off; const int32_t* inv_doc; const void* inv_w; const uint32_t* seg;
     const void* head_strip; int32_t H; int64_t N; int64_t N_pad; int32_t Ts; int32_t ntiles;
     // queries
-    const int64_t* q_indptr; const uint32_t* head_w; const int32_t* tail_term; const uint32_t* tail_w;
-    const int32_t* tail_cnt;
+    const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
+    const uint32_t* tail_w; const int32_t* tail_cnt;
     int64_t q0; int32_t nq; int32_t G;          // queries [q0, q0+nq), G per CTA
     int32_t n_qgroups;
-    // tiles
-    gs_tileset ts; int32_t m;                   // m tiles of the set per CTA
+    gs_tileset ts;
     gs_sink sink;
+    int32_t vec4;                               // dense sink rows are 16-byte aligned
 };
 
+// one posting-list segment [dp, dp+n) applied to one accumulator row
 template <int WT>
-__device__ __forceinline__ void emit(const TermParams& p, int64_t b, int32_t col, int32_t doc,
-                                     typename Num<WT>::A s) {
-    const uint32_t bits = Num<WT>::bits(s);
-    if (p.sink.thr == nullptr) {
-        p.sink.dense[(b - p.q0) * p.sink.ld + col] = bits;
-    } else {
-        const uint64_t key = gs_make_key(gs_ord_bits<WT>(bits), (uint32_t)doc);
-        if (key >= p.sink.thr[b]) {
-            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
-            if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
+__device__ __forceinline__ void scatter_segment(const int32_t* __restrict__ dp, const typename Num<WT>::W* __restrict__ wp,
+                                                int n, typename Num<WT>::A q, typename Num<WT>::A* row, int32_t base,
+                                                int32_t Ts, int lane) {
+    using A = typename Num<WT>::A;
+    if (n <= 32) {
+        if (lane < n) {
+            const int32_t rel = dp[lane] - base;
+            const A w = Num<WT>::widen(wp[lane]);
+            if ((uint32_t)rel < (uint32_t)Ts) row[rel] = Num<WT>::mac(row[rel], q, w);
         }
+        return;
+    }
+    for (int c = lane; c < n; c += 128) {
+        int32_t rel[4];
+        A w[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int i = c + 32 * u;
+            const bool ok = i < n;
+            rel[u] = ok ? dp[i] - base : -1;
+            w[u] = ok ? Num<WT>::widen(wp[i]) : A(0);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if ((uint32_t)rel[u] < (uint32_t)Ts) row[rel[u]] = Num<WT>::mac(row[rel[u]], q, w[u]);
     }
 }
 
-template <int WT, bool HEAD>
-__global__ void __launch_bounds__(kThreads, 1) k_score_term(const TermParams p) {
+template <int WT>
+__device__ __forceinline__ void emit_candidate(const gs_sink& sink, int64_t b, uint64_t thr, int32_t doc,
+                                               typename Num<WT>::A s) {
+    const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(s)), (uint32_t)doc);
+    if (key >= thr) {
+        const uint32_t pos = atomicAdd(&sink.cand_cnt[b], 1u);
+        if ((int64_t)pos < sink.cand_cap) sink.cand[b * sink.cand_cap + pos] = key;
+    }
+}
+
+template <int WT>
+__global__ void __launch_bounds__(kMaxThreads, 1) k_score_term(const TermParams p) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    A* acc = reinterpret_cast<A*>(smem_raw);                       // [cells][Ts]
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Ts = p.Ts, H = p.H;
+    A* acc = reinterpret_cast<A*>(smem_raw);                                  // [G][Ts]
+    A* strips = acc + (size_t)p.G * Ts;                                       // [H][Ts]
+    uint2* hq = reinterpret_cast<uint2*>(strips + (size_t)H * Ts);            // [G][GS_HEAD_MAX] (strip, weight bits)
+    int* hcnt = reinterpret_cast<int*>(hq + (size_t)p.G * GS_HEAD_MAX);       // [G]
+    int* next_row = hcnt + p.G;
+    const int lane = threadIdx.x & 31;
+    const int nthreads = blockDim.x;
     const int qg = blockIdx.x % p.n_qgroups;
-    const int tg = blockIdx.x / p.n_qgroups;
+    const int j = blockIdx.x / p.n_qgroups;                                   // position in the tile set
     const int g0 = qg * p.G;
-    const int Gc = min(p.G, p.nq - g0);                            // queries in this CTA
-    const int j0 = tg * p.m;
-    const int mc = min(p.m, p.ts.count - j0);                      // tiles in this CTA
-    const int ncells = Gc * mc;
-    const int Ts = p.Ts;
-    A* headq = acc + (size_t)p.G * p.m * Ts;                       // [G][32] dense head weights (HEAD only)
+    const int Gc = min(p.G, p.nq - g0);
+    const int tile = p.ts.first + j * p.ts.stride;
+    const int32_t base = tile * Ts;
+    const int quads = Ts >> 2;
 
-    for (int i = threadIdx.x; i < ncells * Ts; i += kThreads) acc[i] = A(0);
-    if (HEAD)
-        for (int i = threadIdx.x; i < Gc * GS_HEAD_MAX; i += kThreads)
-            headq[i] = Num<WT>::qw(p.head_w[(p.q0 + g0) * GS_HEAD_MAX + i]);
+    // ---- stage: zero the accumulators, copy the tile's strips and the group's head lists
+    {
+        int4* a4 = reinterpret_cast<int4*>(acc);
+        for (int i = threadIdx.x; i < Gc * quads; i += nthreads) a4[i] = make_int4(0, 0, 0, 0);
+        if (H > 0) {
+            const W* __restrict__ gstrip = reinterpret_cast<const W*>(p.head_strip) + base;
+            for (int i = threadIdx.x; i < H * quads; i += nthreads) {
+                const int h = i / quads, dq = i - h * quads;
+                const W* src = gstrip + (size_t)h * p.N_pad + 4 * dq;
+                int4 v;
+                if (WT == GS_W_F32) {
+                    v = *reinterpret_cast<const int4*>(src);
+                } else {
+                    const uchar4 u = *reinterpret_cast<const uchar4*>(src);
+                    v = make_int4(u.x, u.y, u.z, u.w);
+                }
+                *reinterpret_cast<int4*>(strips + (size_t)h * Ts + 4 * dq) = v;
+            }
+            for (int i = threadIdx.x; i < Gc * GS_HEAD_MAX; i += nthreads)
+                hq[i] = p.head_pair[(p.q0 + g0) * GS_HEAD_MAX + i];
+            for (int i = threadIdx.x; i < Gc; i += nthreads) hcnt[i] = p.head_cnt[p.q0 + g0 + i];
+        }
+        if (threadIdx.x == 0) *next_row = 0;
+    }
     __syncthreads();
 
-    // ---- scatter phase: warp `warp` owns cells warp, warp+16, ...  (cell = (sub tile, query))
+    // ---- phase 1: scatter the tail lists; a warp owns the rows it draws from the counter
     const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
-    for (int c = warp; c < ncells; c += kWarps) {
-        const int g = c % Gc, sub = c / Gc;
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(next_row, 1);
+        g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        if (g >= Gc) break;
         const int64_t b = p.q0 + g0 + g;
-        const int tile = p.ts.first + (j0 + sub) * p.ts.stride;
-        const int32_t base = tile * Ts;
-        A* row = acc + (size_t)c * Ts;
+        A* row = acc + (size_t)g * Ts;
         const int64_t qa = p.q_indptr[b];
         const int cnt = p.tail_cnt[b];
         for (int i0 = 0; i0 < cnt; i0 += 32) {
-            int64_t off = 0;
-            uint32_t lo = 0, hi = 0, wq = 0;
+            int64_t start = 0;
+            int n = 0;
+            uint32_t wq = 0;
             if (i0 + lane < cnt) {
                 const int32_t t = p.tail_term[qa + i0 + lane];
                 wq = p.tail_w[qa + i0 + lane];
                 const uint32_t* sr = p.seg + (size_t)t * (p.ntiles + 1) + tile;
-                lo = sr[0];
-                hi = sr[1];
-                off = p.inv_off[t];
+                const uint32_t lo = sr[0], hi = sr[1];
+                n = (int)(hi - lo);
+                start = p.inv_off[t] + lo;
             }
-            const int nt = min(32, cnt - i0);
-            for (int j = 0; j < nt; ++j) {
-                const uint32_t lo_j = __shfl_sync(0xFFFFFFFFu, lo, j);
-                const uint32_t hi_j = __shfl_sync(0xFFFFFFFFu, hi, j);
-                if (lo_j >= hi_j) continue;
-                const int64_t off_j = __shfl_sync(0xFFFFFFFFu, off, j);
-                const A q = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, j));
-                for (uint32_t pp = (lo_j & ~31u) + lane; pp < hi_j; pp += 32) {
-                    const int32_t rel = p.inv_doc[off_j + pp] - base;
-                    if ((uint32_t)rel < (uint32_t)Ts) row[rel] = Num<WT>::mac(row[rel], q, inv_w[off_j + pp]);
-                }
+            unsigned m = __ballot_sync(0xFFFFFFFFu, n > 0);
+            while (m) {
+                const int src = __ffs(m) - 1;
+                m &= m - 1;
+                const int n_j = __shfl_sync(0xFFFFFFFFu, n, src);
+                const int64_t start_j = __shfl_sync(0xFFFFFFFFu, start, src);
+                const A q = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
+                scatter_segment<WT>(p.inv_doc + start_j, inv_w + start_j, n_j, q, row, base, Ts, lane);
             }
         }
     }
     __syncthreads();
 
-    // ---- epilogue: (+ head dot product) and hand every cell to the sink
-    const W* __restrict__ strip = reinterpret_cast<const W*>(p.head_strip);
-    for (int sub = 0; sub < mc; ++sub) {
-        const int tile = p.ts.first + (j0 + sub) * p.ts.stride;
-        for (int d = threadIdx.x; d < Ts; d += kThreads) {
-            const int64_t doc = (int64_t)tile * Ts + d;
-            const bool live = doc < p.N;
-            A dreg[GS_HEAD_MAX];
-            if (HEAD) {
-#pragma unroll
-                for (int h = 0; h < GS_HEAD_MAX; ++h)
-                    dreg[h] = (h < p.H && live) ? (A)strip[(size_t)h * p.N_pad + doc] : A(0);
+    // ---- phase 2: head strips + sink.  A thread owns 4 consecutive docs of one query at a time.
+    const bool filter = p.sink.thr != nullptr;
+    for (int item = threadIdx.x; item < Gc * quads; item += nthreads) {
+        const int g = item / quads, dq = item - g * quads;
+        const int64_t b = p.q0 + g0 + g;
+        const int4 a4 = *reinterpret_cast<const int4*>(acc + (size_t)g * Ts + 4 * dq);
+        A s0 = Num<WT>::from_bits(a4.x), s1 = Num<WT>::from_bits(a4.y), s2 = Num<WT>::from_bits(a4.z),
+          s3 = Num<WT>::from_bits(a4.w);
+        if (H > 0) {
+            const uint2* hl = hq + g * GS_HEAD_MAX;
+            const int nh = hcnt[g];
+            for (int i = 0; i < nh; ++i) {
+                const uint2 e = hl[i];
+                const A q = Num<WT>::qw(e.y);
+                const int4 v = *reinterpret_cast<const int4*>(strips + (size_t)e.x * Ts + 4 * dq);
+                s0 = Num<WT>::mac(s0, q, Num<WT>::from_bits(v.x));
+                s1 = Num<WT>::mac(s1, q, Num<WT>::from_bits(v.y));
+                s2 = Num<WT>::mac(s2, q, Num<WT>::from_bits(v.z));
+                s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
             }
-            const int32_t col = (j0 + sub) * Ts + d;
-            for (int g = 0; g < Gc; ++g) {
-                A s = acc[(size_t)(sub * Gc + g) * Ts + d];
-                if (HEAD) {
-                    const A* hq = headq + g * GS_HEAD_MAX;
-#pragma unroll
-                    for (int h = 0; h < GS_HEAD_MAX; ++h) s = Num<WT>::mac(s, hq[h], (W)dreg[h]);
-                }
-                if (live) emit<WT>(p, p.q0 + g0 + g, col, (int32_t)doc, s);
+        }
+        const int64_t doc0 = (int64_t)base + 4 * dq;
+        if (!filter) {
+            uint32_t* out = p.sink.dense + (b - p.q0) * p.sink.ld + (int64_t)j * Ts + 4 * dq;
+            if (doc0 + 3 < p.N && p.vec4) {
+                *reinterpret_cast<uint4*>(out) =
+                    make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
+            } else {
+                if (doc0 + 0 < p.N) out[0] = Num<WT>::bits(s0);
+                if (doc0 + 1 < p.N) out[1] = Num<WT>::bits(s1);
+                if (doc0 + 2 < p.N) out[2] = Num<WT>::bits(s2);
+                if (doc0 + 3 < p.N) out[3] = Num<WT>::bits(s3);
+            }
+        } else {
+            const uint64_t thr = p.sink.thr[b];
+            const uint32_t to = (uint32_t)(thr >> 32);
+            const bool r0 = Num<WT>::below(s0, to), r1 = Num<WT>::below(s1, to), r2 = Num<WT>::below(s2, to),
+                       r3 = Num<WT>::below(s3, to);
+            if (!(r0 && r1 && r2 && r3)) {
+                if (!r0 && doc0 + 0 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 0, s0);
+                if (!r1 && doc0 + 1 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 1, s1);
+                if (!r2 && doc0 + 2 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 2, s2);
+                if (!r3 && doc0 + 3 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 3, s3);
             }
         }
     }
 }
 
-template <int WT, bool HEAD>
-gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
-    GS_CUDA(cudaFuncSetAttribute(k_score_term<WT, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+struct Shape { int G; int threads; size_t smem; };
+
+// shared memory: G accumulator rows + H strips of Ts words, G head lists, G counts, the row counter
+size_t smem_for(const gs_index* ix, int H, int G) {
+    return ((size_t)G + H) * ix->Ts * 4 + (size_t)G * GS_HEAD_MAX * 8 + (size_t)G * 4 + 16;
+}
+
+Shape shape_for(const gs_index* ix, int H, int64_t nq, int group) {
+    const size_t budget = 220 * 1024;
+    int gmax = 0;
+    while (gmax < 4096 && smem_for(ix, H, gmax + 1) <= budget) ++gmax;
+    Shape s{};
+    int G = group > 0 ? group : 64;                 // 2 rows per warp at 1024 threads
+    G = (int)std::max<int64_t>(0, std::min<int64_t>(std::min<int64_t>(G, nq), gmax));
+    s.G = G;
+    s.threads = kMaxThreads;
+    s.smem = smem_for(ix, H, std::max(G, 1));
+    return s;
+}
+
+template <int WT>
+gs_status_t launch(const TermParams& p, unsigned grid, const Shape& sh, cudaStream_t s) {
+    GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
     {
         GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term<WT, HEAD><<<grid, kThreads, smem, s>>>(p);
+        k_score_term<WT><<<grid, sh.threads, sh.smem, s>>>(p);
     }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
@@ -167,38 +267,26 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t
 
 }  // namespace
 
-static int max_cells_for(const gs_index* ix) {
-    const size_t budget = 200 * 1024;   // shared memory for accumulators + head weights
-    return (int)(budget / ((size_t)ix->Ts * 4 + GS_HEAD_MAX * 4));
-}
-int gs_score_term_group(const gs_index* ix, int64_t nq, int group) {
-    int G = group > 0 ? group : (int)std::min<int64_t>(nq, 1 << 20);
-    return (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(G, nq), max_cells_for(ix)));
+int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
+    return shape_for(ix, use_head ? ix->H : 0, nq, group).G;
 }
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
-    const bool head = use_head && ix->H > 0;
-    // cells per CTA: bounded by shared memory (accumulators + head weights)
-    const int max_cells = max_cells_for(ix);
-    if (max_cells < 1) return GS_ERR_OOM;
-    const int G = gs_score_term_group(ix, nq, group);
-    int m = std::max(1, std::min(max_cells / G, kWarps / std::min(G, kWarps)));
-    m = std::min(m, ts.count);
+    const int H = (use_head && ix->H > 0) ? ix->H : 0;
+    const Shape sh = shape_for(ix, H, nq, group);
+    if (sh.G < 1) return GS_ERR_OOM;                 // one accumulator row + the strips do not fit: tile_docs too large
     TermParams p{};
     p.inv_off = ix->inv_off; p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg = ix->seg;
-    p.head_strip = ix->head_strip; p.H = head ? ix->H : 0; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
+    p.head_strip = ix->head_strip; p.H = H; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
     p.ntiles = ix->ntiles;
-    p.q_indptr = qb.indptr; p.head_w = qb.head_w; p.tail_term = qb.tail_term; p.tail_w = qb.tail_w;
-    p.tail_cnt = qb.tail_cnt;
-    p.q0 = q0; p.nq = (int32_t)nq; p.G = G; p.n_qgroups = (int)((nq + G - 1) / G);
-    p.ts = ts; p.m = m; p.sink = sink;
-    const int n_tgroups = (ts.count + m - 1) / m;
-    const int64_t grid = (int64_t)p.n_qgroups * n_tgroups;
+    p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_term = qb.tail_term;
+    p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt;
+    p.q0 = q0; p.nq = (int32_t)nq; p.G = sh.G; p.n_qgroups = (int)((nq + sh.G - 1) / sh.G);
+    p.ts = ts; p.sink = sink;
+    p.vec4 = sink.dense && (((uintptr_t)sink.dense | (uintptr_t)(sink.ld * 4)) & 15) == 0;
+    const int64_t grid = (int64_t)p.n_qgroups * ts.count;
     if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-    const size_t smem = (size_t)G * m * ix->Ts * 4 + (head ? (size_t)G * GS_HEAD_MAX * 4 : 0);
-    if (ix->wtype == GS_W_F32)
-        return head ? launch<GS_W_F32, true>(p, (unsigned)grid, smem, s) : launch<GS_W_F32, false>(p, (unsigned)grid, smem, s);
-    return head ? launch<GS_W_U8, true>(p, (unsigned)grid, smem, s) : launch<GS_W_U8, false>(p, (unsigned)grid, smem, s);
+    return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, sh, s) : launch<GS_W_U8>(p, (unsigned)grid, sh, s);
 }

@@ -370,3 +370,52 @@ def test_mid_prefix_full_compare(gs, mode, algo):
     st = ix.stats()
     assert st["overflow_queries"] == 0
     ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# paper scale (BASELINE.json configs[2] and [3]) in the launch configuration bench.py times
+# ----------------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def paper_docs():
+    return wl.make_docs("paper")            # 8.8M docs, 1.06e9 postings (~3 s on the box's cores)
+
+
+@pytest.mark.parametrize("mode,k", [("f32", 1000), ("u8", 10)])
+def test_paper_scale_sampled(gs, paper_docs, mode, k):
+    """All B=500 queries: structure + every returned score against the oracle's pairwise score (one merge each);
+    a sample of queries (one per host core, at most 16): the complete top-k against the oracle's exhaustive search."""
+    docs = paper_docs if mode == "f32" else paper_docs.to_u8()
+    queries = wl.make_queries("paper" if mode == "f32" else "paper_u8")
+    assert docs.rows == 8_800_000 and queries.rows == 500
+    R_d, R_q = oracle.as_rows(docs, wl.VOCAB), oracle.as_rows(queries, wl.VOCAB)
+    n_s = max(1, min(16, oracle.max_threads()))
+    sample = np.linspace(0, queries.rows - 1, n_s).astype(np.int64)
+    R_s = oracle.as_rows(wl.Csr(*_take_rows(queries, sample)), wl.VOCAB)
+    o_ids, o_sc = oracle.search(R_s, R_d, k)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    for algo in ALGOS:
+        ids, sc = gpu_search(gs, ix, queries, k, algo=algo)
+        assert ix.stats()["overflow_queries"] == 0
+        b_idx = np.repeat(np.arange(queries.rows, dtype=np.int64), k)
+        true = oracle.score_pairs(R_q, R_d, b_idx, ids.reshape(-1).astype(np.int64)).reshape(queries.rows, k)
+        if mode == "u8":
+            assert np.array_equal(sc.astype(np.int64), true)
+            parity.check_int_exact(ids[sample], sc[sample], o_ids, o_sc)
+        else:
+            assert np.all(np.abs(sc - true) <= parity.tol(true))
+            for j, b in enumerate(sample):
+                parity.check_f32_row(ids[b], sc[b], o_ids[j], o_sc[j], true[b], docs.rows)
+        for b in range(queries.rows):                      # structure of every row
+            assert len(np.unique(ids[b])) == k and ids[b].min() >= 0 and ids[b].max() < docs.rows
+            d = np.diff(sc[b].astype(np.float64))
+            assert np.all(d <= 0) and np.all(ids[b][:-1][d == 0] < ids[b][1:][d == 0])
+    ix.close()
+
+
+def _take_rows(csr, rows):
+    indptr, terms, weights = [0], [], []
+    for r in rows:
+        t, w = csr.row(int(r))
+        terms.append(t); weights.append(w)
+        indptr.append(indptr[-1] + len(t))
+    return np.array(indptr, np.int64), np.concatenate(terms), np.concatenate(weights)
