@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--doc-query-tile", type=int, default=0)
     ap.add_argument("--query-group", type=int, default=0)
     ap.add_argument("--tile-docs", type=int, default=0)
+    ap.add_argument("--head-max", type=int, default=0, help="dense strips kept by the index (0 = default 64, -1 = none)")
+    ap.add_argument("--head-density", type=float, default=0.0, help="list density from which a strip is kept (0 = default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-queries", type=int, default=0, help="oracle sample size (0 = one per core)")
@@ -227,11 +229,13 @@ def run_ours(args):
     queries = wl.make_queries(args.config, n_queries=B, row0=rank * B)   # ... and searches its own batch
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
-    ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs, head_max=args.head_max,
+                             head_density=args.head_density)
     torch.cuda.synchronize()
     t_build = time.perf_counter() - t0
     info = ix.info()
     lens = ix.meta()[1].astype(np.int64)
+    head_terms = ix.head_terms()
     q_dev = [torch.from_numpy(a).to(dev) for a in (queries.indptr, queries.terms, queries.weights)]
     sdt = torch.float32 if c["wtype"] == "f32" else torch.int32
     out_ids = torch.empty((B, k), dtype=torch.int32, device=dev)
@@ -263,7 +267,7 @@ def run_ours(args):
                "overflow_queries": st["overflow_queries"], "workspace_bytes": ws_bytes, "clocks": cs.summary(),
                "kernels": {n: {"launches_per_step": v["launches"] / args.steps, "ms_per_step": v["ms"] / args.steps}
                            for n, v in prof.items()}}
-        res["roofline"] = roofline(res, st, info, lens, queries, B, k, peaks, c["wtype"])
+        res["roofline"] = roofline(res, st, info, lens, head_terms, queries, B, k, peaks, c["wtype"])
         del ws
         return res
 
@@ -319,7 +323,8 @@ def run_ours(args):
                 "overflow_queries": main["overflow_queries"], "other_algos": others,
                 "index": {"postings": info["nnz"], "padded_postings": info["padded_nnz"], "bytes_inverted": info["bytes_inverted"],
                           "bytes_forward": info["bytes_forward"], "bytes_head": info["bytes_head"],
-                          "bytes_meta": info["bytes_inverted_meta"], "head_terms": info["head_terms"], "tile_docs": info["tile_docs"],
+                          "bytes_meta": info["bytes_inverted_meta"], "head_terms": info["head_terms"], "head_terms_term_parallel": info["head_terms_term_parallel"],
+                          "forward_tail_postings": info["forward_tail_nnz"], "tile_docs": info["tile_docs"],
                           "build_s": t_build, "generate_s": t_gen},
                 "context": {"paper_h100_qps": 787, "paper_h100_doc_parallel_hbm_frac": 0.626,
                             "note": "paper numbers are H100 + MS MARCO/SPLADE (PAPER.md L292, L340): context, not a baseline"}}
@@ -329,12 +334,13 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def roofline(res, st, info, lens, queries, B, k, peaks, wtype):
+def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
     """Roofline of the dominant scoring kernel of the step (SURVEY §8d byte models).
 
-    doc-parallel (bound hbm): algorithmic bytes per step = passes * bytes(forward index) * (1 + sample share):
-      the forward index is streamed once per tile of `doc_query_tile` queries (PAPER.md L174 streams it once
-      per QUERY: B*N*kbar*12 bytes); the threshold sample re-reads 1/2^shift of it.
+    doc-parallel (bound hbm): algorithmic bytes per step = sum over passes of bytes(forward index) * (1 + sample
+      share): the forward index (indptr + tail CSR + the dense strips the pass's queries use) is streamed once
+      per tile of `doc_query_tile` queries (PAPER.md L174 streams it once per QUERY: B*N*kbar*12 bytes); the
+      threshold sample re-reads 1/2^shift of it.
     term-parallel: algorithmic bytes per step = (4 + w) * U, U = postings of the batch's distinct terms
       (each read once; the paper's model B*qbar*Lbar*8 of L172 counts them once per query: `bytes_paper_model`).
       The kernel is bound by shared-memory read-modify-writes, so its `mac_per_s` is reported too.
@@ -352,10 +358,12 @@ def roofline(res, st, info, lens, queries, B, k, peaks, wtype):
            "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": None,
            "useful_mac_per_step": ts["W"], "mac_per_s": ts["W"] / (kms * 1e-3)}
     if name == "score_doc":
-        alg = rf.doc_parallel_bytes(info["num_docs"], info["nnz"], wtype, B, st["doc_query_tile"], share)
-        one = rf.forward_index_bytes(info["num_docs"], info["nnz"], wtype)
+        sp = rf.strips_per_pass(queries.indptr, queries.terms, head_terms, st["doc_query_tile"])
+        alg = rf.doc_parallel_bytes(info["num_docs"], info["forward_tail_nnz"], wtype, B, st["doc_query_tile"], share, sp)
+        one = rf.forward_index_bytes(info["num_docs"], info["forward_tail_nnz"], wtype, len(head_terms))
         out.update({"doc_query_tile": st["doc_query_tile"], "passes": st["doc_passes"], "bytes_per_step": alg,
-                    "bytes_model": "passes*(8*(N+1)+(4+w)*P)*(1+sample share)", "bytes_one_pass": one,
+                    "bytes_model": "sum_passes(8*(N+1)+(4+w)*P_tail+w*N*strips_used(pass))*(1+sample share)",
+                    "strips_used_per_pass_mean": float(np.mean(sp)) if sp else 0.0, "bytes_one_pass": one,
                     "frac_one_pass": rf.effective_gbps(one, kms) / peaks["hbm_gbs"]})
     else:
         alg = rf.term_parallel_bytes(ts["U"], wtype, share)

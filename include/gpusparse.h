@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define GS_ABI_VERSION 1
+#define GS_ABI_VERSION 2
 #if defined(__GNUC__)
 #define GS_API __attribute__((visibility("default")))
 #else
@@ -86,9 +86,10 @@ typedef struct gs_alloc {
 /* Build options; pass NULL for defaults (fields set to 0 also mean "default"). */
 typedef struct gs_build_opts {
     int32_t tile_docs;        /* doc-id range covered by one accumulator tile (multiple of 32; default 512)   */
-    int32_t head_max;         /* max number of posting lists additionally stored as dense strips (0..32;       */
-                              /* default 32; -1 disables).  A list qualifies when |PL(t)| >= head_density * N  */
-    float head_density;       /* default 0.5: the density at which 4 B/doc beats 8 B/posting                   */
+    int32_t head_max;         /* max number of posting lists additionally stored as dense strips (0..64;       */
+                              /* default 64; -1 disables).  A list qualifies when |PL(t)| >= head_density * N  */
+    float head_density;       /* default 0.25.  4 B/doc beats 8 B/posting from density 0.5 on; below that a    */
+                              /* strip costs bytes but saves the per-posting lookup of the doc-parallel kernel */
     int32_t validate;         /* default 1: reject out-of-range ids, duplicates, non-finite weights            */
 } gs_build_opts_t;
 
@@ -103,9 +104,13 @@ typedef struct gs_info {
     int32_t head_terms;        /* number of dense-strip posting lists                                 */
     int64_t bytes_inverted;    /* doc_ids + weights of the padded lists            Eq. (3)            */
     int64_t bytes_inverted_meta; /* offsets + lengths + tile-segment table                            */
-    int64_t bytes_forward;     /* CSR forward index: indptr + term ids + weights                      */
+    int64_t bytes_forward;     /* forward index, CSR part: indptr + term ids + weights of the postings
+                                  whose term has no strip (the strips are its dense part)             */
     int64_t bytes_head;        /* dense strips                                                        */
     int64_t bytes_total;
+    int64_t forward_tail_nnz;  /* postings held by the CSR part of the forward index                  */
+    int32_t head_terms_term_parallel; /* strips the term-parallel kernel stages per tile (<= 32)      */
+    int32_t reserved;
 } gs_info_t;
 
 /* Search options; pass NULL for defaults. */
@@ -151,6 +156,11 @@ GS_API gs_status_t gs_index_copy_meta(const gs_index_t* index, int64_t* host_off
 /* Copies min(capacity, padded_length(term)) entries; host_weights is float[] or uint8_t[] per wtype. */
 GS_API gs_status_t gs_index_copy_list(const gs_index_t* index, int32_t term, int64_t capacity,
                                int32_t* host_doc_ids, void* host_weights, int64_t* out_padded_length);
+
+/* The terms whose posting lists are also stored as dense strips, densest first: writes
+ * min(capacity, head_terms) term ids to host_terms and the total to *out_count. */
+GS_API gs_status_t gs_index_copy_head_terms(const gs_index_t* index, int32_t capacity, int32_t* host_terms,
+                                     int32_t* out_count);
 
 /* ------------------------------------------------------------------------------------------------
  * Search (§4-§5).

@@ -23,6 +23,7 @@ ALGOS = {"auto": GS_ALGO_AUTO, "term": GS_ALGO_TERM_PARALLEL, "doc": GS_ALGO_DOC
 
 EXPORTS = [
     "gs_index_build", "gs_index_info", "gs_index_free", "gs_index_copy_meta", "gs_index_copy_list",
+    "gs_index_copy_head_terms",
     "gs_search_workspace_bytes", "gs_search", "gs_search_host", "gs_search_stats", "gs_score_dense",
     "gs_topk_workspace_bytes", "gs_topk_dense", "gs_strerror", "gs_version", "gs_abi_version",
     "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name",
@@ -51,7 +52,8 @@ class gs_info_t(ctypes.Structure):
                 ("nnz", ctypes.c_int64), ("padded_nnz", ctypes.c_int64), ("nonempty_terms", ctypes.c_int64),
                 ("tile_docs", ctypes.c_int32), ("num_tiles", ctypes.c_int32), ("head_terms", ctypes.c_int32),
                 ("bytes_inverted", ctypes.c_int64), ("bytes_inverted_meta", ctypes.c_int64),
-                ("bytes_forward", ctypes.c_int64), ("bytes_head", ctypes.c_int64), ("bytes_total", ctypes.c_int64)]
+                ("bytes_forward", ctypes.c_int64), ("bytes_head", ctypes.c_int64), ("bytes_total", ctypes.c_int64),
+                ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 class gs_search_opts_t(ctypes.Structure):
@@ -89,6 +91,7 @@ def lib():
         L.gs_index_free.restype = None
         L.gs_index_copy_meta.argtypes = [vp, vp, vp]
         L.gs_index_copy_list.argtypes = [vp, i32, i64, vp, vp, P(i64)]
+        L.gs_index_copy_head_terms.argtypes = [vp, i32, vp, P(i32)]
         L.gs_search_workspace_bytes.argtypes = [vp, i64, i64, i32, P(gs_search_opts_t), P(sz)]
         L.gs_search.argtypes = [vp, P(gs_csr_t), i32, P(gs_search_opts_t), vp, vp, vp, sz, vp]
         L.gs_search_host.argtypes = [vp, P(gs_csr_t), i32, P(gs_search_opts_t), vp, vp, vp]
@@ -231,6 +234,13 @@ class Index:
         ln = np.empty(self.vocab_size, np.int32)
         _check(lib().gs_index_copy_meta(self._h, off.ctypes.data, ln.ctypes.data))
         return off, ln
+
+    def head_terms(self) -> np.ndarray:
+        """Term ids whose lists are also kept as dense strips, densest first."""
+        n = ctypes.c_int32()
+        out = np.empty(64, np.int32)
+        _check(lib().gs_index_copy_head_terms(self._h, 64, out.ctypes.data, ctypes.byref(n)))
+        return out[:n.value].copy()
 
     def posting_list(self, term: int) -> Tuple[np.ndarray, np.ndarray]:
         """The padded posting list of ``term`` (doc ids incl. -1 sentinels, weights incl. 0 padding)."""

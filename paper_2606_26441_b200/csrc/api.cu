@@ -125,7 +125,7 @@ __global__ void k_zero_u32(uint32_t* p, int64_t n) {
 struct Plan {
     int algo = GS_ALGO_TERM_PARALLEL;
     uint32_t flags = 0;
-    int group = 0, qtile = 16;
+    int group = 0, qtile = 32;
     bool dense_only = false;
     int stride = 1;            // sample = every stride-th tile
     int sample_tiles = 0;
@@ -139,8 +139,9 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
         p.algo = o->algo == GS_ALGO_AUTO ? GS_ALGO_TERM_PARALLEL : o->algo;
         p.flags = o->flags;
         p.group = o->query_group;
-        p.qtile = o->doc_query_tile > 0 ? o->doc_query_tile : 16;
+        p.qtile = o->doc_query_tile;
     }
+    if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : (B <= 16 ? 16 : 32);   // doc-parallel: queries per pass over the forward index
     p.use_head = !(p.flags & GS_FLAG_NO_HEAD_STRIPS);
     int shift = (o && o->sample_shift > 0) ? o->sample_shift : 5;
     // the sample must hold comfortably more than k documents, else its k-th key is a weak bound
@@ -152,7 +153,6 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
         p.cand_cap = std::max<int64_t>(4096, 8 * (int64_t)k * p.stride);
         p.cand_cap = std::min<int64_t>(p.cand_cap, ix->N_pad);
     }
-    (void)B;
     return p;
 }
 
@@ -376,6 +376,7 @@ gs_status_t gs_index_info(const gs_index_t* ix, gs_info_t* out) {
     out->num_tiles = ix->ntiles; out->head_terms = ix->H;
     out->bytes_inverted = ix->bytes_inverted; out->bytes_inverted_meta = ix->bytes_meta;
     out->bytes_forward = ix->bytes_forward; out->bytes_head = ix->bytes_head;
+    out->head_terms_term_parallel = ix->H_term; out->forward_tail_nnz = ix->P_tail;
     out->bytes_total = ix->bytes_inverted + ix->bytes_meta + ix->bytes_forward + ix->bytes_head;
     return GS_OK;
 }
@@ -402,6 +403,13 @@ gs_status_t gs_index_copy_list(const gs_index_t* ix, int32_t term, int64_t capac
         GS_CUDA(cudaMemcpy(host_weights, (const unsigned char*)ix->inv_w + (size_t)off[0] * wb, wb * (size_t)n,
                            cudaMemcpyDeviceToHost));
     }
+    return GS_OK;
+}
+
+gs_status_t gs_index_copy_head_terms(const gs_index_t* ix, int32_t capacity, int32_t* host_terms, int32_t* out_count) {
+    if (!ix || !out_count || capacity < 0 || (capacity > 0 && !host_terms)) return GS_ERR_INVALID_ARG;
+    *out_count = ix->H;
+    for (int32_t h = 0; h < std::min(capacity, ix->H); ++h) host_terms[h] = ix->head_terms_host[h];
     return GS_OK;
 }
 

@@ -6,7 +6,8 @@
 
 #include "../../include/gpusparse.h"
 
-#define GS_HEAD_MAX 32          // dense-strip posting lists kept in registers by the head pass
+#define GS_HEAD_MAX 32          // term-parallel: strips staged per tile / entries of a query's compact head list
+#define GS_STRIP_MAX 64         // dense strips kept by the index (the doc-parallel kernel uses all of them)
 #define GS_SEL_BINS 2048        // radix-select digit: 11 bits
 #define GS_SEL_BITS 11
 
@@ -38,10 +39,12 @@ struct gs_index {
     int32_t Ts = 512;         // docs per accumulator tile
     int32_t ntiles = 0;       // ceil(N / Ts)
     int64_t N_pad = 0;        // ntiles * Ts
-    // forward (doc-major CSR) index — PAPER.md L174
+    // forward (doc-major) index — PAPER.md L174.  Hybrid layout: the H strip terms of a document live in the
+    // dense strips below (column-major, 0 = absent); every other posting lives in this "tail" CSR.
     int64_t* fwd_indptr = nullptr;   // [N+1]
-    int32_t* fwd_terms = nullptr;    // [P]
-    void* fwd_w = nullptr;           // [P] float | uint8
+    int32_t* fwd_terms = nullptr;    // [P_tail]
+    void* fwd_w = nullptr;           // [P_tail] float | uint8
+    int64_t P_tail = 0;              // postings of the terms without a strip
     // inverted index — PAPER.md L79-90
     int64_t* inv_off = nullptr;      // [V+1] start of each padded list (multiple of 32)
     int32_t* inv_len = nullptr;      // [V]   true list length
@@ -50,8 +53,9 @@ struct gs_index {
     // per-(term, tile) segment table: seg[t*(ntiles+1)+j] = number of postings of t with doc < j*Ts
     uint32_t* seg = nullptr;         // [V][ntiles+1]
     // dense strips of the densest lists ("head" terms)
-    int32_t H = 0;
-    int32_t head_terms_host[GS_HEAD_MAX];
+    int32_t H = 0;                   // strips (<= GS_STRIP_MAX), densest list first
+    int32_t H_term = 0;              // the first H_term strips fit the term-parallel kernel's shared memory
+    int32_t head_terms_host[GS_STRIP_MAX];
     int16_t* head_slot = nullptr;    // [V]: strip number of a term or -1
     void* head_strip = nullptr;      // [H][N_pad] float | uint8 (0 where the doc is not in the list)
     // allocator

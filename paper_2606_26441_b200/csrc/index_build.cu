@@ -10,6 +10,7 @@
 // lists directly.  The sort is cub::DeviceRadixSort (a library primitive; the build is not on the
 // timed path).
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
 
 #include <algorithm>
 #include <vector>
@@ -130,6 +131,50 @@ __global__ void k_fill_strip(const int32_t* __restrict__ inv_doc, const W* __res
     if (i < len) strip[inv_doc[off + i]] = inv_w[off + i];
 }
 
+// forward "tail" CSR: the postings of a document whose term has no dense strip, in the row's order.
+// One warp per document; pass 1 counts, pass 2 (after an exclusive scan) writes.
+__global__ void k_tail_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
+                             const int16_t* __restrict__ head_slot, int64_t rows, int32_t V, int64_t* __restrict__ cnt) {
+    const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= rows) return;
+    const int64_t a = indptr[warp], b = indptr[warp + 1];
+    int n = 0;
+    for (int64_t i = a + lane; i < b; i += 32) {
+        const int32_t t = terms[i];
+        n += (t >= 0 && t < V && head_slot[t] < 0) ? 1 : 0;
+    }
+    for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xFFFFFFFFu, n, o);
+    if (lane == 0) cnt[warp] = n;
+}
+
+template <typename W>
+__global__ void k_tail_fill(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms, const W* __restrict__ w,
+                            const int16_t* __restrict__ head_slot, int64_t rows, int32_t V,
+                            const int64_t* __restrict__ tail_indptr, int32_t* __restrict__ out_terms, W* __restrict__ out_w) {
+    const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= rows) return;
+    const int64_t a = indptr[warp], b = indptr[warp + 1];
+    int64_t dst = tail_indptr[warp];
+    for (int64_t i0 = a; i0 < b; i0 += 32) {
+        const int64_t i = i0 + lane;
+        int32_t t = -1;
+        bool keep = false;
+        if (i < b) {
+            t = terms[i];
+            keep = t >= 0 && t < V && head_slot[t] < 0;
+        }
+        const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
+        if (keep) {
+            const int64_t o = dst + __popc(m & ((1u << lane) - 1u));
+            out_terms[o] = t;
+            out_w[o] = w[i];
+        }
+        dst += __popc(m);
+    }
+}
+
 inline unsigned grid_for(int64_t n, int threads = kThreads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
@@ -172,18 +217,6 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     GS_CUDA(cudaStreamSynchronize(s));
     if (h_err) return (gs_status_t)h_err;
 
-    // ---- forward index: a private copy of the CSR (inputs may be released after the call)
-    ix->fwd_indptr = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(N + 1), s);
-    ix->fwd_terms = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)P, s);
-    ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)P, s);
-    if (!ix->fwd_indptr || !ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
-    GS_CUDA(cudaMemcpyAsync(ix->fwd_indptr, docs->indptr, sizeof(int64_t) * (size_t)(N + 1), cudaMemcpyDeviceToDevice, s));
-    if (P > 0) {
-        GS_CUDA(cudaMemcpyAsync(ix->fwd_terms, docs->term_ids, sizeof(int32_t) * (size_t)P, cudaMemcpyDeviceToDevice, s));
-        GS_CUDA(cudaMemcpyAsync(ix->fwd_w, docs->weights, sizeof(W) * (size_t)P, cudaMemcpyDeviceToDevice, s));
-    }
-    ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(N + 1) + (sizeof(int32_t) + sizeof(W)) * (size_t)P);
-
     // ---- list lengths
     ix->inv_len = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)V, s);
     ix->inv_off = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(V + 1), s);
@@ -221,21 +254,59 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     GS_CUDA(cudaMemcpyAsync(ix->inv_off, h_off.data(), sizeof(int64_t) * (size_t)(V + 1), cudaMemcpyHostToDevice, s));
 
     std::vector<int32_t> order;
-    int hmax = o.head_max < 0 ? 0 : (o.head_max == 0 ? GS_HEAD_MAX : std::min(o.head_max, GS_HEAD_MAX));
-    // the tile's strips are staged in shared memory next to the accumulator rows (score_term.cu)
-    hmax = std::max(0, std::min(hmax, (int)(200 * 1024 / (4 * (size_t)ix->Ts)) - 8));
-    float dens = o.head_density > 0.f ? o.head_density : 0.5f;
+    int hmax = o.head_max < 0 ? 0 : (o.head_max == 0 ? GS_STRIP_MAX : std::min(o.head_max, GS_STRIP_MAX));
+    float dens = o.head_density > 0.f ? o.head_density : 0.25f;
     for (int32_t t = 0; t < V; ++t)
         if (N > 0 && (double)h_len[t] >= (double)dens * (double)N && h_len[t] > 0) order.push_back(t);
     std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return h_len[a] > h_len[b]; });
     if ((int)order.size() > hmax) order.resize(hmax);
     ix->H = (int32_t)order.size();
+    // the term-parallel kernel stages a tile's strips in shared memory next to its accumulator rows (score_term.cu):
+    // it uses the densest H_term strips and scatters the other lists
+    ix->H_term = std::max(0, std::min({ix->H, GS_HEAD_MAX, (int)(200 * 1024 / (4 * (size_t)ix->Ts)) - 8}));
     std::vector<int16_t> h_slot(V, (int16_t)-1);
-    for (int h = 0; h < GS_HEAD_MAX; ++h) ix->head_terms_host[h] = h < ix->H ? order[h] : -1;
+    for (int h = 0; h < GS_STRIP_MAX; ++h) ix->head_terms_host[h] = h < ix->H ? order[h] : -1;
     for (int h = 0; h < ix->H; ++h) h_slot[order[h]] = (int16_t)h;
     ix->head_slot = (int16_t*)gs_dev_alloc(ix, sizeof(int16_t) * (size_t)V, s);
     if (!ix->head_slot) return GS_ERR_OOM;
     GS_CUDA(cudaMemcpyAsync(ix->head_slot, h_slot.data(), sizeof(int16_t) * (size_t)V, cudaMemcpyHostToDevice, s));
+
+    // ---- forward index, hybrid: strips for the H densest lists + a CSR of every other posting
+    {
+        int64_t p_tail = P;
+        for (int h = 0; h < ix->H; ++h) p_tail -= h_len[order[h]];
+        ix->P_tail = p_tail;
+        ix->fwd_indptr = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(N + 1), s);
+        ix->fwd_terms = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)std::max<int64_t>(p_tail, 1), s);
+        ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)std::max<int64_t>(p_tail, 1), s);
+        if (!ix->fwd_indptr || !ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
+        if (ix->H == 0) {
+            GS_CUDA(cudaMemcpyAsync(ix->fwd_indptr, docs->indptr, sizeof(int64_t) * (size_t)(N + 1), cudaMemcpyDeviceToDevice, s));
+            if (P > 0) {
+                GS_CUDA(cudaMemcpyAsync(ix->fwd_terms, docs->term_ids, sizeof(int32_t) * (size_t)P, cudaMemcpyDeviceToDevice, s));
+                GS_CUDA(cudaMemcpyAsync(ix->fwd_w, docs->weights, sizeof(W) * (size_t)P, cudaMemcpyDeviceToDevice, s));
+            }
+        } else {
+            int64_t* d_cnt = (int64_t*)tmp.get(sizeof(int64_t) * (size_t)(N + 1));
+            if (!d_cnt) return GS_ERR_OOM;
+            GS_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(int64_t) * (size_t)(N + 1), s));
+            k_tail_count<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, ix->head_slot, N, V, d_cnt);
+            size_t scan_bytes = 0;
+            if (N + 1 > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+            GS_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
+            void* d_scan_tmp = tmp.get(scan_bytes);
+            if (!d_scan_tmp) return GS_ERR_OOM;
+            GS_CUDA(cub::DeviceScan::ExclusiveSum(d_scan_tmp, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
+            k_tail_fill<W><<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, (const W*)docs->weights,
+                                                                ix->head_slot, N, V, ix->fwd_indptr, ix->fwd_terms,
+                                                                (W*)ix->fwd_w);
+            int64_t tail_end = 0;
+            GS_CUDA(cudaMemcpyAsync(&tail_end, ix->fwd_indptr + N, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+            GS_CUDA(cudaStreamSynchronize(s));
+            if (tail_end != p_tail) return GS_ERR_OUT_OF_RANGE;     // some term id was outside [0,V) (validate off)
+        }
+        ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(N + 1) + (sizeof(int32_t) + sizeof(W)) * (size_t)p_tail);
+    }
 
     // ---- padded inverted arrays, pre-filled with the sentinel (doc_id=-1, score=0), L90
     ix->inv_doc = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)ix->P_pad, s);

@@ -2,7 +2,7 @@
 //
 // The paper pads queries to a [B, M] matrix of (term id, weight) in Python (PAPER.md L120-123,
 // L146-152).  Here one warp per query splits its terms into
-//   * head terms (lists kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
+//   * head terms (the H_term densest lists, kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
 //   * tail terms: compacted (row b starts at indptr[b]) into tail_term/tail_w, weights converted to the
 //     accumulator type (float, or int32 for uint8 impacts).
 // Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
@@ -14,7 +14,7 @@ namespace {
 template <int WT>
 __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
                          const void* __restrict__ weights, int64_t B, int32_t V, const int16_t* __restrict__ head_slot,
-                         int use_head, int validate, uint2* __restrict__ head_pair, int32_t* __restrict__ head_cnt,
+                         int h_term, int validate, uint2* __restrict__ head_pair, int32_t* __restrict__ head_cnt,
                          int32_t* __restrict__ tail_term,
                          uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, int32_t* __restrict__ status) {
     const int lane = threadIdx.x & 31;
@@ -43,7 +43,8 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
                     if (terms[j] == t) { atomicCAS(status, 0, (int)GS_ERR_DUPLICATE_TERM); break; }
             }
         }
-        int slot = (ok && use_head) ? (int)head_slot[t] : -1;
+        int slot = (ok && h_term > 0) ? (int)head_slot[t] : -1;
+        if (slot >= h_term) slot = -1;          // a strip the term-parallel kernel does not stage: scatter its list
         const bool is_head = ok && slot >= 0;
         const unsigned mh = __ballot_sync(0xFFFFFFFFu, is_head);
         if (is_head) {
@@ -78,11 +79,11 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     GsProfScope ps(GS_K_INGEST, s);
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                   use_head && ix->H > 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                   use_head ? ix->H_term : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                    qb->tail_w, qb->tail_cnt, qb->status);
     else
         k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                  use_head && ix->H > 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                  use_head ? ix->H_term : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                   qb->tail_w, qb->tail_cnt, qb->status);
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());

@@ -268,13 +268,13 @@ gs_status_t launch(const TermParams& p, unsigned grid, const Shape& sh, cudaStre
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    return shape_for(ix, use_head ? ix->H : 0, nq, group).G;
+    return shape_for(ix, use_head ? ix->H_term : 0, nq, group).G;
 }
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
-    const int H = (use_head && ix->H > 0) ? ix->H : 0;
+    const int H = use_head ? ix->H_term : 0;
     const Shape sh = shape_for(ix, H, nq, group);
     if (sh.G < 1) return GS_ERR_OOM;                 // one accumulator row + the strips do not fit: tile_docs too large
     TermParams p{};

@@ -10,8 +10,12 @@ Pure arithmetic on sizes — no scoring.  Two families of models:
                                                                forward index re-read for EVERY query)
 * OUR kernels' algorithmic bytes (what the method must move at least once per launch):
     term-parallel    bytes = (4 + w) * U                      U = postings of the batch's DISTINCT terms
-    doc-parallel     bytes = passes * (8*(N+1) + (4+w)*P)     passes = ceil(B / query tile): the forward
-                                                               index is streamed once per query TILE
+    doc-parallel     bytes = sum over passes of 8*(N+1) + (4+w)*P_tail + w*N*h_pass
+                                                               passes = ceil(B / query tile): the forward index is
+                                                               streamed once per query TILE; it is a hybrid of a CSR
+                                                               holding the P_tail postings without a dense strip and
+                                                               of H strips (w bytes per doc each), of which a pass
+                                                               reads the h_pass ones some query of its tile uses
   with w = 4 (fp32 weights) or 1 (uint8 impacts).
 """
 from __future__ import annotations
@@ -59,13 +63,32 @@ def batch_term_stats(list_lengths: np.ndarray, query_terms: np.ndarray) -> dict:
     return {"U": int(L[np.unique(t)].sum()), "W": int(L[t].sum()), "distinct_terms": int(np.unique(t).shape[0])}
 
 
-def forward_index_bytes(N: int, P: int, wtype: str) -> int:
-    return 8 * (N + 1) + (4 + weight_bytes(wtype)) * P
+def forward_index_bytes(N: int, P_tail: int, wtype: str, strips: int = 0) -> int:
+    """One pass over the hybrid forward index: indptr + tail CSR + `strips` dense strips of N entries."""
+    w = weight_bytes(wtype)
+    return 8 * (N + 1) + (4 + w) * P_tail + w * N * strips
 
 
-def doc_parallel_bytes(N: int, P: int, wtype: str, B: int, query_tile: int, sample_share: float = 0.0) -> float:
+def strips_per_pass(query_indptr: np.ndarray, query_terms: np.ndarray, head_terms: np.ndarray, query_tile: int) -> list:
+    """For every pass (tile of `query_tile` consecutive queries): how many strip terms its queries contain."""
+    indptr = np.asarray(query_indptr, dtype=np.int64)
+    B = indptr.shape[0] - 1
+    head = np.asarray(head_terms)
+    out = []
+    for a in range(0, B, max(query_tile, 1)):
+        b = min(B, a + query_tile)
+        t = np.asarray(query_terms[indptr[a]:indptr[b]])
+        out.append(int(np.intersect1d(t, head).shape[0]))
+    return out
+
+
+def doc_parallel_bytes(N: int, P_tail: int, wtype: str, B: int, query_tile: int, sample_share: float = 0.0,
+                       strips_by_pass=None) -> float:
     passes = math.ceil(B / max(query_tile, 1))
-    return passes * forward_index_bytes(N, P, wtype) * (1.0 + sample_share)
+    if strips_by_pass is None:
+        strips_by_pass = [0] * passes
+    assert len(strips_by_pass) == passes
+    return sum(forward_index_bytes(N, P_tail, wtype, h) for h in strips_by_pass) * (1.0 + sample_share)
 
 
 def term_parallel_bytes(U: int, wtype: str, sample_share: float = 0.0) -> float:

@@ -129,6 +129,49 @@ def test_tiny_all_scores(gs, tiny, mode, algo, build_kw):
     _dense_parity(gs, docs, queries, tiny.vocab, algo, **build_kw)
 
 
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+@pytest.mark.parametrize("qtile", [8, 16, 32, 64])
+@pytest.mark.parametrize("build_kw", [dict(), dict(head_max=-1), dict(head_max=64, head_density=0.02)])
+def test_doc_parallel_query_tiles(gs, mode, qtile, build_kw):
+    """Every query-tile width of the doc-parallel kernel: several passes with a ragged last one (B = 75),
+    with all / none / 64 of the lists as dense strips; scores element by element, then top-k."""
+    w = wl.make_workload("tiny", n_docs=3000, n_queries=75)
+    docs = w.docs if mode == "f32" else w.docs.to_u8()
+    queries = w.queries if mode == "f32" else w.queries.to_u8()
+    ix = gs.Index.from_numpy(docs, w.vocab, **build_kw)
+    S = ix.score_dense(*dev(queries), algo="doc", doc_query_tile=qtile).cpu().numpy()[:, :docs.rows]
+    R_d, R_q = oracle.as_rows(docs, w.vocab), oracle.as_rows(queries, w.vocab)
+    _, _, A = oracle.search(R_q, R_d, 1, all_scores=True)
+    if mode == "u8":
+        assert np.array_equal(S.astype(np.int64), A.astype(np.int64))
+    else:
+        assert np.all(np.abs(S.astype(np.float64) - A) <= parity.tol(A))
+    ids, sc = gpu_search(gs, ix, queries, 100, algo="doc", doc_query_tile=qtile)
+    compare(gs, docs, queries, w.vocab, 100, ids, sc)
+    ix.close()
+
+
+@pytest.mark.parametrize("qtile", [8, 32, 64])
+def test_doc_parallel_long_rows(gs, qtile):
+    """Documents far longer than the hit queue (128 entries) whose postings nearly all hit the query tile, and
+    queries with thousands of terms (query tile rows spill from shared memory to global memory)."""
+    rng = np.random.default_rng(7)
+    V, N, B = 30522, 257, 40
+    docs = csr_from_dicts([{int(t): float(np.float32(rng.uniform(0.1, 2.0))) for t in rng.choice(V, size=int(n), replace=False)}
+                           for n in rng.integers(1, 3000, size=N)], np.float32)
+    queries = csr_from_dicts([{int(t): float(np.float32(rng.uniform(0.1, 2.0))) for t in rng.choice(V, size=int(n), replace=False)}
+                              for n in rng.integers(1, 6000, size=B)], np.float32)
+    ix = gs.Index.from_numpy(docs, V)
+    S = ix.score_dense(*dev(queries), algo="doc", doc_query_tile=qtile).cpu().numpy()[:, :N]
+    R_d, R_q = oracle.as_rows(docs, V), oracle.as_rows(queries, V)
+    _, _, A = oracle.search(R_q, R_d, 1, all_scores=True)
+    # up to ~600 shared terms per pair: the fp32 bound is n * 2^-24 relative (DESIGN.md §3), beyond BASELINE's 1e-5
+    assert np.all(np.abs(S.astype(np.float64) - A) <= np.maximum(4e-5 * np.abs(A), 1e-6))
+    ids, sc = gpu_search(gs, ix, queries, 10, algo="doc", doc_query_tile=qtile)
+    assert ids.shape == (B, 10) and np.all(ids >= 0)
+    ix.close()
+
+
 @pytest.mark.parametrize("algo", ALGOS)
 @pytest.mark.parametrize("mode", ["f32", "u8"])
 @pytest.mark.parametrize("k", [1, 10, 33, 1000])

@@ -40,3 +40,10 @@ def test_our_models_closed_forms():
     assert rf.forward_index_bytes(3, 7, "u8") == 8 * 4 + 5 * 7
     assert rf.doc_parallel_bytes(3, 7, "f32", B=500, query_tile=16) == 32 * (32 + 56)
     assert rf.doc_parallel_bytes(3, 7, "f32", B=1, query_tile=16, sample_share=0.5) == 1.5 * 88
+    # hybrid forward index: 5 tail postings + strips read by the pass (4 B or 1 B per doc each)
+    assert rf.forward_index_bytes(3, 5, "f32", strips=2) == 32 + 40 + 24
+    assert rf.forward_index_bytes(3, 5, "u8", strips=2) == 32 + 25 + 6
+    indptr = np.array([0, 2, 3, 6], np.int64)
+    terms = np.array([5, 1, 9, 1, 2, 7], np.int32)
+    assert rf.strips_per_pass(indptr, terms, np.array([1, 2, 3]), query_tile=2) == [1, 2]
+    assert rf.doc_parallel_bytes(3, 5, "f32", B=3, query_tile=2, strips_by_pass=[1, 2]) == (32 + 40 + 12) + (32 + 40 + 24)
