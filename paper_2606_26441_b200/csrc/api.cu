@@ -332,6 +332,7 @@ gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_bu
                            gs_stream_t stream, gs_index_t** out) {
     if (out) *out = nullptr;
     if (!out || vocab_size <= 0) return GS_ERR_INVALID_ARG;
+    if (vocab_size > (1 << GS_FWD_DOC_SHIFT)) return GS_ERR_OUT_OF_RANGE;
     GS_TRY(check_device());
     GS_TRY(check_csr_host(docs, true));
     if (docs->rows >= 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;

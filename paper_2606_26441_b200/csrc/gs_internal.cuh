@@ -8,6 +8,7 @@
 
 #define GS_HEAD_MAX 32          // term-parallel: strips staged per tile / entries of a query's compact head list
 #define GS_STRIP_MAX 64         // dense strips kept by the index (the doc-parallel kernel uses all of them)
+#define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V <= 2^27)
 #define GS_SEL_BINS 2048        // radix-select digit: 11 bits
 #define GS_SEL_BITS 11
 
@@ -42,7 +43,7 @@ struct gs_index {
     // forward (doc-major) index — PAPER.md L174.  Hybrid layout: the H strip terms of a document live in the
     // dense strips below (column-major, 0 = absent); every other posting lives in this "tail" CSR.
     int64_t* fwd_indptr = nullptr;   // [N+1]
-    int32_t* fwd_terms = nullptr;    // [P_tail]
+    int32_t* fwd_terms = nullptr;    // [P_tail] term id | (doc & 31) << GS_FWD_DOC_SHIFT
     void* fwd_w = nullptr;           // [P_tail] float | uint8
     int64_t P_tail = 0;              // postings of the terms without a strip
     // inverted index — PAPER.md L79-90

@@ -131,7 +131,9 @@ __global__ void k_fill_strip(const int32_t* __restrict__ inv_doc, const W* __res
     if (i < len) strip[inv_doc[off + i]] = inv_w[off + i];
 }
 
-// forward "tail" CSR: the postings of a document whose term has no dense strip, in the row's order.
+// forward "tail" CSR: the postings of a document whose term has no dense strip, in the row's order.  The term
+// word also carries the document's position inside its aligned block of 32 documents (bits 27..31), so a warp
+// that streams a block's postings as one flat range knows the owner of each posting without a search.
 // One warp per document; pass 1 counts, pass 2 (after an exclusive scan) writes.
 __global__ void k_tail_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
                              const int16_t* __restrict__ head_slot, int64_t rows, int32_t V, int64_t* __restrict__ cnt) {
@@ -168,7 +170,7 @@ __global__ void k_tail_fill(const int64_t* __restrict__ indptr, const int32_t* _
         const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
         if (keep) {
             const int64_t o = dst + __popc(m & ((1u << lane) - 1u));
-            out_terms[o] = t;
+            out_terms[o] = t | (int32_t)((uint32_t)(warp & 31) << GS_FWD_DOC_SHIFT);
             out_w[o] = w[i];
         }
         dst += __popc(m);
@@ -280,26 +282,21 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         ix->fwd_terms = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)std::max<int64_t>(p_tail, 1), s);
         ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)std::max<int64_t>(p_tail, 1), s);
         if (!ix->fwd_indptr || !ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
-        if (ix->H == 0) {
-            GS_CUDA(cudaMemcpyAsync(ix->fwd_indptr, docs->indptr, sizeof(int64_t) * (size_t)(N + 1), cudaMemcpyDeviceToDevice, s));
-            if (P > 0) {
-                GS_CUDA(cudaMemcpyAsync(ix->fwd_terms, docs->term_ids, sizeof(int32_t) * (size_t)P, cudaMemcpyDeviceToDevice, s));
-                GS_CUDA(cudaMemcpyAsync(ix->fwd_w, docs->weights, sizeof(W) * (size_t)P, cudaMemcpyDeviceToDevice, s));
-            }
-        } else {
+        {
             int64_t* d_cnt = (int64_t*)tmp.get(sizeof(int64_t) * (size_t)(N + 1));
             if (!d_cnt) return GS_ERR_OOM;
             GS_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(int64_t) * (size_t)(N + 1), s));
-            k_tail_count<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, ix->head_slot, N, V, d_cnt);
+            if (N > 0) k_tail_count<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, ix->head_slot, N, V, d_cnt);
             size_t scan_bytes = 0;
             if (N + 1 > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
             GS_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
             void* d_scan_tmp = tmp.get(scan_bytes);
             if (!d_scan_tmp) return GS_ERR_OOM;
             GS_CUDA(cub::DeviceScan::ExclusiveSum(d_scan_tmp, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
-            k_tail_fill<W><<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, (const W*)docs->weights,
-                                                                ix->head_slot, N, V, ix->fwd_indptr, ix->fwd_terms,
-                                                                (W*)ix->fwd_w);
+            if (N > 0)
+                k_tail_fill<W><<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, (const W*)docs->weights,
+                                                                    ix->head_slot, N, V, ix->fwd_indptr, ix->fwd_terms,
+                                                                    (W*)ix->fwd_w);
             int64_t tail_end = 0;
             GS_CUDA(cudaMemcpyAsync(&tail_end, ix->fwd_indptr + N, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
             GS_CUDA(cudaStreamSynchronize(s));
