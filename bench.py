@@ -324,7 +324,7 @@ def run_ours(args):
                 "index": {"postings": info["nnz"], "padded_postings": info["padded_nnz"], "bytes_inverted": info["bytes_inverted"],
                           "bytes_forward": info["bytes_forward"], "bytes_head": info["bytes_head"],
                           "bytes_meta": info["bytes_inverted_meta"], "head_terms": info["head_terms"], "head_terms_term_parallel": info["head_terms_term_parallel"],
-                          "forward_tail_postings": info["forward_tail_nnz"], "tile_docs": info["tile_docs"],
+                          "forward_tail_postings": info["forward_tail_nnz"], "forward_padded_postings": info["forward_padded_nnz"], "tile_docs": info["tile_docs"],
                           "build_s": t_build, "generate_s": t_gen},
                 "context": {"paper_h100_qps": 787, "paper_h100_doc_parallel_hbm_frac": 0.626,
                             "note": "paper numbers are H100 + MS MARCO/SPLADE (PAPER.md L292, L340): context, not a baseline"}}
@@ -359,10 +359,10 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
            "useful_mac_per_step": ts["W"], "mac_per_s": ts["W"] / (kms * 1e-3)}
     if name == "score_doc":
         sp = rf.strips_per_pass(queries.indptr, queries.terms, head_terms, st["doc_query_tile"])
-        alg = rf.doc_parallel_bytes(info["num_docs"], info["forward_tail_nnz"], wtype, B, st["doc_query_tile"], share, sp)
-        one = rf.forward_index_bytes(info["num_docs"], info["forward_tail_nnz"], wtype, len(head_terms))
+        alg = rf.doc_parallel_bytes(info["num_docs"], info["forward_padded_nnz"], wtype, B, st["doc_query_tile"], share, sp)
+        one = rf.forward_index_bytes(info["num_docs"], info["forward_padded_nnz"], wtype, len(head_terms))
         out.update({"doc_query_tile": st["doc_query_tile"], "passes": st["doc_passes"], "bytes_per_step": alg,
-                    "bytes_model": "sum_passes(8*(N+1)+(4+w)*P_tail+w*N*strips_used(pass))*(1+sample share)",
+                    "bytes_model": "sum_passes(8*(N/32+1)+(4+w)*P_fwd+w*N*strips_used(pass))*(1+sample share), P_fwd = tail postings padded per 32-doc block",
                     "strips_used_per_pass_mean": float(np.mean(sp)) if sp else 0.0, "bytes_one_pass": one,
                     "frac_one_pass": rf.effective_gbps(one, kms) / peaks["hbm_gbs"]})
     else:

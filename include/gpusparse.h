@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define GS_ABI_VERSION 2
+#define GS_ABI_VERSION 3
 #if defined(__GNUC__)
 #define GS_API __attribute__((visibility("default")))
 #else
@@ -104,13 +104,15 @@ typedef struct gs_info {
     int32_t head_terms;        /* number of dense-strip posting lists                                 */
     int64_t bytes_inverted;    /* doc_ids + weights of the padded lists            Eq. (3)            */
     int64_t bytes_inverted_meta; /* offsets + lengths + tile-segment table                            */
-    int64_t bytes_forward;     /* forward index, CSR part: indptr + term ids + weights of the postings
-                                  whose term has no strip (the strips are its dense part)             */
+    int64_t bytes_forward;     /* forward index, CSR part: one row pointer per block of 32 documents + term
+                                  words + weights of the postings whose term has no strip, each block padded
+                                  to 128 postings (the strips are the dense part of the forward index)  */
     int64_t bytes_head;        /* dense strips                                                        */
     int64_t bytes_total;
     int64_t forward_tail_nnz;  /* postings held by the CSR part of the forward index                  */
     int32_t head_terms_term_parallel; /* strips the term-parallel kernel stages per tile (<= 32)      */
     int32_t reserved;
+    int64_t forward_padded_nnz; /* slots of the CSR part: forward_tail_nnz + block padding             */
 } gs_info_t;
 
 /* Search options; pass NULL for defaults. */

@@ -53,7 +53,8 @@ class gs_info_t(ctypes.Structure):
                 ("tile_docs", ctypes.c_int32), ("num_tiles", ctypes.c_int32), ("head_terms", ctypes.c_int32),
                 ("bytes_inverted", ctypes.c_int64), ("bytes_inverted_meta", ctypes.c_int64),
                 ("bytes_forward", ctypes.c_int64), ("bytes_head", ctypes.c_int64), ("bytes_total", ctypes.c_int64),
-                ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("forward_padded_nnz", ctypes.c_int64)]
 
 
 class gs_search_opts_t(ctypes.Structure):

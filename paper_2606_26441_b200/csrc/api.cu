@@ -141,7 +141,7 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
         p.group = o->query_group;
         p.qtile = o->doc_query_tile;
     }
-    if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : (B <= 16 ? 16 : 32);   // doc-parallel: queries per pass over the forward index
+    if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : 16;   // doc-parallel: queries per pass; 16 is the largest tile that stays HBM bound
     p.use_head = !(p.flags & GS_FLAG_NO_HEAD_STRIPS);
     int shift = (o && o->sample_shift > 0) ? o->sample_shift : 5;
     // the sample must hold comfortably more than k documents, else its k-th key is a weak bound
@@ -332,7 +332,7 @@ gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_bu
                            gs_stream_t stream, gs_index_t** out) {
     if (out) *out = nullptr;
     if (!out || vocab_size <= 0) return GS_ERR_INVALID_ARG;
-    if (vocab_size > (1 << GS_FWD_DOC_SHIFT)) return GS_ERR_OUT_OF_RANGE;
+    if (vocab_size >= (1 << GS_FWD_DOC_SHIFT)) return GS_ERR_OUT_OF_RANGE;
     GS_TRY(check_device());
     GS_TRY(check_csr_host(docs, true));
     if (docs->rows >= 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
@@ -364,7 +364,7 @@ gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_bu
 void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
-    void* ptrs[] = {ix->fwd_indptr, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
+    void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
                     ix->seg, ix->head_slot, ix->head_strip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
@@ -378,6 +378,7 @@ gs_status_t gs_index_info(const gs_index_t* ix, gs_info_t* out) {
     out->bytes_inverted = ix->bytes_inverted; out->bytes_inverted_meta = ix->bytes_meta;
     out->bytes_forward = ix->bytes_forward; out->bytes_head = ix->bytes_head;
     out->head_terms_term_parallel = ix->H_term; out->forward_tail_nnz = ix->P_tail;
+    out->forward_padded_nnz = ix->P_fwd; out->reserved = 0;
     out->bytes_total = ix->bytes_inverted + ix->bytes_meta + ix->bytes_forward + ix->bytes_head;
     return GS_OK;
 }

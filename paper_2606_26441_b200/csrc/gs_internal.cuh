@@ -8,7 +8,8 @@
 
 #define GS_HEAD_MAX 32          // term-parallel: strips staged per tile / entries of a query's compact head list
 #define GS_STRIP_MAX 64         // dense strips kept by the index (the doc-parallel kernel uses all of them)
-#define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V <= 2^27)
+#define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
+#define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings
 #define GS_SEL_BINS 2048        // radix-select digit: 11 bits
 #define GS_SEL_BITS 11
 
@@ -41,11 +42,14 @@ struct gs_index {
     int32_t ntiles = 0;       // ceil(N / Ts)
     int64_t N_pad = 0;        // ntiles * Ts
     // forward (doc-major) index — PAPER.md L174.  Hybrid layout: the H strip terms of a document live in the
-    // dense strips below (column-major, 0 = absent); every other posting lives in this "tail" CSR.
-    int64_t* fwd_indptr = nullptr;   // [N+1]
-    int32_t* fwd_terms = nullptr;    // [P_tail] term id | (doc & 31) << GS_FWD_DOC_SHIFT
-    void* fwd_w = nullptr;           // [P_tail] float | uint8
+    // dense strips below (column-major, 0 = absent); every other posting lives in this "tail" block CSR: one
+    // row pointer per aligned block of 32 documents, each block's range padded to GS_FWD_CHUNK postings.
+    int64_t* fwd_blk = nullptr;      // [n_blk+1] start of each block's range (multiple of GS_FWD_CHUNK)
+    uint32_t* fwd_terms = nullptr;   // [P_fwd] term id | (doc & 31) << GS_FWD_DOC_SHIFT; padding = V | 31 << shift
+    void* fwd_w = nullptr;           // [P_fwd] float | uint8 (0 in the padding)
+    int64_t n_blk = 0;               // ceil(N / 32)
     int64_t P_tail = 0;              // postings of the terms without a strip
+    int64_t P_fwd = 0;               // P_tail + block padding
     // inverted index — PAPER.md L79-90
     int64_t* inv_off = nullptr;      // [V+1] start of each padded list (multiple of 32)
     int32_t* inv_len = nullptr;      // [V]   true list length

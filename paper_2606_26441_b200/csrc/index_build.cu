@@ -131,12 +131,14 @@ __global__ void k_fill_strip(const int32_t* __restrict__ inv_doc, const W* __res
     if (i < len) strip[inv_doc[off + i]] = inv_w[off + i];
 }
 
-// forward "tail" CSR: the postings of a document whose term has no dense strip, in the row's order.  The term
-// word also carries the document's position inside its aligned block of 32 documents (bits 27..31), so a warp
-// that streams a block's postings as one flat range knows the owner of each posting without a search.
-// One warp per document; pass 1 counts, pass 2 (after an exclusive scan) writes.
+// forward "tail" index: the postings of a document whose term has no dense strip, in the row's order, stored per
+// aligned block of 32 documents as ONE flat range padded to a multiple of GS_FWD_CHUNK postings.  The term word also
+// carries the document's position inside its block (bits 27..31), so a warp that streams a block's range with
+// 128-bit loads knows the owner of each posting without a search; padding slots hold the term id V (never a query
+// term) at position 31 with weight 0.  One warp per document counts, one warp per block lays the block out, one
+// warp per document writes.
 __global__ void k_tail_count(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
-                             const int16_t* __restrict__ head_slot, int64_t rows, int32_t V, int64_t* __restrict__ cnt) {
+                             const int16_t* __restrict__ head_slot, int64_t rows, int32_t V, int32_t* __restrict__ cnt) {
     const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (warp >= rows) return;
@@ -150,15 +152,40 @@ __global__ void k_tail_count(const int64_t* __restrict__ indptr, const int32_t* 
     if (lane == 0) cnt[warp] = n;
 }
 
+// lane = document of the block: start of the document inside the block, padded size of the block
+__global__ void k_blk_layout(const int32_t* __restrict__ cnt, int64_t rows, int64_t nblk, int32_t* __restrict__ doc_rel,
+                             int64_t* __restrict__ blk_cnt, unsigned long long* __restrict__ true_total) {
+    const int64_t blk = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (blk >= nblk) return;
+    const int64_t doc = blk * 32 + lane;
+    const int c = doc < rows ? cnt[doc] : 0;
+    int incl = c;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (doc < rows) doc_rel[doc] = incl - c;
+    if (lane == 31) {
+        blk_cnt[blk] = ((int64_t)incl + GS_FWD_CHUNK - 1) / GS_FWD_CHUNK * GS_FWD_CHUNK;
+        atomicAdd(true_total, (unsigned long long)incl);
+    }
+}
+
+__global__ void k_fill_u32(uint32_t* __restrict__ p, int64_t n, uint32_t v) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) p[i] = v;
+}
+
 template <typename W>
 __global__ void k_tail_fill(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms, const W* __restrict__ w,
                             const int16_t* __restrict__ head_slot, int64_t rows, int32_t V,
-                            const int64_t* __restrict__ tail_indptr, int32_t* __restrict__ out_terms, W* __restrict__ out_w) {
+                            const int64_t* __restrict__ fwd_blk, const int32_t* __restrict__ doc_rel,
+                            uint32_t* __restrict__ out_terms, W* __restrict__ out_w) {
     const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (warp >= rows) return;
     const int64_t a = indptr[warp], b = indptr[warp + 1];
-    int64_t dst = tail_indptr[warp];
+    int64_t dst = fwd_blk[warp >> 5] + doc_rel[warp];
     for (int64_t i0 = a; i0 < b; i0 += 32) {
         const int64_t i = i0 + lane;
         int32_t t = -1;
@@ -170,7 +197,7 @@ __global__ void k_tail_fill(const int64_t* __restrict__ indptr, const int32_t* _
         const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
         if (keep) {
             const int64_t o = dst + __popc(m & ((1u << lane) - 1u));
-            out_terms[o] = t | (int32_t)((uint32_t)(warp & 31) << GS_FWD_DOC_SHIFT);
+            out_terms[o] = (uint32_t)t | ((uint32_t)(warp & 31) << GS_FWD_DOC_SHIFT);
             out_w[o] = w[i];
         }
         dst += __popc(m);
@@ -273,36 +300,53 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     if (!ix->head_slot) return GS_ERR_OOM;
     GS_CUDA(cudaMemcpyAsync(ix->head_slot, h_slot.data(), sizeof(int16_t) * (size_t)V, cudaMemcpyHostToDevice, s));
 
-    // ---- forward index, hybrid: strips for the H densest lists + a CSR of every other posting
+    // ---- forward index, hybrid: strips for the H densest lists + a block CSR of every other posting
     {
         int64_t p_tail = P;
         for (int h = 0; h < ix->H; ++h) p_tail -= h_len[order[h]];
         ix->P_tail = p_tail;
-        ix->fwd_indptr = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(N + 1), s);
-        ix->fwd_terms = (int32_t*)gs_dev_alloc(ix, sizeof(int32_t) * (size_t)std::max<int64_t>(p_tail, 1), s);
-        ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)std::max<int64_t>(p_tail, 1), s);
-        if (!ix->fwd_indptr || !ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
-        {
-            int64_t* d_cnt = (int64_t*)tmp.get(sizeof(int64_t) * (size_t)(N + 1));
-            if (!d_cnt) return GS_ERR_OOM;
-            GS_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(int64_t) * (size_t)(N + 1), s));
-            if (N > 0) k_tail_count<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, ix->head_slot, N, V, d_cnt);
-            size_t scan_bytes = 0;
-            if (N + 1 > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-            GS_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
-            void* d_scan_tmp = tmp.get(scan_bytes);
-            if (!d_scan_tmp) return GS_ERR_OOM;
-            GS_CUDA(cub::DeviceScan::ExclusiveSum(d_scan_tmp, scan_bytes, d_cnt, ix->fwd_indptr, (int)(N + 1), s));
-            if (N > 0)
-                k_tail_fill<W><<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, (const W*)docs->weights,
-                                                                    ix->head_slot, N, V, ix->fwd_indptr, ix->fwd_terms,
-                                                                    (W*)ix->fwd_w);
-            int64_t tail_end = 0;
-            GS_CUDA(cudaMemcpyAsync(&tail_end, ix->fwd_indptr + N, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
-            GS_CUDA(cudaStreamSynchronize(s));
-            if (tail_end != p_tail) return GS_ERR_OUT_OF_RANGE;     // some term id was outside [0,V) (validate off)
+        const int64_t nblk = (N + 31) / 32;
+        ix->n_blk = nblk;
+        ix->fwd_blk = (int64_t*)gs_dev_alloc(ix, sizeof(int64_t) * (size_t)(nblk + 1), s);
+        if (!ix->fwd_blk) return GS_ERR_OOM;
+        int32_t* d_cnt = (int32_t*)tmp.get(sizeof(int32_t) * (size_t)std::max<int64_t>(N, 1));
+        int32_t* d_rel = (int32_t*)tmp.get(sizeof(int32_t) * (size_t)std::max<int64_t>(N, 1));
+        int64_t* d_blk_cnt = (int64_t*)tmp.get(sizeof(int64_t) * (size_t)(nblk + 1));
+        unsigned long long* d_true = (unsigned long long*)tmp.get(sizeof(unsigned long long));
+        if (!d_cnt || !d_rel || !d_blk_cnt || !d_true) return GS_ERR_OOM;
+        GS_CUDA(cudaMemsetAsync(d_blk_cnt, 0, sizeof(int64_t) * (size_t)(nblk + 1), s));
+        GS_CUDA(cudaMemsetAsync(d_true, 0, sizeof(unsigned long long), s));
+        if (N > 0) {
+            k_tail_count<<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, ix->head_slot, N, V, d_cnt);
+            k_blk_layout<<<grid_for(nblk * 32), kThreads, 0, s>>>(d_cnt, N, nblk, d_rel, d_blk_cnt, d_true);
         }
-        ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(N + 1) + (sizeof(int32_t) + sizeof(W)) * (size_t)p_tail);
+        if (nblk + 1 > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+        size_t scan_bytes = 0;
+        GS_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, d_blk_cnt, ix->fwd_blk, (int)(nblk + 1), s));
+        void* d_scan_tmp = tmp.get(scan_bytes);
+        if (!d_scan_tmp) return GS_ERR_OOM;
+        GS_CUDA(cub::DeviceScan::ExclusiveSum(d_scan_tmp, scan_bytes, d_blk_cnt, ix->fwd_blk, (int)(nblk + 1), s));
+        int64_t p_fwd = 0;
+        unsigned long long true_total = 0;
+        GS_CUDA(cudaMemcpyAsync(&p_fwd, ix->fwd_blk + nblk, sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaMemcpyAsync(&true_total, d_true, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaStreamSynchronize(s));
+        if ((int64_t)true_total != p_tail) return GS_ERR_OUT_OF_RANGE;     // some term id was outside [0,V) (validate off)
+        ix->P_fwd = p_fwd;
+        ix->fwd_terms = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)std::max<int64_t>(p_fwd, 1), s);
+        ix->fwd_w = gs_dev_alloc(ix, sizeof(W) * (size_t)std::max<int64_t>(p_fwd, 1), s);
+        if (!ix->fwd_terms || !ix->fwd_w) return GS_ERR_OOM;
+        if (p_fwd > 0) {
+            int dev = 0, sms = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            k_fill_u32<<<sms * 8, 512, 0, s>>>(ix->fwd_terms, p_fwd, (uint32_t)V | (31u << GS_FWD_DOC_SHIFT));
+            GS_CUDA(cudaMemsetAsync(ix->fwd_w, 0, sizeof(W) * (size_t)p_fwd, s));
+            k_tail_fill<W><<<grid_for(N * 32), kThreads, 0, s>>>(docs->indptr, docs->term_ids, (const W*)docs->weights,
+                                                                ix->head_slot, N, V, ix->fwd_blk, d_rel, ix->fwd_terms,
+                                                                (W*)ix->fwd_w);
+        }
+        ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(nblk + 1) + (sizeof(uint32_t) + sizeof(W)) * (size_t)p_fwd);
     }
 
     // ---- padded inverted arrays, pre-filled with the sentinel (doc_id=-1, score=0), L90

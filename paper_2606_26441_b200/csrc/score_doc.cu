@@ -7,58 +7,72 @@
 // query (76.3 GB per 500-query batch at 100K docs, Table 7) and names inner-loop
 // instruction overhead as what keeps it at 62.6 % of peak (L179).
 //
-// Here the forward index is streamed ONCE per tile of QT queries, and it is a hybrid:
+// Here the forward index is streamed ONCE per tile of QT queries (one launch per tile = "pass"), and
+// it is a hybrid:
 //   * the H densest posting lists are dense strips [H][N_pad] (0 = term absent).  For them there is
 //     nothing to look up: a thread owns one document, keeps QT accumulators in registers and does
-//     x[h][doc] * Q[h][q] with Q broadcast from shared memory — a small dense contraction that carries
-//     ~85 % of the multiply-adds of the synthetic MS MARCO stand-in at 1 instruction per 32 of them;
-//   * every other posting sits in a "tail" CSR whose term word also carries the document's position
-//     in its aligned block of 32 documents.  A warp owns such a block and streams its postings as ONE
-//     flat range (coalesced, 8 independent loads in flight, next chunk prefetched), tests each term
-//     against a V-bit bitmap of the tile's tail terms (shared memory) and compacts the hits, in
-//     stream order, into a per-warp queue.  Then lane d walks the hits of document d (they are
-//     contiguous in the queue: a binary search finds them): term -> row through a popcount prefix,
-//     row -> its (query, weight) pairs in a small CSR, accumulate into the lane's own row of a
-//     [32][QT+1] shared-memory tile (odd stride: no two lanes share a bank by construction of the
-//     row, no atomics, fixed order).
+//     acc[q] += x[h][doc] * Q[h][q].  Q, the tile's head weights, is copied into CONSTANT memory
+//     before the pass's launch, so every multiplier is a uniform-register operand of the FFMA/IMAD
+//     itself: no shared-memory or register traffic for the ~85 % of the multiply-adds the head
+//     lists carry (a broadcast LDS.128 feeds only 4 FMAs and costs 4 LSU cycles, which bounds the
+//     contraction at a quarter of the FMA rate; measured in DESIGN.md §6);
+//   * every other posting sits in a "tail" block CSR: one row pointer per aligned block of 32
+//     documents, the block's postings one flat range padded to 128, the term word carrying the
+//     document's position in the block.  A warp owns a block and streams its range with 128-bit
+//     loads (next chunk prefetched, next block's first chunk prefetched across the contraction),
+//     tests each term against a V-bit bitmap of the tile's tail terms (shared memory) and compacts
+//     the hits, in stream order, into a per-warp queue (one ballot prefix per 128 postings).  Then
+//     lane d walks the hits of document d (contiguous in the queue: a binary search finds them) in
+//     ONE flattened loop over (hit, pair): term -> row through a popcount prefix, row -> its
+//     (query, weight) pairs, accumulate into the lane's own row of a [32][QT+1] shared-memory tile
+//     (odd stride: no two lanes share a bank, no atomics, fixed order).
 // Each (query, doc) cell is produced by exactly one thread in a fixed order — zero atomics,
-// deterministic.  The query tile (bitmap + popcount prefix, row CSR, head weights [H'][QT]) is built
-// once per pass by k_build_qtile and staged into shared memory.
+// deterministic.  The query tiles (bitmap + popcount prefix, row table, head weights, thresholds)
+// are built once per search by k_build_qtile.
 #include <algorithm>
+#include <cstddef>
+#include <mutex>
+#include <type_traits>
 
 #include "gs_internal.cuh"
 
 namespace {
 
 constexpr uint32_t kTermMask = (1u << GS_FWD_DOC_SHIFT) - 1u;
+constexpr int kMaxQT = 64;
 
-struct QTileHdr {
-    uint32_t R;          // distinct tail terms of the tile (rows)
-    uint32_t nh;         // strips some query of the tile uses
-    uint32_t np;         // (row, query) pairs
-    uint32_t row_off;    // this pass's slice of the shared rowptr array
-    uint32_t pair_off;   // ... and of the shared pairs array
+// What a pass needs with warp-uniform access.  Built in the search workspace by k_build_qtile, copied to
+// c_tile before the pass's launch (stream ordered).  qh is last: a pass copies only its [GS_STRIP_MAX][QT] prefix.
+struct ConstTile {
+    uint32_t nh;                         // strips some query of the tile uses, rounded up to a multiple of 4 (zero rows)
+    uint32_t R;                          // distinct tail terms of the tile (rows)
+    uint32_t np;                         // (row, query) pairs
+    uint32_t row_off;                    // this pass's slice of the shared row array
+    uint32_t pair_off;                   // ... and of the shared pairs array
     uint32_t pad[3];
-    uint32_t hl[GS_STRIP_MAX];
+    uint32_t hl[GS_STRIP_MAX];           // compact position -> strip number (0 beyond nh)
+    uint32_t thr_s[kMaxQT];              // threshold as a score (accumulator bits); "accept all" = NaN / INT32_MIN
+    unsigned long long thr_key[kMaxQT];  // threshold as a key; queries beyond the tile: all ones
+    uint32_t qh[GS_STRIP_MAX * kMaxQT];  // [compact strip][QT] accumulator-typed head weights, row stride QT
 };
+__constant__ ConstTile c_tile;
 
+__host__ __device__ inline size_t tile_copy_bytes(int QT) { return offsetof(ConstTile, qh) + (size_t)GS_STRIP_MAX * QT * 4; }
 __host__ __device__ inline int bm_words(int32_t V) { return ((V + 1 + 31) / 32 + 3) / 4 * 4; }
-// per-pass scratch block: hdr | bitmap[Wd] | prefix[Wd] | Qh[GS_STRIP_MAX][QT]
-__host__ __device__ inline size_t off_bm() { return sizeof(QTileHdr); }
-__host__ __device__ inline size_t off_pre(int Wd) { return off_bm() + (size_t)Wd * 4; }
-__host__ __device__ inline size_t off_qh(int Wd) { return off_pre(Wd) + (size_t)Wd * 4; }
-__host__ __device__ inline size_t pass_bytes(int Wd, int QT) {
-    return (off_qh(Wd) + (size_t)GS_STRIP_MAX * QT * 4 + 255) / 256 * 256;
-}
-// after the pass blocks: rowptr[nnz + passes + 1] | cursor[nnz + passes + 1] | pairs[nnz] (uint2)
-struct SharedScratch { uint32_t* rowptr; uint32_t* cursor; uint2* pairs; };
-__host__ __device__ inline SharedScratch shared_scratch(unsigned char* scratch, int Wd, int QT, int64_t passes, int64_t nnz) {
-    unsigned char* p = scratch + pass_bytes(Wd, QT) * (size_t)passes;
-    const size_t n1 = ((size_t)(nnz + passes + 1) * 4 + 255) / 256 * 256;
+// per-pass scratch block: ConstTile | bitmap[Wd] | prefix[Wd]
+__host__ __device__ inline size_t off_bm() { return (sizeof(ConstTile) + 255) / 256 * 256; }
+__host__ __device__ inline size_t pass_bytes(int Wd) { return (off_bm() + (size_t)Wd * 8 + 255) / 256 * 256; }
+// after the pass blocks: rowptr[n1] | cursor[n1] | rows[n1] (uint2: first pair, end pair) | pairs[nnz] (uint2),  n1 = nnz + passes + 1
+struct SharedScratch { uint32_t* rowptr; uint32_t* cursor; uint2* rows; uint2* pairs; };
+__host__ __device__ inline size_t up256(size_t b) { return (b + 255) / 256 * 256; }
+__host__ __device__ inline SharedScratch shared_scratch(unsigned char* scratch, int Wd, int64_t passes, int64_t nnz) {
+    unsigned char* p = scratch + pass_bytes(Wd) * (size_t)passes;
+    const size_t n1 = (size_t)(nnz + passes + 1);
     SharedScratch s;
     s.rowptr = reinterpret_cast<uint32_t*>(p);
-    s.cursor = reinterpret_cast<uint32_t*>(p + n1);
-    s.pairs = reinterpret_cast<uint2*>(p + 2 * n1);
+    s.cursor = reinterpret_cast<uint32_t*>(p + up256(n1 * 4));
+    s.rows = reinterpret_cast<uint2*>(p + 2 * up256(n1 * 4));
+    s.pairs = reinterpret_cast<uint2*>(p + 2 * up256(n1 * 4) + up256(n1 * 8));
     return s;
 }
 
@@ -88,12 +102,33 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t local, uint32_t* wa
     return warp_tot[warp] + incl - local;
 }
 
+template <int WT> struct NumD;
+template <> struct NumD<GS_W_F32> {
+    using W = float; using A = float;
+    static __device__ __forceinline__ A mac(A acc, A q, A w) { return fmaf(q, w, acc); }
+    static __device__ __forceinline__ A widen(W w) { return w; }
+    static __device__ __forceinline__ A from_bits(uint32_t b) { return __uint_as_float(b); }
+    static __device__ __forceinline__ uint32_t bits(A a) { return __float_as_uint(a); }
+    static __device__ __forceinline__ uint32_t thr_score_bits(uint32_t ord) { return gs_unord_f32(ord); }   // NaN for ord 0
+    static __device__ __forceinline__ uint32_t reject_all_bits() { return 0x7F800000u; }                    // +inf
+};
+template <> struct NumD<GS_W_U8> {
+    using W = uint8_t; using A = int32_t;
+    static __device__ __forceinline__ A mac(A acc, A q, A w) { return acc + q * w; }
+    static __device__ __forceinline__ A widen(W w) { return (int32_t)w; }
+    static __device__ __forceinline__ A from_bits(uint32_t b) { return (int32_t)b; }
+    static __device__ __forceinline__ uint32_t bits(A a) { return (uint32_t)a; }
+    static __device__ __forceinline__ uint32_t thr_score_bits(uint32_t ord) { return ord ^ 0x80000000u; }   // INT32_MIN for ord 0
+    static __device__ __forceinline__ uint32_t reject_all_bits() { return 0x7FFFFFFFu; }                    // INT32_MAX
+};
+
 // ---- build the query tile of pass `blockIdx.x` (one CTA of 1024 threads per pass)
 template <int WT>
 __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
                                                       const void* __restrict__ weights, const int16_t* __restrict__ head_slot,
                                                       int H, int64_t q0, int64_t nq, int QT, int32_t V, int Wd,
-                                                      unsigned char* __restrict__ scratch, int64_t n_passes, int64_t nnz_cap) {
+                                                      const uint64_t* __restrict__ thr, unsigned char* __restrict__ scratch,
+                                                      int64_t n_passes, int64_t nnz_cap) {
     extern __shared__ uint32_t sm[];                  // bitmap[Wd], prefix[Wd]
     __shared__ uint32_t warp_tot[32];
     __shared__ uint32_t s_hmask[2];
@@ -103,16 +138,16 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
     const int pass = blockIdx.x;
     const int64_t qa = q0 + (int64_t)pass * QT;
     const int nqt = (int)min((int64_t)QT, q0 + nq - qa);
-    unsigned char* base = scratch + (size_t)pass * pass_bytes(Wd, QT);
-    QTileHdr* hdr = reinterpret_cast<QTileHdr*>(base);
+    unsigned char* base = scratch + (size_t)pass * pass_bytes(Wd);
+    ConstTile* ct = reinterpret_cast<ConstTile*>(base);
     uint32_t* g_bm = reinterpret_cast<uint32_t*>(base + off_bm());
-    uint32_t* g_pre = reinterpret_cast<uint32_t*>(base + off_pre(Wd));
-    uint32_t* g_qh = reinterpret_cast<uint32_t*>(base + off_qh(Wd));
-    const SharedScratch ss = shared_scratch(scratch, Wd, QT, n_passes, nnz_cap);
+    uint32_t* g_pre = g_bm + Wd;
+    const SharedScratch ss = shared_scratch(scratch, Wd, n_passes, nnz_cap);
     const uint32_t pair_off = (uint32_t)(indptr[qa] - indptr[q0]);
     const uint32_t row_off = pair_off + (uint32_t)pass;
     uint32_t* rowptr = ss.rowptr + row_off;
     uint32_t* cursor = ss.cursor + row_off;
+    uint2* rows = ss.rows + row_off;
     uint2* pairs = ss.pairs + pair_off;
 
     for (int i = threadIdx.x; i < Wd; i += blockDim.x) bm[i] = 0;
@@ -144,15 +179,27 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
     if (threadIdx.x == 0) {   // compact list of the strips some query of the tile uses, padded to a multiple of 4
         uint32_t n = 0;
         for (int h = 0; h < H; ++h)
-            if ((s_hmask[h >> 5] >> (h & 31)) & 1u) hdr->hl[n++] = (uint32_t)h;
-        hdr->nh = n;
-        while (n & 3u) hdr->hl[n++] = 0u;           // padding rows carry zero weights
-        hdr->R = R;
-        hdr->row_off = row_off;
-        hdr->pair_off = pair_off;
+            if ((s_hmask[h >> 5] >> (h & 31)) & 1u) ct->hl[n++] = (uint32_t)h;
+        const uint32_t n4 = (n + 3u) & ~3u;
+        for (uint32_t i = n; i < GS_STRIP_MAX; ++i) ct->hl[i] = 0u;      // padding rows carry zero weights
+        ct->nh = n4;
+        ct->R = R;
+        ct->row_off = row_off;
+        ct->pair_off = pair_off;
+    }
+    for (int i = threadIdx.x; i < kMaxQT; i += blockDim.x) {
+        // thresholds of the tile's queries (filter phase); without thresholds every cell is accepted
+        uint64_t key = ~0ull;
+        uint32_t sb = NumD<WT>::reject_all_bits();
+        if (i < nqt) {
+            key = thr ? thr[qa + i] : 0ull;
+            sb = NumD<WT>::thr_score_bits((uint32_t)(key >> 32));
+        }
+        ct->thr_key[i] = key;
+        ct->thr_s[i] = sb;
     }
     for (int i = threadIdx.x; i < Wd; i += blockDim.x) { g_bm[i] = bm[i]; g_pre[i] = pre[i]; }
-    for (int i = threadIdx.x; i < GS_STRIP_MAX * QT; i += blockDim.x) g_qh[i] = 0u;
+    for (int i = threadIdx.x; i < GS_STRIP_MAX * QT; i += blockDim.x) ct->qh[i] = 0u;
     for (uint32_t i = threadIdx.x; i <= R; i += blockDim.x) cursor[i] = 0u;
     __syncthreads();
     // pairs per row
@@ -172,13 +219,15 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
         uint32_t run = block_excl_scan(local, warp_tot, &s_total);
         for (uint32_t r = r0; r < r1; ++r) {
             rowptr[r] = run;
+            rows[r] = make_uint2(run, run + cursor[r]);
             run += cursor[r];
         }
     }
     __syncthreads();
-    if (threadIdx.x == 0) { rowptr[R] = s_total; hdr->np = s_total; }
+    if (threadIdx.x == 0) { rowptr[R] = s_total; ct->np = s_total; }
     for (uint32_t i = threadIdx.x; i <= R; i += blockDim.x) cursor[i] = 0u;
     __syncthreads();
+    // queries in order, so the pairs of a row are sorted by query: a fixed accumulation order
     for (int j = 0; j < nqt; ++j) {
         const int64_t a = indptr[qa + j], e = indptr[qa + j + 1];
         for (int64_t i = a + threadIdx.x; i < e; i += blockDim.x) {
@@ -192,7 +241,7 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                 const uint32_t below = hs < 32 ? (s_hmask[0] & ((1u << hs) - 1u))
                                                : (s_hmask[1] & ((1u << (hs - 32)) - 1u));
                 const int ci = __popc(below) + (hs >= 32 ? __popc(s_hmask[0]) : 0);
-                g_qh[(size_t)ci * QT + j] = w;
+                ct->qh[(size_t)ci * QT + j] = w;
             } else {
                 const uint32_t word = bm[t >> 5];
                 const uint32_t r = pre[t >> 5] + __popc(word & ((1u << (t & 31)) - 1u));
@@ -200,48 +249,102 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                 pairs[rowptr[r] + pos] = make_uint2((uint32_t)j, w);
             }
         }
+        __syncthreads();
     }
 }
 
-template <int WT> struct NumD;
-template <> struct NumD<GS_W_F32> {
-    using W = float; using A = float;
-    static __device__ __forceinline__ A mac(A acc, A q, A w) { return fmaf(q, w, acc); }
-    static __device__ __forceinline__ A widen(W w) { return w; }
-    static __device__ __forceinline__ A from_bits(uint32_t b) { return __uint_as_float(b); }
-    static __device__ __forceinline__ uint32_t bits(A a) { return __float_as_uint(a); }
-    static __device__ __forceinline__ A thr_score(uint32_t ord) { return __uint_as_float(gs_unord_f32(ord)); }  // NaN for 0
-};
-template <> struct NumD<GS_W_U8> {
-    using W = uint8_t; using A = int32_t;
-    static __device__ __forceinline__ A mac(A acc, A q, A w) { return acc + q * w; }
-    static __device__ __forceinline__ A widen(W w) { return (int32_t)w; }
-    static __device__ __forceinline__ A from_bits(uint32_t b) { return (int32_t)b; }
-    static __device__ __forceinline__ uint32_t bits(A a) { return (uint32_t)a; }
-    static __device__ __forceinline__ A thr_score(uint32_t ord) { return (int32_t)(ord ^ 0x80000000u); }
-};
-
 struct DocParams {
-    const int64_t* fwd_indptr; const int32_t* fwd_terms; const void* fwd_w;
+    const int64_t* fwd_blk; const uint32_t* fwd_terms; const void* fwd_w;
     const void* strips; int64_t N_pad;
     int64_t N; int32_t V; int32_t Ts; int32_t Wd;
-    const unsigned char* scratch; const uint32_t* rowptr; const uint2* pairs;   // shared rowptr / pairs arrays
-    int32_t sparse_cap_bytes;                   // shared memory left for a pass's row CSR
-    int64_t q0; int32_t nq;                     // queries [q0, q0+nq) in tiles of QT
+    const uint32_t* tile_bm;                    // this pass's bitmap[Wd] | prefix[Wd]
+    const uint2* rows; const uint2* pairs;      // shared row / pairs arrays (the pass's slices start at c_tile.row_off / pair_off)
+    int32_t sparse_cap_bytes;                   // shared memory left for a pass's row table + pairs
+    int64_t qa; int32_t nqt;                    // queries [qa, qa+nqt) of the batch; q_rel = qa - q0 of the launch
+    int64_t q_rel;
     gs_tileset ts;
     gs_sink sink;
-    int32_t ctas_per_pass;
 };
 
 template <int QT> struct Geo {
     static constexpr int AST = QT + 1;                 // row stride of the accumulator tile (odd: lane rows hit distinct banks)
     static constexpr int NW = QT <= 16 ? 32 : (QT == 32 ? 20 : 12);              // warps per CTA
-    static constexpr int QCAP = QT <= 8 ? 384 : (QT == 16 ? 512 : (QT == 32 ? 640 : 896));   // hit-queue entries per warp
+    // hit-queue entries per warp: a block's hits (281 / 536 / 838 on average at QT = 16 / 32 / 64 on the MS MARCO
+    // stand-in) should fit, because a walk over part of a block leaves the lanes of the other documents idle
+    static constexpr int QCAP = QT <= 8 ? 640 : (QT == 16 ? 512 : (QT == 32 ? 768 : 1152));
     static constexpr size_t per_warp = (size_t)QCAP * 8 + (size_t)32 * AST * 4;
-    static __host__ __device__ size_t fixed(int Wd) {
-        return (size_t)GS_STRIP_MAX * QT * 4 + (size_t)QT * 8 + (size_t)QT * 4 + GS_STRIP_MAX * 4 + (size_t)Wd * 8;
-    }
+    static __host__ __device__ size_t fixed(int Wd) { return (size_t)Wd * 8; }
 };
+
+__device__ __forceinline__ uint4 ld_stream4(const uint4* p) { return __ldcs(p); }
+__device__ __forceinline__ uint32_t ld_stream1(const uint32_t* p) { return __ldcs(p); }
+
+// Dense strip contraction of one document (thread = document): acc[q] += x[h][doc] * Q[h][q] over the strips the
+// tile uses.  A separate (not inlined) function: compiled on its own, the strip loop's index stays in a uniform
+// register, so every weight is fetched by a uniform constant load (LDCU c[3][UR+imm]) and used as the uniform
+// operand of the FFMA/IMAD itself, and the body (4 x QT multiply-adds) stays small in the instruction cache.
+// The accumulators travel through the lane's own row of the shared-memory tile (conflict-free).
+__device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, float x, unsigned long long c) {
+    // (a.lo * x + c.lo, a.hi * x + c.hi): one FFMA2, each half an IEEE fp32 fma (same result as two fmaf)
+    unsigned long long d, xx;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(xx) : "f"(x));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(xx), "l"(c));
+    return d;
+}
+
+template <int WT, int QT>
+__device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ myacc,
+                                          const typename NumD<WT>::W* __restrict__ sp, int64_t N_pad) {
+    using A = typename NumD<WT>::A;
+    const int nh = (int)c_tile.nh;
+    if constexpr (WT == GS_W_F32) {
+        // packed pairs of queries: one FFMA2 (uniform-register weight pair x scalar strip value) per two cells
+        unsigned long long acc[QT / 2];
+#pragma unroll
+        for (int q = 0; q < QT / 2; ++q)
+            asm("mov.b64 %0, {%1, %2};" : "=l"(acc[q]) : "f"(myacc[2 * q]), "f"(myacc[2 * q + 1]));
+#pragma unroll 1
+        for (int i0 = 0; i0 < nh; i0 += 4) {
+            float x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) x[u] = sp[(size_t)c_tile.hl[i0 + u] * N_pad];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+#pragma unroll
+                for (int q = 0; q < QT; q += 4) {
+                    const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(&c_tile.qh[(i0 + u) * QT + q]);
+                    acc[q / 2] = fma_f32x2(v.x, x[u], acc[q / 2]);
+                    acc[q / 2 + 1] = fma_f32x2(v.y, x[u], acc[q / 2 + 1]);
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < QT / 2; ++q) {
+            float lo, hi;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(acc[q]));
+            myacc[2 * q] = lo;
+            myacc[2 * q + 1] = hi;
+        }
+    } else {
+        A acc[QT];
+#pragma unroll
+        for (int q = 0; q < QT; ++q) acc[q] = myacc[q];
+#pragma unroll 1
+        for (int i0 = 0; i0 < nh; i0 += 4) {
+            A x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) x[u] = NumD<WT>::widen(sp[(size_t)c_tile.hl[i0 + u] * N_pad]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+#pragma unroll
+                for (int q = 0; q < QT; ++q)
+                    acc[q] = NumD<WT>::mac(acc[q], NumD<WT>::from_bits(c_tile.qh[(i0 + u) * QT + q]), x[u]);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < QT; ++q) myacc[q] = acc[q];
+    }
+}
 
 template <int WT, int QT>
 __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocParams p) {
@@ -251,66 +354,49 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     constexpr int AST = G::AST, NW = G::NW, QCAP = G::QCAP;
     extern __shared__ __align__(16) unsigned char smem[];
     const int Wd = p.Wd;
-    const int pass = blockIdx.x / p.ctas_per_pass;
-    const int cta = blockIdx.x % p.ctas_per_pass;
-    const unsigned char* base = p.scratch + (size_t)pass * pass_bytes(Wd, QT);
-    const QTileHdr* hdr = reinterpret_cast<const QTileHdr*>(base);
-    const uint32_t R = hdr->R, np = hdr->np;
-    const int nh = (int)hdr->nh;
-    const uint32_t* g_rowptr = p.rowptr + hdr->row_off;
-    const uint2* g_pairs = p.pairs + hdr->pair_off;
-    const bool sparse_in_smem = (size_t)(R + 2) * 4 + (size_t)np * 8 <= (size_t)p.sparse_cap_bytes;
+    const uint32_t R = c_tile.R, np = c_tile.np;
+    const int nh = (int)c_tile.nh;
+    const uint2* g_rows = p.rows + c_tile.row_off;
+    const uint2* g_pairs = p.pairs + c_tile.pair_off;
+    const bool sparse_in_smem = (size_t)(R + np) * 8 <= (size_t)p.sparse_cap_bytes;
 
-    A* s_qh = reinterpret_cast<A*>(smem);                                         // [GS_STRIP_MAX][QT]
-    uint64_t* s_thr = reinterpret_cast<uint64_t*>(s_qh + GS_STRIP_MAX * QT);      // [QT]
-    A* s_thr_s = reinterpret_cast<A*>(s_thr + QT);                                // [QT]
-    uint32_t* s_hl = reinterpret_cast<uint32_t*>(s_thr_s + QT);                   // [GS_STRIP_MAX]
-    uint32_t* s_bm = s_hl + GS_STRIP_MAX;                                         // [Wd]
+    uint32_t* s_bm = reinterpret_cast<uint32_t*>(smem);                           // [Wd]
     uint32_t* s_pre = s_bm + Wd;                                                  // [Wd]
     unsigned char* pw = reinterpret_cast<unsigned char*>(s_pre + Wd);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint2* queue = reinterpret_cast<uint2*>(pw + (size_t)warp * G::per_warp);     // [QCAP]
     A* s_acc = reinterpret_cast<A*>(queue + QCAP);                                // [32][AST]
-    uint2* s_pairs = reinterpret_cast<uint2*>(pw + (size_t)NW * G::per_warp);     // [np]      when it fits
-    uint32_t* s_rowptr = reinterpret_cast<uint32_t*>(s_pairs + np);               // [R+1]
+    uint2* s_pairs = reinterpret_cast<uint2*>(pw + (size_t)NW * G::per_warp);     // [np]  when it fits
+    uint2* s_rows = s_pairs + np;                                                 // [R]
 
-    const int64_t qa = p.q0 + (int64_t)pass * QT;
-    const int nqt = (int)min((int64_t)QT, p.q0 + p.nq - qa);
     const bool filter = p.sink.thr != nullptr;
     {   // stage the query tile
-        const uint32_t* g_bm = reinterpret_cast<const uint32_t*>(base + off_bm());
-        for (int i = threadIdx.x; i < 2 * Wd; i += NW * 32) s_bm[i] = g_bm[i];       // bitmap and prefix are adjacent
-        const uint4* qs = reinterpret_cast<const uint4*>(base + off_qh(Wd));
-        uint4* qd = reinterpret_cast<uint4*>(s_qh);
-        const int nh4 = (nh + 3) & ~3;
-        for (int i = threadIdx.x; i < nh4 * QT / 4; i += NW * 32) qd[i] = qs[i];
-        for (int i = threadIdx.x; i < GS_STRIP_MAX; i += NW * 32) s_hl[i] = hdr->hl[i];
-        for (int i = threadIdx.x; i < QT; i += NW * 32) {
-            const uint64_t t = (filter && i < nqt) ? p.sink.thr[qa + i] : 0ull;
-            s_thr[i] = t;
-            s_thr_s[i] = NumD<WT>::thr_score((uint32_t)(t >> 32));
-        }
+        for (int i = threadIdx.x; i < 2 * Wd; i += NW * 32) s_bm[i] = p.tile_bm[i];   // bitmap and prefix are adjacent
         if (sparse_in_smem) {
             for (uint32_t i = threadIdx.x; i < np; i += NW * 32) s_pairs[i] = g_pairs[i];
-            for (uint32_t i = threadIdx.x; i <= R; i += NW * 32) s_rowptr[i] = g_rowptr[i];
+            for (uint32_t i = threadIdx.x; i < R; i += NW * 32) s_rows[i] = g_rows[i];
         }
     }
     __syncthreads();
-    const uint32_t* rowptr = sparse_in_smem ? s_rowptr : g_rowptr;      // generic pointers: either space
-    const uint2* pairs = sparse_in_smem ? s_pairs : g_pairs;
+    // the block loop exists twice, with the row table and the pairs in shared memory (the normal case) or, when a
+    // tile's tables do not fit, in global memory: one address space per instantiation, no generic loads
+    auto run = [&](auto sp_tag) {
+    constexpr bool SP = decltype(sp_tag)::value;
+    const uint2* rows = SP ? s_rows : g_rows;
+    const uint2* pairs = SP ? s_pairs : g_pairs;
 
-    const W* __restrict__ fw = reinterpret_cast<const W*>(p.fwd_w);
     const W* __restrict__ strips = reinterpret_cast<const W*>(p.strips);
     const unsigned lt = (1u << lane) - 1u;
     A* myacc = s_acc + lane * AST;
     const int subs_per_tile = p.Ts >> 5;
     const int64_t n_subs = (int64_t)p.ts.count * subs_per_tile;
+    const int64_t sb_stride = (int64_t)gridDim.x * NW;
 
-    // lane d applies the queued hits of document d (contiguous: the queue is in stream order)
+    // lane d applies the queued hits of document d (contiguous: the queue is in stream order); one loop over (hit, pair)
     auto walk = [&](int n) {
         __syncwarp();
         int lo = 0, hi = n;
-        for (int it = 32 - __clz(n); it > 0; --it) {          // lower bound of the first entry with doc >= lane
+        for (int it = 32 - __clz(n); it > 0; --it) {          // lower bound of the first entry with doc position >= lane
             const int mid = (lo + hi) >> 1;
             if (lo < hi) {
                 if ((int)(queue[mid].x >> GS_FWD_DOC_SHIFT) < lane) lo = mid + 1; else hi = mid;
@@ -318,101 +404,122 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         }
         int end = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
         if (lane == 31) end = n;
-        for (int j = lo; j < end; ++j) {
-            const uint2 e = queue[j];
-            const uint32_t t = e.x & kTermMask;
-            const A w = NumD<WT>::from_bits(e.y);
-            const uint32_t word = s_bm[t >> 5];
-            const uint32_t r = s_pre[t >> 5] + __popc(word & ((1u << (t & 31)) - 1u));
-            const uint32_t p0 = rowptr[r], p1 = rowptr[r + 1];
-            for (uint32_t i = p0; i < p1; ++i) {
-                const uint2 pr = pairs[i];
-                myacc[pr.x] = NumD<WT>::mac(myacc[pr.x], NumD<WT>::from_bits(pr.y), w);
+        int j = lo;
+        uint32_t i = 0, i_end = 0;
+        A w = A(0);
+        for (;;) {
+            if (i == i_end) {                                  // next hit of this document
+                if (j >= end) break;
+                const uint2 e = queue[j++];
+                const uint32_t t = e.x & kTermMask;
+                w = NumD<WT>::from_bits(e.y);
+                const uint32_t word = s_bm[t >> 5];
+                const uint2 r = rows[s_pre[t >> 5] + __popc(word & ((1u << (t & 31)) - 1u))];
+                i = r.x;
+                i_end = r.y;                                   // every row holds at least one pair
             }
+            const uint2 pr = pairs[i++];
+            myacc[pr.x] = NumD<WT>::mac(myacc[pr.x], NumD<WT>::from_bits(pr.y), w);
         }
         __syncwarp();
     };
 
-    for (int64_t sb = (int64_t)cta * NW + warp; sb < n_subs; sb += (int64_t)p.ctas_per_pass * NW) {
+    // block -> (start, chunks) of its posting range, or nothing beyond the collection
+    auto block_of = [&](int64_t sb, int64_t& doc0) -> int64_t {
         const int64_t tile = p.ts.first + (sb / subs_per_tile) * (int64_t)p.ts.stride;
-        const int64_t doc0 = tile * p.Ts + (sb % subs_per_tile) * 32;
-        if (doc0 >= p.N) continue;
+        doc0 = tile * p.Ts + (sb % subs_per_tile) * 32;
+        return doc0 < p.N ? (doc0 >> 5) : -1;
+    };
+    const uint32_t* __restrict__ wp1 = reinterpret_cast<const uint32_t*>(p.fwd_w);     // u8: 4 weights per word
+    const uint4* __restrict__ wp4 = reinterpret_cast<const uint4*>(p.fwd_w);           // f32
+    const uint4* __restrict__ tp4 = reinterpret_cast<const uint4*>(p.fwd_terms);
+    // chunk c (128 postings) of the index: lane holds postings 4*lane .. 4*lane+3
+    auto load_chunk = [&](int64_t chunk, uint4& t4, uint4& w4) {
+        t4 = ld_stream4(tp4 + chunk * 32 + lane);
+        if (WT == GS_W_F32) {
+            w4 = ld_stream4(wp4 + chunk * 32 + lane);
+        } else {
+            const uint32_t v = ld_stream1(wp1 + chunk * 32 + lane);
+            w4 = make_uint4(v & 0xFFu, (v >> 8) & 0xFFu, (v >> 16) & 0xFFu, v >> 24);
+        }
+    };
+
+    int64_t sb = (int64_t)blockIdx.x * NW + warp;
+    int64_t doc0 = 0, c0 = 0, c1 = 0;              // chunk range of the current block
+    uint4 tc = make_uint4(0, 0, 0, 0), wc = tc;
+    if (sb < n_subs) {
+        const int64_t blk = block_of(sb, doc0);
+        if (blk >= 0) {
+            c0 = p.fwd_blk[blk] / GS_FWD_CHUNK;
+            c1 = p.fwd_blk[blk + 1] / GS_FWD_CHUNK;
+            if (c0 < c1) load_chunk(c0, tc, wc);
+        } else {
+            c0 = c1 = -1;
+        }
+    }
+    for (; sb < n_subs; sb += sb_stride) {
+        // the next block's range, asked for now, needed after the walk
+        const int64_t sbn = sb + sb_stride;
+        int64_t doc0n = 0, blkn = -1, c0n = -1, c1n = -1;
+        if (sbn < n_subs) blkn = block_of(sbn, doc0n);
+        if (blkn >= 0) { c0n = p.fwd_blk[blkn] / GS_FWD_CHUNK; c1n = p.fwd_blk[blkn + 1] / GS_FWD_CHUNK; }
+        if (c0 < 0) {                              // block beyond the collection
+            doc0 = doc0n; c0 = c0n; c1 = c1n;
+            if (c0 >= 0 && c0 < c1) load_chunk(c0, tc, wc);
+            continue;
+        }
         for (int i = lane; i < 32 * AST; i += 32) s_acc[i] = A(0);
 
         // ---- tail: the block's postings as one flat range -> bitmap filter -> hit queue -> per-document walk
-        const int64_t A0 = p.fwd_indptr[doc0];
-        const int n = (int)(p.fwd_indptr[min(doc0 + 32, p.N)] - A0);
-        const int32_t* __restrict__ tp = p.fwd_terms + A0;
-        const W* __restrict__ wp = fw + A0;
         int cnt = 0;
-        uint32_t tw[4], ww[4];
-        auto load_chunk = [&](int cbase, uint32_t (&t4)[4], uint32_t (&w4)[4]) {
+        for (int64_t c = c0; c < c1; ++c) {
+            uint4 tn = make_uint4(0, 0, 0, 0), wn = tn;
+            if (c + 1 < c1) load_chunk(c + 1, tn, wn);                       // prefetch
+            if (cnt + GS_FWD_CHUNK > QCAP) { walk(cnt); cnt = 0; }
+            const uint32_t tw[4] = {tc.x, tc.y, tc.z, tc.w};
+            const uint32_t ww[4] = {wc.x, wc.y, wc.z, wc.w};
+            uint32_t h[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int idx = cbase + 32 * u + lane;
-                const bool valid = idx < n;
-                t4[u] = valid ? (uint32_t)tp[idx] : (uint32_t)p.V;            // bit V of the bitmap is never set
-                w4[u] = valid ? NumD<WT>::bits(NumD<WT>::widen(wp[idx])) : 0u;
-            }
-        };
-        load_chunk(0, tw, ww);
-        for (int cbase = 0; cbase < n; cbase += 128) {
-            uint32_t tn[4], wn[4];
-            load_chunk(cbase + 128, tn, wn);                                  // prefetch (all-invalid past the end)
+            for (int u = 0; u < 4; ++u) h[u] = (s_bm[(tw[u] >> 5) & (kTermMask >> 5)] >> (tw[u] & 31u)) & 1u;
+            const uint32_t nhit = h[0] + h[1] + h[2] + h[3];
+            const unsigned b0 = __ballot_sync(0xFFFFFFFFu, nhit & 1u), b1 = __ballot_sync(0xFFFFFFFFu, nhit & 2u),
+                           b2 = __ballot_sync(0xFFFFFFFFu, nhit & 4u);
+            if ((b0 | b1 | b2) != 0u) {
+                int pos = cnt + __popc(b0 & lt) + 2 * __popc(b1 & lt) + 4 * __popc(b2 & lt);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const uint32_t t = tw[u] & kTermMask;
-                const bool hit = (s_bm[t >> 5] >> (t & 31)) & 1u;
-                const unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
-                if (m != 0u) {
-                    if (cnt + 32 > QCAP) { walk(cnt); cnt = 0; }
-                    if (hit) queue[cnt + __popc(m & lt)] = make_uint2(tw[u], ww[u]);
-                    cnt += __popc(m);
+                for (int u = 0; u < 4; ++u) {
+                    if (h[u]) queue[pos] = make_uint2(tw[u], ww[u]);
+                    pos += (int)h[u];
                 }
+                cnt += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) { tw[u] = tn[u]; ww[u] = wn[u]; }
+            tc = tn; wc = wn;
         }
         walk(cnt);
+        // first chunk of the next block: in flight during the contraction
+        if (c0n >= 0 && c0n < c1n) load_chunk(c0n, tc, wc);
 
-        // ---- head strips: thread = document, QT accumulators in registers
+        // ---- head strips: thread = document, QT accumulators in registers, weights as uniform constant operands
+        const int64_t doc = doc0 + lane;
+        if (nh > 0) strips_phase<WT, QT>(myacc, strips + doc, p.N_pad);
         A acc[QT];
 #pragma unroll
         for (int q = 0; q < QT; ++q) acc[q] = myacc[q];
-        const int64_t doc = doc0 + lane;
-        const W* sp = strips + doc;
-        for (int i = 0; i < nh; i += 4) {
-            A x[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) x[u] = NumD<WT>::widen(sp[(size_t)s_hl[i + u] * p.N_pad]);
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const A* qrow = s_qh + (i + u) * QT;
-#pragma unroll
-                for (int q = 0; q < QT; q += 4) {
-                    const int4 v = *reinterpret_cast<const int4*>(qrow + q);
-                    acc[q + 0] = NumD<WT>::mac(acc[q + 0], NumD<WT>::from_bits((uint32_t)v.x), x[u]);
-                    acc[q + 1] = NumD<WT>::mac(acc[q + 1], NumD<WT>::from_bits((uint32_t)v.y), x[u]);
-                    acc[q + 2] = NumD<WT>::mac(acc[q + 2], NumD<WT>::from_bits((uint32_t)v.z), x[u]);
-                    acc[q + 3] = NumD<WT>::mac(acc[q + 3], NumD<WT>::from_bits((uint32_t)v.w), x[u]);
-                }
-            }
-        }
 
         // ---- sink: this thread owns the cells (qa + q, doc)
         if (doc < p.N) {
             if (!filter) {
-                uint32_t* out = p.sink.dense + (qa - p.q0) * p.sink.ld + sb * 32 + lane;
+                uint32_t* out = p.sink.dense + p.q_rel * p.sink.ld + sb * 32 + lane;
 #pragma unroll
                 for (int q = 0; q < QT; ++q)
-                    if (q < nqt) out[(int64_t)q * p.sink.ld] = NumD<WT>::bits(acc[q]);
+                    if (q < p.nqt) out[(int64_t)q * p.sink.ld] = NumD<WT>::bits(acc[q]);
             } else {
 #pragma unroll
                 for (int q = 0; q < QT; ++q) {
-                    if (q < nqt && !(acc[q] < s_thr_s[q])) {
+                    if (!(acc[q] < NumD<WT>::from_bits(c_tile.thr_s[q]))) {
                         const uint64_t key = gs_make_key(gs_ord_bits<WT>(NumD<WT>::bits(acc[q])), (uint32_t)doc);
-                        if (key >= s_thr[q]) {
-                            const int64_t b = qa + q;
+                        if (q < p.nqt && key >= c_tile.thr_key[q]) {
+                            const int64_t b = p.qa + q;
                             const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
                             if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                         }
@@ -421,41 +528,68 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
             }
         }
         __syncwarp();
+        doc0 = doc0n; c0 = c0n; c1 = c1n;
     }
+    };
+    if (sparse_in_smem) run(std::true_type{}); else run(std::false_type{});
 }
 
 int norm_qt(int qtile) {
     if (qtile <= 0) return 32;
     int q = 8;
-    while (q < qtile && q < 64) q <<= 1;
+    while (q < qtile && q < kMaxQT) q <<= 1;
     return q;
 }
 
+// The constant tile is one per device: searches that use it are serialised (host side by the mutex, device side by
+// making a search's stream wait for the previous search's last pass).
+std::mutex g_tile_mu;
+cudaEvent_t g_tile_free[64] = {};
+
 template <int WT, int QT>
-gs_status_t launch_doc(DocParams p, int64_t n_subs, int n_passes, int sms, int smem_max, cudaStream_t s) {
+gs_status_t launch_passes(DocParams p, const unsigned char* scratch, int Wd, int64_t n_subs, int n_passes, int64_t q0, int64_t nq,
+                          int sms, int smem_max, cudaStream_t s) {
     using G = Geo<QT>;
-    const size_t fixed = G::fixed(p.Wd) + (size_t)G::NW * G::per_warp;
+    const size_t fixed = G::fixed(Wd) + (size_t)G::NW * G::per_warp;
     if (fixed > (size_t)smem_max) return GS_ERR_OUT_OF_RANGE;     // vocabulary too large for the shared-memory bitmap
     const size_t smem = (size_t)smem_max;
     p.sparse_cap_bytes = (int32_t)(smem - fixed);
-    p.ctas_per_pass = (int)std::max<int64_t>(1, std::min<int64_t>(sms, (n_subs + G::NW - 1) / G::NW));
-    const unsigned grid = (unsigned)(p.ctas_per_pass * n_passes);
+    const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, (n_subs + G::NW - 1) / G::NW));
     GS_CUDA(cudaFuncSetAttribute(k_score_doc<WT, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    {
-        GsProfScope ps(GS_K_SCORE_DOC, s);
-        k_score_doc<WT, QT><<<grid, G::NW * 32, smem, s>>>(p);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lock(g_tile_mu);
+    cudaEvent_t& ev = g_tile_free[dev & 63];
+    if (!ev) GS_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    else GS_CUDA(cudaStreamWaitEvent(s, ev, 0));
+    for (int pass = 0; pass < n_passes; ++pass) {
+        const unsigned char* base = scratch + (size_t)pass * pass_bytes(Wd);
+        {
+            GsProfScope ps(GS_K_QTILE, s, 0);
+            GS_CUDA(cudaMemcpyToSymbolAsync(c_tile, base, tile_copy_bytes(QT), 0, cudaMemcpyDeviceToDevice, s));
+        }
+        p.tile_bm = reinterpret_cast<const uint32_t*>(base + off_bm());
+        p.qa = q0 + (int64_t)pass * QT;
+        p.q_rel = (int64_t)pass * QT;
+        p.nqt = (int32_t)std::min<int64_t>(QT, q0 + nq - p.qa);
+        {
+            GsProfScope ps(GS_K_SCORE_DOC, s);
+            k_score_doc<WT, QT><<<grid, G::NW * 32, smem, s>>>(p);
+        }
+        ++gs_tls_launches;
     }
-    ++gs_tls_launches;
+    GS_CUDA(cudaEventRecord(ev, s));
     GS_CUDA(cudaGetLastError());
     return GS_OK;
 }
 template <int WT>
-gs_status_t launch_doc_qt(int QT, const DocParams& p, int64_t n_subs, int n_passes, int sms, int smem_max, cudaStream_t s) {
+gs_status_t launch_doc_qt(int QT, const DocParams& p, const unsigned char* scratch, int Wd, int64_t n_subs, int n_passes,
+                          int64_t q0, int64_t nq, int sms, int smem_max, cudaStream_t s) {
     switch (QT) {
-        case 8: return launch_doc<WT, 8>(p, n_subs, n_passes, sms, smem_max, s);
-        case 16: return launch_doc<WT, 16>(p, n_subs, n_passes, sms, smem_max, s);
-        case 32: return launch_doc<WT, 32>(p, n_subs, n_passes, sms, smem_max, s);
-        default: return launch_doc<WT, 64>(p, n_subs, n_passes, sms, smem_max, s);
+        case 8: return launch_passes<WT, 8>(p, scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
+        case 16: return launch_passes<WT, 16>(p, scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
+        case 32: return launch_passes<WT, 32>(p, scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
+        default: return launch_passes<WT, 64>(p, scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
     }
 }
 
@@ -467,8 +601,8 @@ size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, 
     const int QT = norm_qt(qtile);
     const int64_t passes = std::max<int64_t>((nq + QT - 1) / QT, 1);
     const int Wd = bm_words(ix->V);
-    const size_t n1 = ((size_t)(q_nnz + passes + 1) * 4 + 255) / 256 * 256;
-    return pass_bytes(Wd, QT) * (size_t)passes + 2 * n1 + ((size_t)q_nnz * 8 + 255) / 256 * 256;
+    const size_t n1 = (size_t)(q_nnz + passes + 1);
+    return pass_bytes(Wd) * (size_t)passes + 2 * up256(n1 * 4) + up256(n1 * 8) + up256((size_t)q_nnz * 8);
 }
 
 gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_qbatch& qb, int64_t q0, int64_t nq,
@@ -492,24 +626,24 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
         if (ix->wtype == GS_W_F32) {
             GS_CUDA(cudaFuncSetAttribute(k_build_qtile<GS_W_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
             k_build_qtile<GS_W_F32><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                              QT, ix->V, Wd, (unsigned char*)scratch, passes_cap, q->nnz);
+                                                              QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz);
         } else {
             GS_CUDA(cudaFuncSetAttribute(k_build_qtile<GS_W_U8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
             k_build_qtile<GS_W_U8><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                             QT, ix->V, Wd, (unsigned char*)scratch, passes_cap, q->nnz);
+                                                             QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz);
         }
         ++gs_tls_launches;
         GS_CUDA(cudaGetLastError());
     }
-    const SharedScratch ss = shared_scratch((unsigned char*)scratch, Wd, QT, passes_cap, q->nnz);
+    const SharedScratch ss = shared_scratch((unsigned char*)scratch, Wd, passes_cap, q->nnz);
     DocParams p{};
-    p.fwd_indptr = ix->fwd_indptr; p.fwd_terms = ix->fwd_terms; p.fwd_w = ix->fwd_w;
+    p.fwd_blk = ix->fwd_blk; p.fwd_terms = ix->fwd_terms; p.fwd_w = ix->fwd_w;
     p.strips = ix->head_strip; p.N_pad = ix->N_pad;
     p.N = ix->N; p.V = ix->V; p.Ts = ix->Ts; p.Wd = Wd;
-    p.scratch = (const unsigned char*)scratch; p.rowptr = ss.rowptr; p.pairs = ss.pairs;
-    p.q0 = q0; p.nq = (int32_t)nq;
+    p.rows = ss.rows; p.pairs = ss.pairs;
     p.ts = ts; p.sink = sink;
     const int64_t n_subs = (int64_t)ts.count * (ix->Ts / 32);
-    return ix->wtype == GS_W_F32 ? launch_doc_qt<GS_W_F32>(QT, p, n_subs, n_passes, sms, smem_max, s)
-                                 : launch_doc_qt<GS_W_U8>(QT, p, n_subs, n_passes, sms, smem_max, s);
+    return ix->wtype == GS_W_F32
+               ? launch_doc_qt<GS_W_F32>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s)
+               : launch_doc_qt<GS_W_U8>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
 }

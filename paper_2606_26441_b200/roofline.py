@@ -64,9 +64,10 @@ def batch_term_stats(list_lengths: np.ndarray, query_terms: np.ndarray) -> dict:
 
 
 def forward_index_bytes(N: int, P_tail: int, wtype: str, strips: int = 0) -> int:
-    """One pass over the hybrid forward index: indptr + tail CSR + `strips` dense strips of N entries."""
+    """One pass over the hybrid forward index: one row pointer per block of 32 documents + the tail block CSR
+    (`P_tail` slots: postings plus the padding of every block to 128) + `strips` dense strips of N entries."""
     w = weight_bytes(wtype)
-    return 8 * (N + 1) + (4 + w) * P_tail + w * N * strips
+    return 8 * ((N + 31) // 32 + 1) + (4 + w) * P_tail + w * N * strips
 
 
 def strips_per_pass(query_indptr: np.ndarray, query_terms: np.ndarray, head_terms: np.ndarray, query_tile: int) -> list:

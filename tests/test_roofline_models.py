@@ -36,14 +36,16 @@ def test_our_models_closed_forms():
     st = rf.batch_term_stats(L, q_terms)
     assert st == {"U": 20, "W": 27, "distinct_terms": 3}
     assert rf.term_parallel_bytes(20, "f32") == 160 and rf.term_parallel_bytes(20, "u8") == 100
-    assert rf.forward_index_bytes(3, 7, "f32") == 8 * 4 + 8 * 7
-    assert rf.forward_index_bytes(3, 7, "u8") == 8 * 4 + 5 * 7
-    assert rf.doc_parallel_bytes(3, 7, "f32", B=500, query_tile=16) == 32 * (32 + 56)
-    assert rf.doc_parallel_bytes(3, 7, "f32", B=1, query_tile=16, sample_share=0.5) == 1.5 * 88
-    # hybrid forward index: 5 tail postings + strips read by the pass (4 B or 1 B per doc each)
-    assert rf.forward_index_bytes(3, 5, "f32", strips=2) == 32 + 40 + 24
-    assert rf.forward_index_bytes(3, 5, "u8", strips=2) == 32 + 25 + 6
+    # 70 documents = 3 blocks of 32 -> 4 row pointers; 128 slots (postings + block padding)
+    assert rf.forward_index_bytes(70, 128, "f32") == 8 * 4 + 8 * 128
+    assert rf.forward_index_bytes(70, 128, "u8") == 8 * 4 + 5 * 128
+    assert rf.forward_index_bytes(64, 0, "f32") == 8 * 3 and rf.forward_index_bytes(65, 0, "f32") == 8 * 4
+    assert rf.doc_parallel_bytes(70, 128, "f32", B=500, query_tile=16) == 32 * (32 + 1024)
+    assert rf.doc_parallel_bytes(70, 128, "f32", B=1, query_tile=16, sample_share=0.5) == 1.5 * 1056
+    # hybrid forward index: tail slots + strips read by the pass (4 B or 1 B per doc each)
+    assert rf.forward_index_bytes(3, 5, "f32", strips=2) == 16 + 40 + 24
+    assert rf.forward_index_bytes(3, 5, "u8", strips=2) == 16 + 25 + 6
     indptr = np.array([0, 2, 3, 6], np.int64)
     terms = np.array([5, 1, 9, 1, 2, 7], np.int32)
     assert rf.strips_per_pass(indptr, terms, np.array([1, 2, 3]), query_tile=2) == [1, 2]
-    assert rf.doc_parallel_bytes(3, 5, "f32", B=3, query_tile=2, strips_by_pass=[1, 2]) == (32 + 40 + 12) + (32 + 40 + 24)
+    assert rf.doc_parallel_bytes(3, 5, "f32", B=3, query_tile=2, strips_by_pass=[1, 2]) == (16 + 40 + 12) + (16 + 40 + 24)
