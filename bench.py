@@ -58,6 +58,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-queries", type=int, default=0, help="oracle sample size (0 = one per core)")
+    ap.add_argument("--latency-queries", type=int, default=200, help="single-query searches timed for the batch-1 latency leg (0 = skip)")
+    ap.add_argument("--suite", action="store_true", help="also measure BASELINE.json configs 1,2,4,5 (QPS, latency, roofline) into the line's `suite` key")
     return ap.parse_args()
 
 
@@ -203,6 +205,39 @@ def timed_steps(torch, dist, fn, steps, warmup, world):
     return ms
 
 
+def latency_leg(torch, ix, queries, k, n, algo, batch=1, **opt):
+    """Per-call latency of gs_search for `n` distinct batches of `batch` queries (device-resident CSR slices),
+    CUDA events around each call plus a stream synchronise per call (SURVEY §8d timing protocol)."""
+    dev = ix.device
+    n = max(1, min(n, queries.rows // batch))
+    slices = []
+    for i in range(n):
+        q = queries.slice_rows(i * batch, (i + 1) * batch)
+        slices.append(([torch.from_numpy(a).to(dev) for a in (q.indptr, q.terms, q.weights)], q.nnz))
+    max_nnz = max(z for _, z in slices)
+    ws = torch.empty(ix.workspace_bytes(batch, max_nnz, k, algo=algo, **opt), dtype=torch.uint8, device=dev)
+    sdt = torch.float32 if queries.weights.dtype == np.float32 else torch.int32
+    out_ids = torch.empty((batch, k), dtype=torch.int32, device=dev)
+    out_sc = torch.empty((batch, k), dtype=sdt, device=dev)
+    s = torch.cuda.current_stream()
+    for (q, _) in slices[:3]:
+        ix.search(*q, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, **opt)
+    torch.cuda.synchronize()
+    ms = []
+    for (q, _) in slices:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(s)
+        ix.search(*q, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, **opt)
+        e1.record(s)
+        e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    st = ix.stats(ws)
+    ms = np.array(ms)
+    return {"batch": batch, "calls": int(n), "algo": algo, "algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"),
+            "p50_ms": float(np.percentile(ms, 50)), "p99_ms": float(np.percentile(ms, 99)), "mean_ms": float(ms.mean()),
+            "p50_ms_per_query": float(np.percentile(ms, 50)) / batch}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -307,6 +342,11 @@ def run_ours(args):
                "h2d_bytes_per_step": int(sum(a.nbytes for a in pn)), "d2h_bytes_per_step": int(h_ids.numel() * 4 + h_sc.numel() * 4),
                "api": "gs_search_host (pinned host buffers; H2D + search + D2H + stream sync per step, host wall clock)"}
 
+    # ---- batch-1 latency (BASELINE.json metric: "batch-1 p50 ms/query"), both kernels, on the same index
+    latency = None
+    if world == 1 and args.latency_queries > 0:
+        latency = {a: latency_leg(torch, ix, queries, k, args.latency_queries, a) for a in ("term", "doc")}
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         full, _ = time_oracle(docs, queries, wl.VOCAB, k, args.cpu_sample_queries)
@@ -317,7 +357,7 @@ def run_ours(args):
                 "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32" if c["wtype"] == "f32" else "u8", "data": "synthetic",
                 "config": config_dict(args, c, n_docs, B, k, f"{args.algo}->{main['algo_used']}"),
-                "ms_per_query": main["ms_per_query"], "clocks": main["clocks"], "e2e": e2e,
+                "ms_per_query": main["ms_per_query"], "clocks": main["clocks"], "e2e": e2e, "latency_b1": latency,
                 "gpu_launches": int(main["launches_per_step"] * args.steps), "roofline": main["roofline"],
                 "cpu_baseline": cpu, "kernels": main["kernels"], "candidates_per_query": main["candidates_per_query"],
                 "overflow_queries": main["overflow_queries"], "other_algos": others,
@@ -328,10 +368,61 @@ def run_ours(args):
                           "build_s": t_build, "generate_s": t_gen},
                 "context": {"paper_h100_qps": 787, "paper_h100_doc_parallel_hbm_frac": 0.626,
                             "note": "paper numbers are H100 + MS MARCO/SPLADE (PAPER.md L292, L340): context, not a baseline"}}
-        print(json.dumps(line), flush=True)
     ix.close()
+    del ix, q_dev, out_ids, out_sc
+    if rank == 0:
+        if args.suite and world == 1:
+            line["suite"] = {name: suite_entry(torch, gs, wl, name, args, peaks)
+                             for name in ("tiny", "mid", "paper_u8", "skew_b1", "skew_b32")}
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def suite_entry(torch, gs, wl, name, args, peaks):
+    """One BASELINE.json config other than the headline one: QPS of both kernels (CUDA events, queries resident),
+    roofline of the scoring kernel, per-call latency.  Parity of these configs is the business of tests/."""
+    c = wl.CONFIGS[name]
+    dev = torch.device("cuda:0")
+    B, k = c["B"], c["k"]
+    docs = wl.make_docs(name)
+    n_lat = max(args.latency_queries, 1) if B <= 32 else 0
+    queries = wl.make_queries(name, n_queries=max(B, n_lat * B))
+    batch = queries.slice_rows(0, B)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs, head_max=args.head_max,
+                             head_density=args.head_density)
+    info, lens, head_terms = ix.info(), ix.meta()[1].astype(np.int64), ix.head_terms()
+    q_dev = [torch.from_numpy(a).to(dev) for a in (batch.indptr, batch.terms, batch.weights)]
+    sdt = torch.float32 if c["wtype"] == "f32" else torch.int32
+    out_ids = torch.empty((B, k), dtype=torch.int32, device=dev)
+    out_sc = torch.empty((B, k), dtype=sdt, device=dev)
+    res = {"workload": f"N={docs.rows} docs, Zipf s={c['s']}, {c['wtype']} weights, B={B}, k={k}", "algos": {}}
+    steps = max(args.steps, 3)
+    for algo in ("term", "doc"):
+        ws = torch.empty(ix.workspace_bytes(B, batch.nnz, k, algo=algo), dtype=torch.uint8, device=dev)
+
+        def step():
+            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo)
+
+        ms = timed_steps(torch, None, step, steps, max(args.warmup, 3), 1)
+        st = ix.stats(ws)
+        gs.profile_enable(True)
+        for _ in range(steps):
+            step()
+        torch.cuda.synchronize()
+        prof = gs.profile_read()
+        gs.profile_enable(False)
+        r = {"algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"), "ms_per_step": ms / steps, "qps": B * steps / (ms * 1e-3),
+             "ms_per_query": ms / steps / B, "overflow_queries": st["overflow_queries"],
+             "kernels": {n: {"launches_per_step": v["launches"] / steps, "ms_per_step": v["ms"] / steps} for n, v in prof.items()}}
+        r["roofline"] = roofline(r, st, info, lens, head_terms, batch, B, k, peaks, c["wtype"])
+        del r["kernels"]
+        if n_lat:
+            r["latency"] = latency_leg(torch, ix, queries, k, n_lat, algo, batch=B)
+        res["algos"][algo] = r
+        del ws
+    ix.close()
+    return res
 
 
 def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
