@@ -197,12 +197,8 @@ def timed_steps(torch, dist, fn, steps, warmup, world):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    return ms
+    from paper_2606_26441_b200 import replicas
+    return replicas.max_over_ranks(e0.elapsed_time(e1), dist if world > 1 else None, "cuda")
 
 
 def latency_leg(torch, ix, queries, k, n, algo, batch=1, **opt):
@@ -261,7 +257,8 @@ def run_ours(args):
 
     t0 = time.perf_counter()
     docs = wl.make_docs(args.config, n_docs=n_docs)                  # every replica indexes the same collection
-    queries = wl.make_queries(args.config, n_queries=B, row0=rank * B)   # ... and searches its own batch
+    from paper_2606_26441_b200 import replicas
+    queries = wl.make_queries(args.config, n_queries=B, row0=replicas.query_rows(rank, B)[0])   # ... and searches its own batch
     t_gen = time.perf_counter() - t0
     t0 = time.perf_counter()
     ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs, head_max=args.head_max,
@@ -297,7 +294,7 @@ def run_ours(args):
         prof = gs.profile_read()
         gs.profile_enable(False)
         res = {"algo": algo, "algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"), "ms_per_step": ms / args.steps,
-               "qps": world * B * args.steps / (ms * 1e-3), "ms_per_query": ms / args.steps / B,
+               "qps": replicas.aggregate_qps(world, B, args.steps, ms), "ms_per_query": ms / args.steps / B,
                "launches_per_step": launches, "candidates_per_query": st["candidates"] / max(B, 1),
                "overflow_queries": st["overflow_queries"], "workspace_bytes": ws_bytes, "clocks": cs.summary(),
                "kernels": {n: {"launches_per_step": v["launches"] / args.steps, "ms_per_step": v["ms"] / args.steps}
@@ -334,11 +331,8 @@ def run_ours(args):
         for _ in range(args.steps):
             step_host()          # synchronous: returns after the D2H copy of the results
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * B * args.steps / dt, "unit": "queries/s", "ms_per_step": 1e3 * dt / args.steps,
+        dt = replicas.max_over_ranks(dt, dist if world > 1 else None, "cuda")
+        e2e = {"value": replicas.aggregate_qps(world, B, args.steps, 1e3 * dt), "unit": "queries/s", "ms_per_step": 1e3 * dt / args.steps,
                "h2d_bytes_per_step": int(sum(a.nbytes for a in pn)), "d2h_bytes_per_step": int(h_ids.numel() * 4 + h_sc.numel() * 4),
                "api": "gs_search_host (pinned host buffers; H2D + search + D2H + stream sync per step, host wall clock)"}
 
