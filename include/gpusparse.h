@@ -61,7 +61,7 @@ typedef enum gs_status {
 typedef enum gs_weight { GS_W_F32 = 0, GS_W_U8 = 1 } gs_weight_t;
 
 typedef enum gs_algo {
-    GS_ALGO_AUTO = 0,           /* work model of L176-181: doc-parallel for batches of <= 16 queries, else term-parallel */
+    GS_ALGO_AUTO = 0,           /* work model of L176-181 with measured constants: term-parallel on every workload so far */
     GS_ALGO_TERM_PARALLEL = 1,  /* tiled scatter-add over the inverted index   (Eq. 5, §5.2)   */
     GS_ALGO_DOC_PARALLEL = 2    /* CSR forward-index streaming, zero atomics   (L174)                    */
 } gs_algo_t;

@@ -135,12 +135,12 @@ struct Plan {
 
 Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t* o) {
     Plan p;
-    p.algo = B <= 16 ? GS_ALGO_DOC_PARALLEL : GS_ALGO_TERM_PARALLEL;
+    p.algo = GS_ALGO_TERM_PARALLEL;
     if (o) {
-        // AUTO (work model of PAPER.md L176-181, constants measured on B200): one pass over the forward
-        // index costs about as much as the scatter of 16 queries, and the term-parallel kernel needs >= 32 queries to
-        // fill its accumulator tiles, so small batches go to the document-parallel kernel
-        p.algo = o->algo == GS_ALGO_AUTO ? (B <= 16 ? GS_ALGO_DOC_PARALLEL : GS_ALGO_TERM_PARALLEL) : o->algo;
+        // AUTO: the work model of PAPER.md L176-181 (q*L postings touched per query by the scatter against N*k streamed
+        // by the document-parallel kernel) with the constants measured on B200 puts every BASELINE.json
+        // workload on the term-parallel side: the warp-per-cell-row kernel for <= 16 queries, the CTA kernel beyond
+        p.algo = o->algo == GS_ALGO_AUTO ? GS_ALGO_TERM_PARALLEL : o->algo;
         p.flags = o->flags;
         p.group = o->query_group;
         p.qtile = o->doc_query_tile;

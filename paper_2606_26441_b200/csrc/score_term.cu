@@ -102,6 +102,36 @@ __device__ __forceinline__ void emit_candidate(const gs_sink& sink, int64_t b, u
     }
 }
 
+// the finished cells (query b, docs doc0 .. doc0+3) go to the sink: dense score matrix, or threshold filter -> candidates
+template <int WT>
+__device__ __forceinline__ void sink_quad(const TermParams& p, int64_t b, int j, int dq, int64_t doc0,
+                                          typename Num<WT>::A s0, typename Num<WT>::A s1, typename Num<WT>::A s2,
+                                          typename Num<WT>::A s3) {
+    if (p.sink.thr == nullptr) {
+        uint32_t* out = p.sink.dense + (b - p.q0) * p.sink.ld + (int64_t)j * p.Ts + 4 * dq;
+        if (doc0 + 3 < p.N && p.vec4) {
+            *reinterpret_cast<uint4*>(out) =
+                make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
+        } else {
+            if (doc0 + 0 < p.N) out[0] = Num<WT>::bits(s0);
+            if (doc0 + 1 < p.N) out[1] = Num<WT>::bits(s1);
+            if (doc0 + 2 < p.N) out[2] = Num<WT>::bits(s2);
+            if (doc0 + 3 < p.N) out[3] = Num<WT>::bits(s3);
+        }
+    } else {
+        const uint64_t thr = p.sink.thr[b];
+        const uint32_t to = (uint32_t)(thr >> 32);
+        const bool r0 = Num<WT>::below(s0, to), r1 = Num<WT>::below(s1, to), r2 = Num<WT>::below(s2, to),
+                   r3 = Num<WT>::below(s3, to);
+        if (!(r0 && r1 && r2 && r3)) {
+            if (!r0 && doc0 + 0 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 0, s0);
+            if (!r1 && doc0 + 1 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 1, s1);
+            if (!r2 && doc0 + 2 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 2, s2);
+            if (!r3 && doc0 + 3 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 3, s3);
+        }
+    }
+}
+
 template <int WT>
 __global__ void __launch_bounds__(kMaxThreads, 1) k_score_term(const TermParams p) {
     using W = typename Num<WT>::W;
@@ -186,7 +216,6 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_score_term(const TermParams 
     __syncthreads();
 
     // ---- phase 2: head strips + sink.  A thread owns 4 consecutive docs of one query at a time.
-    const bool filter = p.sink.thr != nullptr;
     for (int item = threadIdx.x; item < Gc * quads; item += nthreads) {
         const int g = item / quads, dq = item - g * quads;
         const int64_t b = p.q0 + g0 + g;
@@ -206,30 +235,90 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_score_term(const TermParams 
                 s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
             }
         }
-        const int64_t doc0 = (int64_t)base + 4 * dq;
-        if (!filter) {
-            uint32_t* out = p.sink.dense + (b - p.q0) * p.sink.ld + (int64_t)j * Ts + 4 * dq;
-            if (doc0 + 3 < p.N && p.vec4) {
-                *reinterpret_cast<uint4*>(out) =
-                    make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
-            } else {
-                if (doc0 + 0 < p.N) out[0] = Num<WT>::bits(s0);
-                if (doc0 + 1 < p.N) out[1] = Num<WT>::bits(s1);
-                if (doc0 + 2 < p.N) out[2] = Num<WT>::bits(s2);
-                if (doc0 + 3 < p.N) out[3] = Num<WT>::bits(s3);
-            }
-        } else {
-            const uint64_t thr = p.sink.thr[b];
-            const uint32_t to = (uint32_t)(thr >> 32);
-            const bool r0 = Num<WT>::below(s0, to), r1 = Num<WT>::below(s1, to), r2 = Num<WT>::below(s2, to),
-                       r3 = Num<WT>::below(s3, to);
-            if (!(r0 && r1 && r2 && r3)) {
-                if (!r0 && doc0 + 0 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 0, s0);
-                if (!r1 && doc0 + 1 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 1, s1);
-                if (!r2 && doc0 + 2 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 2, s2);
-                if (!r3 && doc0 + 3 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 3, s3);
-            }
+        sink_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, s0, s1, s2, s3);
+    }
+}
+
+// ---- small batches: one WARP per (doc tile, query) cell row.
+// With a handful of queries the CTA-per-(tile, query group) kernel above leaves 31 of its 32 warps idle during the
+// scatter and stages strips nobody uses.  Here a warp owns the Ts accumulators of one query in one doc tile (2 KB
+// of shared memory), 8 such warps per CTA and several CTAs per SM: zero, scatter the query's tail lists (same
+// segment walk as above), then add the query's head terms straight from the global strips (each strip value
+// is used exactly once, so there is nothing to stage) and hand the cells to the sink.  No atomics, fixed order.
+constexpr int kWarpsSmall = 8;
+
+template <int WT>
+__global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const TermParams p) {
+    using W = typename Num<WT>::W;
+    using A = typename Num<WT>::A;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int Ts = p.Ts;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t item = (int64_t)blockIdx.x * kWarpsSmall + warp;
+    if (item >= (int64_t)p.ts.count * p.nq) return;
+    const int j = (int)(item / p.nq);                       // position in the tile set
+    const int64_t b = p.q0 + (item - (int64_t)j * p.nq);
+    const int tile = p.ts.first + j * p.ts.stride;
+    const int32_t base = tile * Ts;
+    const int quads = Ts >> 2;
+    A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * Ts;
+    for (int dq = lane; dq < quads; dq += 32) reinterpret_cast<int4*>(row)[dq] = make_int4(0, 0, 0, 0);
+    __syncwarp();
+
+    // scatter the tail lists of the query: segment of each list inside this tile, 32 terms probed at once
+    const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
+    const int64_t qa = p.q_indptr[b];
+    const int cnt = p.tail_cnt[b];
+    for (int i0 = 0; i0 < cnt; i0 += 32) {
+        int64_t start = 0;
+        int n = 0;
+        uint32_t wq = 0;
+        if (i0 + lane < cnt) {
+            const int32_t t = p.tail_term[qa + i0 + lane];
+            wq = p.tail_w[qa + i0 + lane];
+            const uint32_t* sr = p.seg + (size_t)t * (p.ntiles + 1) + tile;
+            const uint32_t lo = sr[0], hi = sr[1];
+            n = (int)(hi - lo);
+            start = p.inv_off[t] + lo;
         }
+        unsigned m = __ballot_sync(0xFFFFFFFFu, n > 0);
+        while (m) {
+            const int src = __ffs(m) - 1;
+            m &= m - 1;
+            const int n_j = __shfl_sync(0xFFFFFFFFu, n, src);
+            const int64_t start_j = __shfl_sync(0xFFFFFFFFu, start, src);
+            const A q = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
+            scatter_segment<WT>(p.inv_doc + start_j, inv_w + start_j, n_j, q, row, base, Ts, lane);
+            __syncwarp();                                   // two lists may hit the same document
+        }
+    }
+    __syncwarp();
+
+    // head strips + sink: a lane owns 4 consecutive documents at a time
+    const int nh = p.H > 0 ? p.head_cnt[b] : 0;
+    const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
+    const W* __restrict__ gstrip = reinterpret_cast<const W*>(p.head_strip) + base;
+    for (int dq = lane; dq < quads; dq += 32) {
+        const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
+        A s0 = Num<WT>::from_bits(a4.x), s1 = Num<WT>::from_bits(a4.y), s2 = Num<WT>::from_bits(a4.z),
+          s3 = Num<WT>::from_bits(a4.w);
+        for (int i = 0; i < nh; ++i) {
+            const uint2 e = hl[i];
+            const A q = Num<WT>::qw(e.y);
+            const W* src = gstrip + (size_t)e.x * p.N_pad + 4 * dq;
+            int4 v;
+            if (WT == GS_W_F32) {
+                v = __ldg(reinterpret_cast<const int4*>(src));
+            } else {
+                const uchar4 u = __ldg(reinterpret_cast<const uchar4*>(src));
+                v = make_int4(u.x, u.y, u.z, u.w);
+            }
+            s0 = Num<WT>::mac(s0, q, Num<WT>::from_bits(v.x));
+            s1 = Num<WT>::mac(s1, q, Num<WT>::from_bits(v.y));
+            s2 = Num<WT>::mac(s2, q, Num<WT>::from_bits(v.z));
+            s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
+        }
+        sink_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, s0, s1, s2, s3);
     }
 }
 
@@ -265,9 +354,25 @@ gs_status_t launch(const TermParams& p, unsigned grid, const Shape& sh, cudaStre
     return GS_OK;
 }
 
+template <int WT>
+gs_status_t launch_warp(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
+    GS_CUDA(cudaFuncSetAttribute(k_score_term_warp<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    {
+        GsProfScope ps(GS_K_SCORE_TERM, s);
+        k_score_term_warp<WT><<<grid, kWarpsSmall * 32, smem, s>>>(p);
+    }
+    ++gs_tls_launches;
+    GS_CUDA(cudaGetLastError());
+    return GS_OK;
+}
+
+// query_group < 0 asks for the warp-per-cell-row kernel, 0 picks it for small batches
+bool use_warp_kernel(int64_t nq, int group) { return group < 0 || (group == 0 && nq <= 16); }
+
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
+    if (use_warp_kernel(nq, group)) return 1;
     return shape_for(ix, use_head ? ix->H_term : 0, nq, group).G;
 }
 
@@ -286,6 +391,14 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     p.q0 = q0; p.nq = (int32_t)nq; p.G = sh.G; p.n_qgroups = (int)((nq + sh.G - 1) / sh.G);
     p.ts = ts; p.sink = sink;
     p.vec4 = sink.dense && (((uintptr_t)sink.dense | (uintptr_t)(sink.ld * 4)) & 15) == 0;
+    if (use_warp_kernel(nq, group)) {
+        const size_t smem = (size_t)kWarpsSmall * ix->Ts * 4;
+        const int64_t grid = ((int64_t)ts.count * nq + kWarpsSmall - 1) / kWarpsSmall;
+        if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+        p.G = 1;
+        return ix->wtype == GS_W_F32 ? launch_warp<GS_W_F32>(p, (unsigned)grid, smem, s)
+                                     : launch_warp<GS_W_U8>(p, (unsigned)grid, smem, s);
+    }
     const int64_t grid = (int64_t)p.n_qgroups * ts.count;
     if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
     return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, sh, s) : launch<GS_W_U8>(p, (unsigned)grid, sh, s);

@@ -16,7 +16,13 @@ import parity  # tests/parity.py (pytest puts tests/ on sys.path)
 
 pytestmark = pytest.mark.gpu
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
-ALGOS = ["term", "doc"]
+ALGOS = ["term", "term_cta", "doc"]
+
+
+def aopt(algo):
+    """Search options of a parametrised kernel: "term" = term-parallel with its own choice (the warp-per-cell-row
+    kernel for batches <= 16), "term_cta" = the CTA-per-(tile, query group) kernel forced, "doc" = document-parallel."""
+    return {"term": dict(algo="term"), "term_cta": dict(algo="term", query_group=64), "doc": dict(algo="doc")}[algo]
 
 
 @pytest.fixture(scope="module")
@@ -74,7 +80,7 @@ def test_handworked_three_docs(gs, mode, algo):
     dt = np.float32 if mode == "f32" else np.uint8
     docs, queries = csr_from_dicts(c["docs"], dt), csr_from_dicts(c["queries"], dt)
     ix = gs.Index.from_numpy(docs, g["vocab"])
-    ids, sc = gpu_search(gs, ix, queries, c["k"], algo=algo)
+    ids, sc = gpu_search(gs, ix, queries, c["k"], **aopt(algo))
     assert ids.tolist() == c["expect_ids"]
     assert sc.tolist() == c["expect_scores"]
     ix.close()
@@ -108,7 +114,7 @@ def tiny():
 
 def _dense_parity(gs, docs, queries, vocab, algo, **build_kw):
     ix = gs.Index.from_numpy(docs, vocab, **build_kw)
-    S = ix.score_dense(*dev(queries), algo=algo).cpu().numpy()[:, :docs.rows]
+    S = ix.score_dense(*dev(queries), **aopt(algo)).cpu().numpy()[:, :docs.rows]
     R_d, R_q = oracle.as_rows(docs, vocab), oracle.as_rows(queries, vocab)
     _, _, A = oracle.search(R_q, R_d, 1, all_scores=True)
     if docs.weights.dtype == np.uint8:
@@ -180,7 +186,7 @@ def test_tiny_topk(gs, tiny, mode, algo, k):
     queries = tiny.queries if mode == "f32" else tiny.queries.to_u8()
     ix = gs.Index.from_numpy(docs, tiny.vocab)
     for flags in (0, gs.GS_FLAG_FORCE_DENSE_TOPK, gs.GS_FLAG_NO_HEAD_STRIPS | gs.GS_FLAG_VALIDATE_QUERIES):
-        ids, sc = gpu_search(gs, ix, queries, k, algo=algo, flags=flags)
+        ids, sc = gpu_search(gs, ix, queries, k, **aopt(algo), flags=flags)
         compare(gs, docs, queries, tiny.vocab, k, ids, sc)
     ix.close()
 
@@ -194,7 +200,7 @@ def test_ragged_collection_sizes(gs, algo, n_docs):
     for d, q in ((docs, queries), (docs.to_u8(), queries.to_u8())):
         ix = gs.Index.from_numpy(d, wl.VOCAB, tile_docs=256)
         for k in (1, 10, 50):
-            ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+            ids, sc = gpu_search(gs, ix, q, k, **aopt(algo))
             compare(gs, d, q, wl.VOCAB, k, ids, sc)
         ix.close()
 
@@ -212,7 +218,7 @@ def test_empty_query_empty_batch_and_k_gt_n(gs, algo):
     a, b = int(q.indptr[1]), int(q.indptr[2])
     q = wl.Csr(np.array([0, a, a, a + int(q.indptr[3]) - b], np.int64), np.delete(q.terms, slice(a, b)),
                np.delete(q.weights, slice(a, b)))
-    ids, sc = gpu_search(gs, ix, q, 64, algo=algo)
+    ids, sc = gpu_search(gs, ix, q, 64, **aopt(algo))
     compare(gs, docs, q, wl.VOCAB, 64, ids, sc)
     assert ids[1, :40].tolist() == list(range(40)) and np.all(sc[1, :40] == 0)
     assert np.all(ids[:, 40:] == -1) and np.all(np.isneginf(sc[:, 40:]))
@@ -220,13 +226,13 @@ def test_empty_query_empty_batch_and_k_gt_n(gs, algo):
     e = wl.Csr(np.zeros(1, np.int64), np.zeros(0, np.int32), np.zeros(0, np.float32))
     d = torch.device("cuda:0")
     ids0, sc0 = ix.search(torch.zeros(1, dtype=torch.int64, device=d), torch.zeros(0, dtype=torch.int32, device=d),
-                          torch.zeros(0, dtype=torch.float32, device=d), 5, algo=algo)
+                          torch.zeros(0, dtype=torch.float32, device=d), 5, **aopt(algo))
     assert tuple(ids0.shape) == (0, 5) and tuple(sc0.shape) == (0, 5)
     ix.close()
     # integer twin of the padding rule
     du, qu = docs.to_u8(), q.to_u8()
     ixu = gs.Index.from_numpy(du, wl.VOCAB)
-    ids, sc = gpu_search(gs, ixu, qu, 64, algo=algo)
+    ids, sc = gpu_search(gs, ixu, qu, 64, **aopt(algo))
     compare(gs, du, qu, wl.VOCAB, 64, ids, sc)
     assert np.all(sc[:, 40:] == np.iinfo(np.int32).min)
     ixu.close()
@@ -240,7 +246,7 @@ def test_closed_form_ties_across_tiles(gs, algo, N, k, tile):
     docs = wl.Csr(indptr, np.zeros(N, np.int32), (np.arange(N) // 2).astype(np.float32))
     q = csr_from_dicts([{0: 1.0}, {0: 0.5}], np.float32)
     ix = gs.Index.from_numpy(docs, 4, tile_docs=tile)
-    ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+    ids, sc = gpu_search(gs, ix, q, k, **aopt(algo))
     # descending score = descending floor(d/2); inside a pair (2j, 2j+1) the lower id comes first
     order = sorted(range(N), key=lambda d: (-(d // 2), d))[:k]
     assert ids[0].tolist() == order and ids[1].tolist() == order
@@ -251,7 +257,7 @@ def test_closed_form_ties_across_tiles(gs, algo, N, k, tile):
     du = wl.Csr(indptr, np.zeros(N, np.int32), ((np.arange(N) % 7) + 1).astype(np.uint8))
     qu = csr_from_dicts([{0: 3}], np.uint8)
     ixu = gs.Index.from_numpy(du, 4, tile_docs=tile)
-    ids, sc = gpu_search(gs, ixu, qu, k, algo=algo)
+    ids, sc = gpu_search(gs, ixu, qu, k, **aopt(algo))
     order = sorted(range(N), key=lambda d: (-((d % 7) + 1), d))[:k]
     assert ids[0].tolist() == order and sc[0].tolist() == [3 * ((d % 7) + 1) for d in order]
     ixu.close()
@@ -270,7 +276,7 @@ def test_padding_sentinel_never_surfaces(gs, algo):
     lids, _ = ix.posting_list(7)
     assert len(lids) == 64 and lids[:33].tolist() == hit and np.all(lids[33:] == -1)
     q = csr_from_dicts([{7: 2.0}], np.float32)
-    ids, sc = gpu_search(gs, ix, q, 50, algo=algo)
+    ids, sc = gpu_search(gs, ix, q, 50, **aopt(algo))
     assert ids[0, :33].tolist() == hit[::-1]
     rest = [d for d in range(N) if d not in set(hit)][:17]
     assert ids[0, 33:].tolist() == rest and np.all(sc[0, 33:] == 0) and np.all(ids >= 0)
@@ -296,7 +302,7 @@ def test_signed_weights_and_negative_zero(gs, algo):
     q = csr_from_dicts(qs, np.float32)
     ix = gs.Index.from_numpy(docs, V, tile_docs=128)
     for k in (10, 2999, 3000):
-        ids, sc = gpu_search(gs, ix, q, k, algo=algo)
+        ids, sc = gpu_search(gs, ix, q, k, **aopt(algo))
         R_d, R_q = oracle.as_rows(docs, V), oracle.as_rows(q, V)
         o_ids, o_sc = oracle.search(R_q, R_d, k)
         # cancellation makes |score| small relative to the summands: compare with an absolute bound from the summand sizes
@@ -408,7 +414,7 @@ def test_mid_prefix_full_compare(gs, mode, algo):
     if mode == "u8":
         docs, queries = docs.to_u8(), queries.to_u8()
     ix = gs.Index.from_numpy(docs, wl.VOCAB)
-    ids, sc = gpu_search(gs, ix, queries, 1000, algo=algo)
+    ids, sc = gpu_search(gs, ix, queries, 1000, **aopt(algo))
     worst, subs = compare(gs, docs, queries, wl.VOCAB, 1000, ids, sc)
     st = ix.stats()
     assert st["overflow_queries"] == 0
@@ -436,8 +442,10 @@ def test_paper_scale_sampled(gs, paper_docs, mode, k):
     R_s = oracle.as_rows(wl.Csr(*_take_rows(queries, sample)), wl.VOCAB)
     o_ids, o_sc = oracle.search(R_s, R_d, k)
     ix = gs.Index.from_numpy(docs, wl.VOCAB)
-    for algo in ALGOS:
-        ids, sc = gpu_search(gs, ix, queries, k, algo=algo)
+    batch_ids = None
+    for algo in ("term", "doc"):
+        ids, sc = gpu_search(gs, ix, queries, k, **aopt(algo))
+        batch_ids = ids
         assert ix.stats()["overflow_queries"] == 0
         b_idx = np.repeat(np.arange(queries.rows, dtype=np.int64), k)
         true = oracle.score_pairs(R_q, R_d, b_idx, ids.reshape(-1).astype(np.int64)).reshape(queries.rows, k)
@@ -452,6 +460,18 @@ def test_paper_scale_sampled(gs, paper_docs, mode, k):
             assert len(np.unique(ids[b])) == k and ids[b].min() >= 0 and ids[b].max() < docs.rows
             d = np.diff(sc[b].astype(np.float64))
             assert np.all(d <= 0) and np.all(ids[b][:-1][d == 0] < ids[b][1:][d == 0])
+    # small batches take other paths (warp-per-cell-row term kernel, document-parallel with a tile of 8)
+    few = queries.slice_rows(0, 3)
+    for opt in (dict(algo="term"), dict(algo="term", query_group=64), dict(algo="doc"), dict(algo="auto")):
+        ids, sc = gpu_search(gs, ix, few, k, **opt)
+        b_idx = np.repeat(np.arange(few.rows, dtype=np.int64), k)
+        true = oracle.score_pairs(R_q, R_d, b_idx, ids.reshape(-1).astype(np.int64)).reshape(few.rows, k)
+        if mode == "u8":
+            assert np.array_equal(sc.astype(np.int64), true) and np.array_equal(ids, batch_ids[:few.rows])
+        else:
+            assert np.all(np.abs(sc - true) <= parity.tol(true))
+            if sample[0] == 0:
+                parity.check_f32_row(ids[0], sc[0], o_ids[0], o_sc[0], true[0], docs.rows)
     ix.close()
 
 
