@@ -11,6 +11,7 @@
 //   4. a query whose candidate list overflowed is re-run through the dense path (exact, slower).
 // GS_FLAG_FORCE_DENSE_TOPK (or a collection of only a few tiles) uses the dense path for everything.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -147,7 +148,16 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
     }
     if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : 16;   // doc-parallel: queries per pass; 16 is the largest tile that stays HBM bound
     p.use_head = !(p.flags & GS_FLAG_NO_HEAD_STRIPS);
-    int shift = (o && o->sample_shift > 0) ? o->sample_shift : 5;
+    // Threshold sample = 1/2^shift of the doc tiles.  The select phases read the sample (N/2^shift cells per query) and
+    // the candidates (about k*2^shift per query): for a few queries, where they are what a search spends its time on,
+    // balance the two (2^shift ~ sqrt(N/k)); large batches keep 1/32 (candidate lists of 8*k*32 keys per query).
+    int shift = 5;
+    if (o && o->sample_shift > 0) {
+        shift = o->sample_shift;
+    } else if (B <= 16 && ix->N > 0) {
+        const double r = std::sqrt((double)ix->N / (double)k);
+        while (shift < 10 && (double)(1 << (shift + 1)) <= r * 1.4142) ++shift;
+    }
     // the sample must hold comfortably more than k documents, else its k-th key is a weak bound
     while (shift > 0 && ((int64_t)(ix->ntiles >> shift)) * ix->Ts < 4 * (int64_t)k) --shift;
     p.dense_only = (p.flags & GS_FLAG_FORCE_DENSE_TOPK) || shift == 0 || ix->ntiles < 4;

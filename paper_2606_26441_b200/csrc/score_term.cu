@@ -294,10 +294,18 @@ __global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const Term
     }
     __syncwarp();
 
-    // head strips + sink: a lane owns 4 consecutive documents at a time
+    // head strips + sink: a lane owns 4 consecutive documents at a time.  Filter mode makes two passes over the row so
+    // that a warp reserves its slice of the query's candidate list with ONE atomic: pass 1 finishes the scores in place
+    // and counts the cells that pass the threshold, pass 2 writes their keys.
     const int nh = p.H > 0 ? p.head_cnt[b] : 0;
     const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
     const W* __restrict__ gstrip = reinterpret_cast<const W*>(p.head_strip) + base;
+    const bool filter = p.sink.thr != nullptr;
+    const uint64_t thr = filter ? p.sink.thr[b] : 0ull;
+    auto passes = [&](A sc, int64_t doc) -> bool {
+        return doc < p.N && gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc)), (uint32_t)doc) >= thr;
+    };
+    uint32_t n_pass = 0;
     for (int dq = lane; dq < quads; dq += 32) {
         const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
         A s0 = Num<WT>::from_bits(a4.x), s1 = Num<WT>::from_bits(a4.y), s2 = Num<WT>::from_bits(a4.z),
@@ -318,7 +326,39 @@ __global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const Term
             s2 = Num<WT>::mac(s2, q, Num<WT>::from_bits(v.z));
             s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
         }
-        sink_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, s0, s1, s2, s3);
+        const int64_t doc0 = (int64_t)base + 4 * dq;
+        if (!filter) {
+            sink_quad<WT>(p, b, j, dq, doc0, s0, s1, s2, s3);
+        } else {
+            reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
+            n_pass += (uint32_t)passes(s0, doc0) + (uint32_t)passes(s1, doc0 + 1) + (uint32_t)passes(s2, doc0 + 2) +
+                      (uint32_t)passes(s3, doc0 + 3);
+        }
+    }
+    if (!filter) return;
+    uint32_t incl = n_pass;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    if (total == 0u) return;
+    uint32_t pos = 0;
+    if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b], total);
+    pos = __shfl_sync(0xFFFFFFFFu, pos, 0) + incl - n_pass;
+    uint64_t* cand = p.sink.cand + b * p.sink.cand_cap;
+    for (int dq = lane; dq < quads; dq += 32) {
+        const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
+        const A sc[4] = {Num<WT>::from_bits(a4.x), Num<WT>::from_bits(a4.y), Num<WT>::from_bits(a4.z), Num<WT>::from_bits(a4.w)};
+        const int64_t doc0 = (int64_t)base + 4 * dq;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (passes(sc[u], doc0 + u)) {
+                if ((int64_t)pos < p.sink.cand_cap)
+                    cand[pos] = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc[u])), (uint32_t)(doc0 + u));
+                ++pos;
+            }
+        }
     }
 }
 

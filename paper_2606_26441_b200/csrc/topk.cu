@@ -7,6 +7,8 @@
 // one pass collects the k keys >= it, and a bitonic network (warp shuffles for the short strides,
 // shared memory for the long ones) sorts them.  The select runs either over dense score rows
 // (fallback / threshold sample) or over the candidate key lists the scoring kernels emit.
+#include <cooperative_groups.h>
+
 #include <algorithm>
 
 #include "gs_internal.cuh"
@@ -34,7 +36,10 @@ template <int WT>
 __device__ __forceinline__ uint64_t src_key(const gs_sel_src& s, int64_t b, int64_t i) {
     if (s.keys) return s.keys[b * s.cap + i];
     int64_t doc = i;
-    if (s.Ts > 0) doc = ((int64_t)s.ts.first + (i / s.Ts) * s.ts.stride) * s.Ts + (i % s.Ts);
+    if (s.Ts > 0) {                                   // column -> doc id of a strided tile set (columns < 2^31)
+        const uint32_t jt = (uint32_t)i / (uint32_t)s.Ts;
+        doc = ((int64_t)s.ts.first + (int64_t)jt * s.ts.stride) * s.Ts + ((uint32_t)i - jt * (uint32_t)s.Ts);
+    }
     if (doc >= s.n_docs) return 0ull;
     return gs_make_key(gs_ord_bits<WT>(s.dense[b * s.ld + i]), (uint32_t)doc);
 }
@@ -212,6 +217,174 @@ __global__ void k_sel_sort(const SelState* __restrict__ st, const uint64_t* __re
     }
 }
 
+// ---- one thread-block CLUSTER per row: the whole select (histogram passes, pick, collect, bitonic sort, decode) in
+// ONE launch.  Used when a row has at most kRowFusedMax items (candidate lists, threshold samples).  The CTAs of a
+// cluster split the row; each keeps a histogram in its own shared memory, every CTA sums the cluster's histograms
+// through distributed shared memory and takes the same decision, the selected keys are gathered in CTA 0's shared
+// memory (remote atomics, aggregated per warp), which sorts and decodes them.  The row is re-read from L2 once per
+// digit.  15 launches become 1 — what a batch-1 search spends its time on once scoring takes 0.15 ms — and a
+// large batch keeps all SMs busy with one cluster per query.
+constexpr int kRowThreads = 1024;
+constexpr int64_t kRowFusedMax = 1 << 20;
+constexpr int kRowUnroll = 4;
+
+template <int WT>
+__global__ void __launch_bounds__(kRowThreads) k_sel_row(gs_sel_src src, int32_t k, int kp2, int32_t* __restrict__ out_ids,
+                                                         uint32_t* __restrict__ out_scores, uint64_t* __restrict__ out_thr) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    uint64_t* sk = reinterpret_cast<uint64_t*>(sm_raw);                        // [kp2]   (used in CTA 0)
+    uint32_t* hist = reinterpret_cast<uint32_t*>(sk + kp2);                    // [GS_SEL_BINS]
+    __shared__ uint32_t part[kRowThreads / 32];
+    __shared__ unsigned long long s_prefix;
+    __shared__ uint32_t s_krem, s_cnt;
+    __shared__ int s_shift, s_done;
+    const int64_t b = blockIdx.x / C;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t n = src_count(src, b);
+    const int64_t per = ((n + C - 1) / C + 3) / 4 * 4;                         // this CTA's slice of the row
+    const int64_t i_lo = min(n, per * rank), i_hi = min(n, i_lo + per);
+    if (tid == 0) {
+        int64_t live = n;
+        if (!src.keys) {
+            live = 0;
+            if (src.Ts > 0) {
+                for (int64_t j = 0; j < src.ts.count; ++j) {
+                    const int64_t d0 = ((int64_t)src.ts.first + j * src.ts.stride) * src.Ts;
+                    live += max((int64_t)0, min((int64_t)src.Ts, src.n_docs - d0));
+                }
+            } else live = min(n, src.n_docs);
+        }
+        s_prefix = 0ull;
+        s_krem = (uint32_t)min((int64_t)k, live);
+        s_shift = 64;
+        s_done = live <= k ? 1 : 0;            // everything is selected: threshold key 0 (no live key is 0)
+        s_cnt = 0;
+    }
+    __syncthreads();
+    while (!s_done) {                          // every CTA of the cluster takes the same decisions
+        const int shift = s_shift;
+        const unsigned long long prefix = s_prefix;
+        const int width = min(GS_SEL_BITS, shift);
+        const int lo = shift - width;
+        const uint64_t himask = shift >= 64 ? 0ull : ~((1ull << shift) - 1ull);
+        for (int i = tid; i < GS_SEL_BINS; i += kRowThreads) hist[i] = 0;
+        __syncthreads();
+        for (int64_t base = i_lo; base < i_hi; base += kRowUnroll * kRowThreads) {   // uniform trip count; loads in flight
+            uint64_t key[kRowUnroll];
+#pragma unroll
+            for (int u = 0; u < kRowUnroll; ++u) {
+                const int64_t i = base + tid + (int64_t)u * kRowThreads;
+                key[u] = i < i_hi ? src_key<WT>(src, b, i) : 0ull;
+            }
+#pragma unroll
+            for (int u = 0; u < kRowUnroll; ++u) {
+                // scores share their leading bits, so a digit's counter is hot: one atomic per distinct digit per warp
+                const bool live = key[u] != 0ull && (key[u] & himask) == prefix;
+                const uint32_t digit = live ? (uint32_t)((key[u] >> lo) & ((1u << width) - 1u)) : 0xFFFFFFFFu;
+                const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
+                if (live && lane == __ffs(peers) - 1) atomicAdd(&hist[digit], (uint32_t)__popc(peers));
+            }
+        }
+        cluster.sync();
+        // thread t owns bins 2t, 2t+1 (summed over the cluster); suffix sums from the top bin down
+        uint32_t c0 = 0, c1 = 0;
+        for (int r = 0; r < C; ++r) {
+            const uint2 v = *reinterpret_cast<const uint2*>(cluster.map_shared_rank(hist, r) + 2 * tid);
+            c0 += v.x;
+            c1 += v.y;
+        }
+        uint32_t incl = c0 + c1;                                  // inclusive suffix sum over threads >= tid
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_down_sync(0xFFFFFFFFu, incl, o);
+            if (lane + o < 32) incl += v;
+        }
+        if (lane == 0) part[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t v = part[lane], inc2 = v;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_down_sync(0xFFFFFFFFu, inc2, o);
+                if (lane + o < 32) inc2 += u;
+            }
+            part[lane] = inc2 - v;                                // items in warps above this one
+        }
+        __syncthreads();
+        const uint32_t k_rem = s_krem;
+        uint32_t above = part[warp] + incl - (c0 + c1);           // items in bins strictly above this thread's bins
+        cluster.sync();                                           // all remote reads done before the next zeroing; s_krem read
+        for (int j = 1; j >= 0; --j) {
+            const uint32_t c = j ? c1 : c0;
+            if (above < k_rem && above + c >= k_rem) {            // exactly one (thread, bin) matches
+                s_prefix = prefix | ((unsigned long long)(2 * tid + j) << lo);
+                s_krem = k_rem - above;
+                s_shift = lo;
+                if (c == k_rem - above || lo == 0) s_done = 1;    // the whole bin is wanted, or no bits are left
+            }
+            above += c;
+        }
+        __syncthreads();
+    }
+    // collect the keys >= threshold (exactly min(k, live) of them: all keys are distinct) in CTA 0, sort, decode
+    const uint64_t thr = s_prefix;
+    if (rank == 0)
+        for (int i = tid; i < kp2; i += kRowThreads) sk[i] = 0ull;
+    cluster.sync();
+    uint64_t* sk0 = cluster.map_shared_rank(sk, 0);
+    uint32_t* cnt0 = cluster.map_shared_rank(&s_cnt, 0);
+    for (int64_t base = i_lo; base < i_hi; base += kRowUnroll * kRowThreads) {
+        uint64_t key[kRowUnroll];
+#pragma unroll
+        for (int u = 0; u < kRowUnroll; ++u) {
+            const int64_t i = base + tid + (int64_t)u * kRowThreads;
+            key[u] = i < i_hi ? src_key<WT>(src, b, i) : 0ull;
+        }
+#pragma unroll
+        for (int u = 0; u < kRowUnroll; ++u) {
+            const bool take = key[u] != 0ull && key[u] >= thr;
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, take);
+            if (m) {
+                uint32_t pos0 = 0;
+                if (lane == __ffs(m) - 1) pos0 = atomicAdd(cnt0, (uint32_t)__popc(m));
+                pos0 = __shfl_sync(0xFFFFFFFFu, pos0, __ffs(m) - 1);
+                const uint32_t pos = pos0 + __popc(m & ((1u << lane) - 1u));
+                if (take && pos < (uint32_t)k) sk0[pos] = key[u];
+            }
+        }
+    }
+    cluster.sync();
+    if (rank != 0) return;
+    const uint32_t cnt = min(s_cnt, (uint32_t)k);
+    for (int size = 2; size <= kp2; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int i = tid; i < kp2 / 2; i += kRowThreads) {
+                const int lo2 = 2 * i - (i & (stride - 1));
+                const int hi2 = lo2 + stride;
+                const bool desc = (lo2 & size) == 0;
+                const uint64_t x = sk[lo2], y = sk[hi2];
+                if ((x < y) == desc) { sk[lo2] = y; sk[hi2] = x; }
+            }
+            __syncthreads();
+        }
+    }
+    for (int i = tid; i < k; i += kRowThreads) {
+        const uint64_t key = sk[i];
+        if (out_ids) {
+            if (key == 0ull) {
+                out_ids[b * k + i] = -1;
+                out_scores[b * k + i] = WT == GS_W_F32 ? 0xFF800000u : 0x80000000u;   // -inf | INT32_MIN
+            } else {
+                out_ids[b * k + i] = (int32_t)(0xFFFFFFFFu - (uint32_t)key);
+                const uint32_t o = (uint32_t)(key >> 32);
+                out_scores[b * k + i] = WT == GS_W_F32 ? gs_unord_f32(o) : (o ^ 0x80000000u);
+            }
+        }
+    }
+    if (tid == 0 && out_thr) out_thr[b] = cnt >= (uint32_t)k ? sk[k - 1] : 0ull;
+}
+
 struct Scratch { SelState* st; uint32_t* hist; uint64_t* sel; };
 Scratch carve(void* scratch, int64_t rows, int32_t k) {
     unsigned char* p = (unsigned char*)scratch;
@@ -233,6 +406,34 @@ gs_status_t run_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* 
     const int64_t max_items = src.keys ? src.cap : src.n_cols;
     const unsigned chunks = (unsigned)std::max<int64_t>(1, (max_items + kItemsPerCta - 1) / kItemsPerCta);
     if (rows > 65535) return GS_ERR_OUT_OF_RANGE;
+    if (max_items <= kRowFusedMax && !out_keys && !out_cnt) {
+        int kp2 = 32;
+        while (kp2 < k) kp2 <<= 1;
+        const size_t smem = (size_t)kp2 * 8 + GS_SEL_BINS * 4;
+        GS_CUDA(cudaFuncSetAttribute(k_sel_row<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        // CTAs per row: enough to spread a few rows over the chip, one when there are rows to spare
+        int C = 1;
+        while (C < 8 && rows * C < 128 && max_items > (int64_t)C * 8192) C <<= 1;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)(rows * C));
+        cfg.blockDim = dim3(kRowThreads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)C;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        {
+            GsProfScope ps(GS_K_SELECT, s);
+            GS_CUDA(cudaLaunchKernelEx(&cfg, k_sel_row<WT>, src, k, kp2, out_ids, (uint32_t*)out_scores, out_thr));
+        }
+        ++gs_tls_launches;
+        GS_CUDA(cudaGetLastError());
+        return GS_OK;
+    }
     {
         GsProfScope ps(GS_K_SELECT, s, 14);
         k_sel_init<<<(unsigned)rows, 256, 0, s>>>(src, rows, k, sc.st, sc.hist);
