@@ -110,7 +110,7 @@ typedef struct gs_info {
     int64_t bytes_head;        /* dense strips                                                        */
     int64_t bytes_total;
     int64_t forward_tail_nnz;  /* postings held by the CSR part of the forward index                  */
-    int32_t head_terms_term_parallel; /* strips the term-parallel kernel stages per tile (<= 32)      */
+    int32_t head_terms_term_parallel; /* strips the term-parallel kernel reads (= head_terms)          */
     int32_t reserved;
     int64_t forward_padded_nnz; /* slots of the CSR part: forward_tail_nnz + block padding             */
 } gs_info_t;
@@ -122,7 +122,7 @@ typedef struct gs_info {
 typedef struct gs_search_opts {
     int32_t algo;             /* gs_algo_t                                                              */
     uint32_t flags;
-    int32_t query_group;      /* term-parallel: queries per accumulator tile (0 = auto)                 */
+    int32_t query_group;      /* term-parallel: (doc tile, query) cell rows = warps per CTA, 1..8 (0 = 2)  */
     int32_t doc_query_tile;   /* doc-parallel: queries per pass over the forward index (0 = auto)       */
     int32_t sample_shift;     /* threshold sample = 1/2^shift of the doc tiles (0 = auto)               */
 } gs_search_opts_t;
@@ -136,7 +136,7 @@ typedef struct gs_stats {
     int32_t sample_tiles;      /* doc tiles scored densely to obtain the thresholds                    */
     int32_t doc_query_tile;    /* doc-parallel: queries per pass over the forward index (0 otherwise)  */
     int32_t doc_passes;        /* doc-parallel: passes over the forward index per full-collection launch */
-    int32_t query_group;       /* term-parallel: queries sharing one CTA's accumulator tiles           */
+    int32_t query_group;       /* term-parallel: cell rows (warps) per CTA                             */
 } gs_stats_t;
 
 /* ------------------------------------------------------------------------------------------------

@@ -391,7 +391,7 @@ gs_status_t gs_index_info(const gs_index_t* ix, gs_info_t* out) {
     out->num_tiles = ix->ntiles; out->head_terms = ix->H;
     out->bytes_inverted = ix->bytes_inverted; out->bytes_inverted_meta = ix->bytes_meta;
     out->bytes_forward = ix->bytes_forward; out->bytes_head = ix->bytes_head;
-    out->head_terms_term_parallel = ix->H_term; out->forward_tail_nnz = ix->P_tail;
+    out->head_terms_term_parallel = ix->H; out->forward_tail_nnz = ix->P_tail;
     out->forward_padded_nnz = ix->P_fwd; out->reserved = 0;
     out->bytes_total = ix->bytes_inverted + ix->bytes_meta + ix->bytes_forward + ix->bytes_head;
     return GS_OK;

@@ -6,8 +6,8 @@
 
 #include "../../include/gpusparse.h"
 
-#define GS_HEAD_MAX 32          // term-parallel: strips staged per tile / entries of a query's compact head list
-#define GS_STRIP_MAX 64         // dense strips kept by the index (the doc-parallel kernel uses all of them)
+#define GS_STRIP_MAX 64         // dense strips kept by the index
+#define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
 #define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings
 #define GS_SEL_BINS 2048        // radix-select digit: 11 bits
@@ -59,7 +59,6 @@ struct gs_index {
     uint32_t* seg = nullptr;         // [V][ntiles+1]
     // dense strips of the densest lists ("head" terms)
     int32_t H = 0;                   // strips (<= GS_STRIP_MAX), densest list first
-    int32_t H_term = 0;              // the first H_term strips fit the term-parallel kernel's shared memory
     int32_t head_terms_host[GS_STRIP_MAX];
     int16_t* head_slot = nullptr;    // [V]: strip number of a term or -1
     void* head_strip = nullptr;      // [H][N_pad] float | uint8 (0 where the doc is not in the list)
@@ -152,7 +151,7 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
 
-int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head);   // queries per CTA actually used
+int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head);   // cell rows (warps) per CTA actually used
 int gs_score_doc_qtile(int qtile);                                    // queries per pass actually used
 
 // doc-parallel: scratch holds the transposed query tile(s)

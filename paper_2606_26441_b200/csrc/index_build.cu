@@ -290,9 +290,6 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return h_len[a] > h_len[b]; });
     if ((int)order.size() > hmax) order.resize(hmax);
     ix->H = (int32_t)order.size();
-    // the term-parallel kernel stages a tile's strips in shared memory next to its accumulator rows (score_term.cu):
-    // it uses the densest H_term strips and scatters the other lists
-    ix->H_term = std::max(0, std::min({ix->H, GS_HEAD_MAX, (int)(200 * 1024 / (4 * (size_t)ix->Ts)) - 8}));
     std::vector<int16_t> h_slot(V, (int16_t)-1);
     for (int h = 0; h < GS_STRIP_MAX; ++h) ix->head_terms_host[h] = h < ix->H ? order[h] : -1;
     for (int h = 0; h < ix->H; ++h) h_slot[order[h]] = (int16_t)h;

@@ -2,7 +2,7 @@
 //
 // The paper pads queries to a [B, M] matrix of (term id, weight) in Python (PAPER.md L120-123,
 // L146-152).  Here one warp per query splits its terms into
-//   * head terms (the H_term densest lists, kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
+//   * head terms (the H densest lists, kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
 //   * tail terms: compacted (row b starts at indptr[b]) into tail_term/tail_w, weights converted to the
 //     accumulator type (float, or int32 for uint8 impacts).
 // Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
@@ -44,7 +44,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
             }
         }
         int slot = (ok && h_term > 0) ? (int)head_slot[t] : -1;
-        if (slot >= h_term) slot = -1;          // a strip the term-parallel kernel does not stage: scatter its list
+        if (slot >= h_term) slot = -1;
         const bool is_head = ok && slot >= 0;
         const unsigned mh = __ballot_sync(0xFFFFFFFFu, is_head);
         if (is_head) {
@@ -79,11 +79,11 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     GsProfScope ps(GS_K_INGEST, s);
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                   use_head ? ix->H_term : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                   use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                    qb->tail_w, qb->tail_cnt, qb->status);
     else
         k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                  use_head ? ix->H_term : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                  use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                   qb->tail_w, qb->tail_cnt, qb->status);
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());

@@ -3,26 +3,30 @@
 // PAPER.md Eq. (5): scores[d] += w_i * PL(t_i)[d] for all d in PL(t_i), one independent
 // scatter per query term; the paper launches one program per (query, term) that atomically adds
 // into a global [B,N] buffer (L118-125, L137-172) and names "scattered atomics" as the cost
-// (L172, L411).  Here the doc-id axis is cut into tiles of Ts docs and a CTA owns one doc tile x a
-// group of G queries; its G x Ts accumulators live in SHARED memory.
+// (L172, L411).  Here the doc-id axis is cut into tiles of Ts docs and ONE WARP owns the Ts
+// accumulators of one query in one doc tile ("cell row", 2 KB of shared memory at Ts = 512); a CTA
+// is a handful of such warps working on consecutive queries of the same tile, several CTAs per SM:
 //
-//   phase 1 (scatter, "tail" lists): a warp takes whole accumulator rows (queries) off a shared
-//     counter, so a row is only ever touched by one warp: plain LDS/FFMA/STS, no atomics, fixed
-//     order.  The per-(term, tile) segment table turns "the part of PL(t) inside this tile" into two
-//     loads, probed for 32 query terms at once (one per lane); only non-empty segments are visited,
-//     and each is streamed with coalesced loads, several independent 32-posting chunks in flight.
-//   phase 2 (epilogue, "head" lists): the <= 32 densest lists are stored as dense strips; the tile's
-//     strips are staged in shared memory once per CTA and every thread owns 4 consecutive documents
-//     of one query: 128-bit shared loads of the accumulators and of the strip of every head term
-//     the query actually contains (per-query compact lists), then the finished cells go to the sink
-//     (dense score matrix, or threshold filter -> candidate list).
+//   1. zero the row;
+//   2. scatter the query's "tail" lists: the per-(term, tile) segment table turns "the part of
+//      PL(t) inside this tile" into two loads, probed for 32 query terms at once (one per lane,
+//      the weights travel by warp shuffle); only non-empty segments are visited, each streamed
+//      with coalesced loads, several independent 32-posting chunks in flight.  The row is only
+//      ever touched by its warp: plain LDS/FFMA/STS, no atomics, fixed order;
+//   3. add the query's "head" terms — the densest lists, stored as dense strips — straight from
+//      the global strips (128-bit loads, a lane owns 4 consecutive documents; the warps of a CTA
+//      share a tile, so the strips come out of L1), through the query's compact (strip, weight) list;
+//   4. hand the finished cells to the sink: dense score matrix, or threshold filter -> candidate
+//      list, where the warp reserves its slice of the list with ONE atomic.
+//
+// An earlier version gave a CTA a group of 64 queries and staged the tile's strips in shared memory;
+// measured on B200 it was slower at every batch size (barrier stalls, idle warps, strips nobody
+// used): DESIGN.md §7.
 #include <algorithm>
 
 #include "gs_internal.cuh"
 
 namespace {
-
-constexpr int kMaxThreads = 1024;
 
 template <int WT> struct Num;
 template <> struct Num<GS_W_F32> {
@@ -33,9 +37,6 @@ template <> struct Num<GS_W_F32> {
     static __device__ __forceinline__ A mac(A acc, A q, A w) { return fmaf(q, w, acc); }
     static __device__ __forceinline__ A widen(W w) { return w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return __float_as_uint(a); }
-    static __device__ __forceinline__ bool below(A s, uint32_t thr_ord) {
-        return s < __uint_as_float(gs_unord_f32(thr_ord));      // false for a NaN threshold (thr_ord == 0: accept all)
-    }
 };
 template <> struct Num<GS_W_U8> {
     using W = uint8_t;
@@ -45,7 +46,6 @@ template <> struct Num<GS_W_U8> {
     static __device__ __forceinline__ A mac(A acc, A q, A w) { return acc + q * w; }
     static __device__ __forceinline__ A widen(W w) { return (int32_t)w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return (uint32_t)a; }
-    static __device__ __forceinline__ bool below(A s, uint32_t thr_ord) { return s < (int32_t)(thr_ord ^ 0x80000000u); }
 };
 
 struct TermParams {
@@ -55,8 +55,8 @@ struct TermParams {
     // queries
     const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
     const uint32_t* tail_w; const int32_t* tail_cnt;
-    int64_t q0; int32_t nq; int32_t G;          // queries [q0, q0+nq), G per CTA
-    int32_t n_qgroups;
+    int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
+    int32_t warps;                              // cell rows (warps) per CTA
     gs_tileset ts;
     gs_sink sink;
     int32_t vec4;                               // dense sink rows are 16-byte aligned
@@ -92,169 +92,32 @@ __device__ __forceinline__ void scatter_segment(const int32_t* __restrict__ dp, 
     }
 }
 
+// dense sink: the finished cells (query b, docs doc0 .. doc0+3) go to the score matrix
 template <int WT>
-__device__ __forceinline__ void emit_candidate(const gs_sink& sink, int64_t b, uint64_t thr, int32_t doc,
-                                               typename Num<WT>::A s) {
-    const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(s)), (uint32_t)doc);
-    if (key >= thr) {
-        const uint32_t pos = atomicAdd(&sink.cand_cnt[b], 1u);
-        if ((int64_t)pos < sink.cand_cap) sink.cand[b * sink.cand_cap + pos] = key;
-    }
-}
-
-// the finished cells (query b, docs doc0 .. doc0+3) go to the sink: dense score matrix, or threshold filter -> candidates
-template <int WT>
-__device__ __forceinline__ void sink_quad(const TermParams& p, int64_t b, int j, int dq, int64_t doc0,
-                                          typename Num<WT>::A s0, typename Num<WT>::A s1, typename Num<WT>::A s2,
-                                          typename Num<WT>::A s3) {
-    if (p.sink.thr == nullptr) {
-        uint32_t* out = p.sink.dense + (b - p.q0) * p.sink.ld + (int64_t)j * p.Ts + 4 * dq;
-        if (doc0 + 3 < p.N && p.vec4) {
-            *reinterpret_cast<uint4*>(out) =
-                make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
-        } else {
-            if (doc0 + 0 < p.N) out[0] = Num<WT>::bits(s0);
-            if (doc0 + 1 < p.N) out[1] = Num<WT>::bits(s1);
-            if (doc0 + 2 < p.N) out[2] = Num<WT>::bits(s2);
-            if (doc0 + 3 < p.N) out[3] = Num<WT>::bits(s3);
-        }
+__device__ __forceinline__ void store_quad(const TermParams& p, int64_t b, int j, int dq, int64_t doc0,
+                                           typename Num<WT>::A s0, typename Num<WT>::A s1, typename Num<WT>::A s2,
+                                           typename Num<WT>::A s3) {
+    uint32_t* out = p.sink.dense + (b - p.q0) * p.sink.ld + (int64_t)j * p.Ts + 4 * dq;
+    if (doc0 + 3 < p.N && p.vec4) {
+        *reinterpret_cast<uint4*>(out) = make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
     } else {
-        const uint64_t thr = p.sink.thr[b];
-        const uint32_t to = (uint32_t)(thr >> 32);
-        const bool r0 = Num<WT>::below(s0, to), r1 = Num<WT>::below(s1, to), r2 = Num<WT>::below(s2, to),
-                   r3 = Num<WT>::below(s3, to);
-        if (!(r0 && r1 && r2 && r3)) {
-            if (!r0 && doc0 + 0 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 0, s0);
-            if (!r1 && doc0 + 1 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 1, s1);
-            if (!r2 && doc0 + 2 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 2, s2);
-            if (!r3 && doc0 + 3 < p.N) emit_candidate<WT>(p.sink, b, thr, (int32_t)doc0 + 3, s3);
-        }
+        if (doc0 + 0 < p.N) out[0] = Num<WT>::bits(s0);
+        if (doc0 + 1 < p.N) out[1] = Num<WT>::bits(s1);
+        if (doc0 + 2 < p.N) out[2] = Num<WT>::bits(s2);
+        if (doc0 + 3 < p.N) out[3] = Num<WT>::bits(s3);
     }
 }
 
-template <int WT>
-__global__ void __launch_bounds__(kMaxThreads, 1) k_score_term(const TermParams p) {
-    using W = typename Num<WT>::W;
-    using A = typename Num<WT>::A;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Ts = p.Ts, H = p.H;
-    A* acc = reinterpret_cast<A*>(smem_raw);                                  // [G][Ts]
-    A* strips = acc + (size_t)p.G * Ts;                                       // [H][Ts]
-    uint2* hq = reinterpret_cast<uint2*>(strips + (size_t)H * Ts);            // [G][GS_HEAD_MAX] (strip, weight bits)
-    int* hcnt = reinterpret_cast<int*>(hq + (size_t)p.G * GS_HEAD_MAX);       // [G]
-    int* next_row = hcnt + p.G;
-    const int lane = threadIdx.x & 31;
-    const int nthreads = blockDim.x;
-    const int qg = blockIdx.x % p.n_qgroups;
-    const int j = blockIdx.x / p.n_qgroups;                                   // position in the tile set
-    const int g0 = qg * p.G;
-    const int Gc = min(p.G, p.nq - g0);
-    const int tile = p.ts.first + j * p.ts.stride;
-    const int32_t base = tile * Ts;
-    const int quads = Ts >> 2;
-
-    // ---- stage: zero the accumulators, copy the tile's strips and the group's head lists
-    {
-        int4* a4 = reinterpret_cast<int4*>(acc);
-        for (int i = threadIdx.x; i < Gc * quads; i += nthreads) a4[i] = make_int4(0, 0, 0, 0);
-        if (H > 0) {
-            const W* __restrict__ gstrip = reinterpret_cast<const W*>(p.head_strip) + base;
-            for (int i = threadIdx.x; i < H * quads; i += nthreads) {
-                const int h = i / quads, dq = i - h * quads;
-                const W* src = gstrip + (size_t)h * p.N_pad + 4 * dq;
-                int4 v;
-                if (WT == GS_W_F32) {
-                    v = *reinterpret_cast<const int4*>(src);
-                } else {
-                    const uchar4 u = *reinterpret_cast<const uchar4*>(src);
-                    v = make_int4(u.x, u.y, u.z, u.w);
-                }
-                *reinterpret_cast<int4*>(strips + (size_t)h * Ts + 4 * dq) = v;
-            }
-            for (int i = threadIdx.x; i < Gc * GS_HEAD_MAX; i += nthreads)
-                hq[i] = p.head_pair[(p.q0 + g0) * GS_HEAD_MAX + i];
-            for (int i = threadIdx.x; i < Gc; i += nthreads) hcnt[i] = p.head_cnt[p.q0 + g0 + i];
-        }
-        if (threadIdx.x == 0) *next_row = 0;
-    }
-    __syncthreads();
-
-    // ---- phase 1: scatter the tail lists; a warp owns the rows it draws from the counter
-    const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
-    for (;;) {
-        int g = 0;
-        if (lane == 0) g = atomicAdd(next_row, 1);
-        g = __shfl_sync(0xFFFFFFFFu, g, 0);
-        if (g >= Gc) break;
-        const int64_t b = p.q0 + g0 + g;
-        A* row = acc + (size_t)g * Ts;
-        const int64_t qa = p.q_indptr[b];
-        const int cnt = p.tail_cnt[b];
-        for (int i0 = 0; i0 < cnt; i0 += 32) {
-            int64_t start = 0;
-            int n = 0;
-            uint32_t wq = 0;
-            if (i0 + lane < cnt) {
-                const int32_t t = p.tail_term[qa + i0 + lane];
-                wq = p.tail_w[qa + i0 + lane];
-                const uint32_t* sr = p.seg + (size_t)t * (p.ntiles + 1) + tile;
-                const uint32_t lo = sr[0], hi = sr[1];
-                n = (int)(hi - lo);
-                start = p.inv_off[t] + lo;
-            }
-            unsigned m = __ballot_sync(0xFFFFFFFFu, n > 0);
-            while (m) {
-                const int src = __ffs(m) - 1;
-                m &= m - 1;
-                const int n_j = __shfl_sync(0xFFFFFFFFu, n, src);
-                const int64_t start_j = __shfl_sync(0xFFFFFFFFu, start, src);
-                const A q = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
-                scatter_segment<WT>(p.inv_doc + start_j, inv_w + start_j, n_j, q, row, base, Ts, lane);
-            }
-        }
-    }
-    __syncthreads();
-
-    // ---- phase 2: head strips + sink.  A thread owns 4 consecutive docs of one query at a time.
-    for (int item = threadIdx.x; item < Gc * quads; item += nthreads) {
-        const int g = item / quads, dq = item - g * quads;
-        const int64_t b = p.q0 + g0 + g;
-        const int4 a4 = *reinterpret_cast<const int4*>(acc + (size_t)g * Ts + 4 * dq);
-        A s0 = Num<WT>::from_bits(a4.x), s1 = Num<WT>::from_bits(a4.y), s2 = Num<WT>::from_bits(a4.z),
-          s3 = Num<WT>::from_bits(a4.w);
-        if (H > 0) {
-            const uint2* hl = hq + g * GS_HEAD_MAX;
-            const int nh = hcnt[g];
-            for (int i = 0; i < nh; ++i) {
-                const uint2 e = hl[i];
-                const A q = Num<WT>::qw(e.y);
-                const int4 v = *reinterpret_cast<const int4*>(strips + (size_t)e.x * Ts + 4 * dq);
-                s0 = Num<WT>::mac(s0, q, Num<WT>::from_bits(v.x));
-                s1 = Num<WT>::mac(s1, q, Num<WT>::from_bits(v.y));
-                s2 = Num<WT>::mac(s2, q, Num<WT>::from_bits(v.z));
-                s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
-            }
-        }
-        sink_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, s0, s1, s2, s3);
-    }
-}
-
-// ---- small batches: one WARP per (doc tile, query) cell row.
-// With a handful of queries the CTA-per-(tile, query group) kernel above leaves 31 of its 32 warps idle during the
-// scatter and stages strips nobody uses.  Here a warp owns the Ts accumulators of one query in one doc tile (2 KB
-// of shared memory), 8 such warps per CTA and several CTAs per SM: zero, scatter the query's tail lists (same
-// segment walk as above), then add the query's head terms straight from the global strips (each strip value
-// is used exactly once, so there is nothing to stage) and hand the cells to the sink.  No atomics, fixed order.
-constexpr int kWarpsSmall = 8;
+constexpr int kWarpsDefault = 2, kWarpsMax = 8;
 
 template <int WT>
-__global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const TermParams p) {
+__global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams p) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int Ts = p.Ts;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t item = (int64_t)blockIdx.x * kWarpsSmall + warp;
+    const int64_t item = (int64_t)blockIdx.x * p.warps + warp;
     if (item >= (int64_t)p.ts.count * p.nq) return;
     const int j = (int)(item / p.nq);                       // position in the tile set
     const int64_t b = p.q0 + (item - (int64_t)j * p.nq);
@@ -328,7 +191,7 @@ __global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const Term
         }
         const int64_t doc0 = (int64_t)base + 4 * dq;
         if (!filter) {
-            sink_quad<WT>(p, b, j, dq, doc0, s0, s1, s2, s3);
+            store_quad<WT>(p, b, j, dq, doc0, s0, s1, s2, s3);
         } else {
             reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
             n_pass += (uint32_t)passes(s0, doc0) + (uint32_t)passes(s1, doc0 + 1) + (uint32_t)passes(s2, doc0 + 2) +
@@ -362,84 +225,47 @@ __global__ void __launch_bounds__(kWarpsSmall * 32) k_score_term_warp(const Term
     }
 }
 
-struct Shape { int G; int threads; size_t smem; };
-
-// shared memory: G accumulator rows + H strips of Ts words, G head lists, G counts, the row counter
-size_t smem_for(const gs_index* ix, int H, int G) {
-    return ((size_t)G + H) * ix->Ts * 4 + (size_t)G * GS_HEAD_MAX * 8 + (size_t)G * 4 + 16;
-}
-
-Shape shape_for(const gs_index* ix, int H, int64_t nq, int group) {
-    const size_t budget = 220 * 1024;
-    int gmax = 0;
-    while (gmax < 4096 && smem_for(ix, H, gmax + 1) <= budget) ++gmax;
-    Shape s{};
-    int G = group > 0 ? group : 64;                 // 2 rows per warp at 1024 threads
-    G = (int)std::max<int64_t>(0, std::min<int64_t>(std::min<int64_t>(G, nq), gmax));
-    s.G = G;
-    s.threads = kMaxThreads;
-    s.smem = smem_for(ix, H, std::max(G, 1));
-    return s;
-}
+int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
 template <int WT>
-gs_status_t launch(const TermParams& p, unsigned grid, const Shape& sh, cudaStream_t s) {
-    GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh.smem));
+gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
+    GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     {
         GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term<WT><<<grid, sh.threads, sh.smem, s>>>(p);
+        k_score_term<WT><<<grid, p.warps * 32, smem, s>>>(p);
     }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;
 }
-
-template <int WT>
-gs_status_t launch_warp(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
-    GS_CUDA(cudaFuncSetAttribute(k_score_term_warp<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    {
-        GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term_warp<WT><<<grid, kWarpsSmall * 32, smem, s>>>(p);
-    }
-    ++gs_tls_launches;
-    GS_CUDA(cudaGetLastError());
-    return GS_OK;
-}
-
-// query_group < 0 asks for the warp-per-cell-row kernel, 0 picks it for small batches
-bool use_warp_kernel(int64_t nq, int group) { return group < 0 || (group == 0 && nq <= 16); }
 
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    if (use_warp_kernel(nq, group)) return 1;
-    return shape_for(ix, use_head ? ix->H_term : 0, nq, group).G;
+    (void)ix; (void)nq; (void)use_head;
+    return norm_warps(group);
 }
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
-    const int H = use_head ? ix->H_term : 0;
-    const Shape sh = shape_for(ix, H, nq, group);
-    if (sh.G < 1) return GS_ERR_OOM;                 // one accumulator row + the strips do not fit: tile_docs too large
     TermParams p{};
     p.inv_off = ix->inv_off; p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg = ix->seg;
-    p.head_strip = ix->head_strip; p.H = H; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
+    p.head_strip = ix->head_strip; p.H = use_head ? ix->H : 0; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
     p.ntiles = ix->ntiles;
     p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_term = qb.tail_term;
     p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt;
-    p.q0 = q0; p.nq = (int32_t)nq; p.G = sh.G; p.n_qgroups = (int)((nq + sh.G - 1) / sh.G);
+    p.q0 = q0; p.nq = (int32_t)nq;
+    p.warps = norm_warps(group);
     p.ts = ts; p.sink = sink;
     p.vec4 = sink.dense && (((uintptr_t)sink.dense | (uintptr_t)(sink.ld * 4)) & 15) == 0;
-    if (use_warp_kernel(nq, group)) {
-        const size_t smem = (size_t)kWarpsSmall * ix->Ts * 4;
-        const int64_t grid = ((int64_t)ts.count * nq + kWarpsSmall - 1) / kWarpsSmall;
-        if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-        p.G = 1;
-        return ix->wtype == GS_W_F32 ? launch_warp<GS_W_F32>(p, (unsigned)grid, smem, s)
-                                     : launch_warp<GS_W_U8>(p, (unsigned)grid, smem, s);
-    }
-    const int64_t grid = (int64_t)p.n_qgroups * ts.count;
+    int dev = 0, smem_max = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    while (p.warps > 1 && (size_t)p.warps * ix->Ts * 4 > (size_t)smem_max) p.warps >>= 1;
+    const size_t smem = (size_t)p.warps * ix->Ts * 4;
+    if (smem > (size_t)smem_max) return GS_ERR_OOM;                 // one accumulator row does not fit: tile_docs too large
+    const int64_t grid = ((int64_t)ts.count * nq + p.warps - 1) / p.warps;
     if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-    return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, sh, s) : launch<GS_W_U8>(p, (unsigned)grid, sh, s);
+    return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, smem, s) : launch<GS_W_U8>(p, (unsigned)grid, smem, s);
 }

@@ -16,13 +16,13 @@ import parity  # tests/parity.py (pytest puts tests/ on sys.path)
 
 pytestmark = pytest.mark.gpu
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
-ALGOS = ["term", "term_cta", "doc"]
+ALGOS = ["term", "term_w2", "doc"]
 
 
 def aopt(algo):
-    """Search options of a parametrised kernel: "term" = term-parallel with its own choice (the warp-per-cell-row
-    kernel for batches <= 16), "term_cta" = the CTA-per-(tile, query group) kernel forced, "doc" = document-parallel."""
-    return {"term": dict(algo="term"), "term_cta": dict(algo="term", query_group=64), "doc": dict(algo="doc")}[algo]
+    """Search options of a parametrised kernel: "term" = term-parallel (default: 2 cell rows per CTA), "term_w2" = the same
+    kernel with 5 cell rows per CTA (other tile/query interleaving), "doc" = document-parallel."""
+    return {"term": dict(algo="term"), "term_w2": dict(algo="term", query_group=5), "doc": dict(algo="doc")}[algo]
 
 
 @pytest.fixture(scope="module")
@@ -326,7 +326,9 @@ def host_topk(row, k):
     return order
 
 
-@pytest.mark.parametrize("n,k", [(1, 1), (100, 100), (5000, 10), (100_000, 1000), (300_001, 4096)])
+# rows of up to 2^20 items take the one-launch cluster select, longer rows the multi-launch one: both sides of the switch
+@pytest.mark.parametrize("n,k", [(1, 1), (100, 100), (5000, 10), (100_000, 1000), (300_001, 4096), (1_048_576, 10),
+                                 (1_048_577, 1000), (1_300_003, 4096)])
 def test_topk_dense_synthetic_f32(gs, n, k):
     import torch
     rng = np.random.default_rng(n + k)
@@ -460,9 +462,9 @@ def test_paper_scale_sampled(gs, paper_docs, mode, k):
             assert len(np.unique(ids[b])) == k and ids[b].min() >= 0 and ids[b].max() < docs.rows
             d = np.diff(sc[b].astype(np.float64))
             assert np.all(d <= 0) and np.all(ids[b][:-1][d == 0] < ids[b][1:][d == 0])
-    # small batches take other paths (warp-per-cell-row term kernel, document-parallel with a tile of 8)
+    # small batches take other plans (bigger threshold sample stride, document-parallel with a tile of 8)
     few = queries.slice_rows(0, 3)
-    for opt in (dict(algo="term"), dict(algo="term", query_group=64), dict(algo="doc"), dict(algo="auto")):
+    for opt in (dict(algo="term"), dict(algo="term", query_group=8), dict(algo="doc"), dict(algo="auto")):
         ids, sc = gpu_search(gs, ix, few, k, **opt)
         b_idx = np.repeat(np.arange(few.rows, dtype=np.int64), k)
         true = oracle.score_pairs(R_q, R_d, b_idx, ids.reshape(-1).astype(np.int64)).reshape(few.rows, k)
