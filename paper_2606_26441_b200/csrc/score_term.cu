@@ -56,7 +56,8 @@ struct TermParams {
     const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
     const uint32_t* tail_w; const int32_t* tail_cnt;
     int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
-    int32_t warps;                              // cell rows (warps) per CTA
+    int32_t warps;                              // cell rows (warps) per CTA (small-batch kernel)
+    int32_t chunk, n_chunks;                    // staged kernel: queries per CTA, CTAs per doc tile
     gs_tileset ts;
     gs_sink sink;
     int32_t vec4;                               // dense sink rows are 16-byte aligned
@@ -109,26 +110,26 @@ __device__ __forceinline__ void store_quad(const TermParams& p, int64_t b, int j
 }
 
 constexpr int kWarpsDefault = 2, kWarpsMax = 8;
+constexpr int kSegBatch = 2;      // segments whose first 32 postings are loaded together
+constexpr int kQuadRounds = 2;    // rounds of 32 quads (128 documents) a lane keeps in registers in the epilogue
 
-template <int WT>
-__global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams p) {
+// One (doc tile, query) cell row, done by one warp.  STAGED: the tile's strips are in shared memory (s_strip, [H][Ts]);
+// otherwise they are read from the global strips.
+template <int WT, bool STAGED>
+__device__ __forceinline__ void process_item(const TermParams& p, typename Num<WT>::A* row,
+                                             const typename Num<WT>::W* s_strip, int j, int64_t b, int lane) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     const int Ts = p.Ts;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t item = (int64_t)blockIdx.x * p.warps + warp;
-    if (item >= (int64_t)p.ts.count * p.nq) return;
-    const int j = (int)(item / p.nq);                       // position in the tile set
-    const int64_t b = p.q0 + (item - (int64_t)j * p.nq);
     const int tile = p.ts.first + j * p.ts.stride;
     const int32_t base = tile * Ts;
     const int quads = Ts >> 2;
-    A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * Ts;
     for (int dq = lane; dq < quads; dq += 32) reinterpret_cast<int4*>(row)[dq] = make_int4(0, 0, 0, 0);
     __syncwarp();
 
-    // scatter the tail lists of the query: segment of each list inside this tile, 32 terms probed at once
+    // scatter the tail lists of the query: segment of each list inside this tile, 32 terms probed at once.  The
+    // non-empty segments are applied one after the other (two lists may hit the same document), but the first 32
+    // postings of kSegBatch segments are LOADED together, so their latencies overlap.
     const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
     const int64_t qa = p.q_indptr[b];
     const int cnt = p.tail_cnt[b];
@@ -146,56 +147,107 @@ __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams 
         }
         unsigned m = __ballot_sync(0xFFFFFFFFu, n > 0);
         while (m) {
-            const int src = __ffs(m) - 1;
-            m &= m - 1;
-            const int n_j = __shfl_sync(0xFFFFFFFFu, n, src);
-            const int64_t start_j = __shfl_sync(0xFFFFFFFFu, start, src);
-            const A q = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
-            scatter_segment<WT>(p.inv_doc + start_j, inv_w + start_j, n_j, q, row, base, Ts, lane);
-            __syncwarp();                                   // two lists may hit the same document
+            int n_j[kSegBatch];
+            int64_t start_j[kSegBatch];
+            A q_j[kSegBatch], w_j[kSegBatch];
+            int32_t rel_j[kSegBatch];
+#pragma unroll
+            for (int u = 0; u < kSegBatch; ++u) {
+                n_j[u] = 0;
+                if (m) {                                    // uniform
+                    const int src = __ffs(m) - 1;
+                    m &= m - 1;
+                    n_j[u] = __shfl_sync(0xFFFFFFFFu, n, src);
+                    start_j[u] = __shfl_sync(0xFFFFFFFFu, start, src);
+                    q_j[u] = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
+                    const bool ok = lane < n_j[u];
+                    rel_j[u] = ok ? p.inv_doc[start_j[u] + lane] - base : -1;
+                    w_j[u] = ok ? Num<WT>::widen(inv_w[start_j[u] + lane]) : A(0);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < kSegBatch; ++u) {
+                if (n_j[u] > 0) {                           // uniform
+                    if ((uint32_t)rel_j[u] < (uint32_t)Ts) row[rel_j[u]] = Num<WT>::mac(row[rel_j[u]], q_j[u], w_j[u]);
+                    if (n_j[u] > 32)
+                        scatter_segment<WT>(p.inv_doc + start_j[u] + 32, inv_w + start_j[u] + 32, n_j[u] - 32, q_j[u], row, base, Ts, lane);
+                    __syncwarp();                           // two lists may hit the same document
+                }
+            }
         }
     }
     __syncwarp();
 
-    // head strips + sink: a lane owns 4 consecutive documents at a time.  Filter mode makes two passes over the row so
-    // that a warp reserves its slice of the query's candidate list with ONE atomic: pass 1 finishes the scores in place
-    // and counts the cells that pass the threshold, pass 2 writes their keys.
+    // head strips + sink.  A lane owns 4 consecutive documents ("quad") in each of up to kQuadRounds rounds of 32
+    // quads; the strip loop is the OUTER loop, so one (strip, weight) entry feeds kQuadRounds independent 128-bit
+    // strip loads.  Filter mode makes two passes over the row so that a warp reserves its slice of the query's
+    // candidate list with ONE atomic: pass 1 finishes the scores in place and counts the cells that pass the
+    // threshold, pass 2 writes their keys.
     const int nh = p.H > 0 ? p.head_cnt[b] : 0;
     const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
-    const W* __restrict__ gstrip = reinterpret_cast<const W*>(p.head_strip) + base;
+    const W* __restrict__ gstrip = STAGED ? s_strip : reinterpret_cast<const W*>(p.head_strip) + base;
+    const size_t strip_ld = STAGED ? (size_t)Ts : (size_t)p.N_pad;
     const bool filter = p.sink.thr != nullptr;
     const uint64_t thr = filter ? p.sink.thr[b] : 0ull;
+    // score of the threshold key: a cell above it passes, a cell equal to it is decided by the full key (doc id)
+    const A thr_s = Num<WT>::from_bits((int)(WT == GS_W_F32 ? gs_unord_f32((uint32_t)(thr >> 32)) : ((uint32_t)(thr >> 32) ^ 0x80000000u)));
+    const bool accept_all = thr == 0ull;
     auto passes = [&](A sc, int64_t doc) -> bool {
-        return doc < p.N && gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc)), (uint32_t)doc) >= thr;
+        if (doc >= p.N) return false;
+        if (accept_all || sc > thr_s) return true;
+        return sc == thr_s && gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc)), (uint32_t)doc) >= thr;
     };
     uint32_t n_pass = 0;
-    for (int dq = lane; dq < quads; dq += 32) {
-        const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
-        A s0 = Num<WT>::from_bits(a4.x), s1 = Num<WT>::from_bits(a4.y), s2 = Num<WT>::from_bits(a4.z),
-          s3 = Num<WT>::from_bits(a4.w);
-        for (int i = 0; i < nh; ++i) {
-            const uint2 e = hl[i];
-            const A q = Num<WT>::qw(e.y);
-            const W* src = gstrip + (size_t)e.x * p.N_pad + 4 * dq;
-            int4 v;
-            if (WT == GS_W_F32) {
-                v = __ldg(reinterpret_cast<const int4*>(src));
-            } else {
-                const uchar4 u = __ldg(reinterpret_cast<const uchar4*>(src));
-                v = make_int4(u.x, u.y, u.z, u.w);
-            }
-            s0 = Num<WT>::mac(s0, q, Num<WT>::from_bits(v.x));
-            s1 = Num<WT>::mac(s1, q, Num<WT>::from_bits(v.y));
-            s2 = Num<WT>::mac(s2, q, Num<WT>::from_bits(v.z));
-            s3 = Num<WT>::mac(s3, q, Num<WT>::from_bits(v.w));
+    for (int dq0 = 0; dq0 < quads; dq0 += 32 * kQuadRounds) {
+        A sc[kQuadRounds][4];
+#pragma unroll
+        for (int r = 0; r < kQuadRounds; ++r) {
+            const int dq = dq0 + 32 * r + lane;
+            const int4 a4 = dq < quads ? reinterpret_cast<const int4*>(row)[dq] : make_int4(0, 0, 0, 0);
+            sc[r][0] = Num<WT>::from_bits(a4.x); sc[r][1] = Num<WT>::from_bits(a4.y);
+            sc[r][2] = Num<WT>::from_bits(a4.z); sc[r][3] = Num<WT>::from_bits(a4.w);
         }
-        const int64_t doc0 = (int64_t)base + 4 * dq;
-        if (!filter) {
-            store_quad<WT>(p, b, j, dq, doc0, s0, s1, s2, s3);
-        } else {
-            reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(s0), Num<WT>::bits(s1), Num<WT>::bits(s2), Num<WT>::bits(s3));
-            n_pass += (uint32_t)passes(s0, doc0) + (uint32_t)passes(s1, doc0 + 1) + (uint32_t)passes(s2, doc0 + 2) +
-                      (uint32_t)passes(s3, doc0 + 3);
+        for (int i = 0; i < nh; ++i) {
+            const uint2 e = __ldg(hl + i);
+            const A q = Num<WT>::qw(e.y);
+            const W* src = gstrip + (size_t)e.x * strip_ld + 4 * (dq0 + lane);
+            int4 v[kQuadRounds];
+#pragma unroll
+            for (int r = 0; r < kQuadRounds; ++r) {
+                if (dq0 + 32 * r + lane < quads) {
+                    if (WT == GS_W_F32) {
+                        v[r] = STAGED ? *reinterpret_cast<const int4*>(src + 128 * r) : __ldg(reinterpret_cast<const int4*>(src + 128 * r));
+                    } else {
+                        const uchar4 u = STAGED ? *reinterpret_cast<const uchar4*>(src + 128 * r)
+                                                : __ldg(reinterpret_cast<const uchar4*>(src + 128 * r));
+                        v[r] = make_int4(u.x, u.y, u.z, u.w);
+                    }
+                } else {
+                    v[r] = make_int4(0, 0, 0, 0);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < kQuadRounds; ++r) {
+                sc[r][0] = Num<WT>::mac(sc[r][0], q, Num<WT>::from_bits(v[r].x));
+                sc[r][1] = Num<WT>::mac(sc[r][1], q, Num<WT>::from_bits(v[r].y));
+                sc[r][2] = Num<WT>::mac(sc[r][2], q, Num<WT>::from_bits(v[r].z));
+                sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < kQuadRounds; ++r) {
+            const int dq = dq0 + 32 * r + lane;
+            if (dq < quads) {
+                const int64_t doc0 = (int64_t)base + 4 * dq;
+                if (!filter) {
+                    store_quad<WT>(p, b, j, dq, doc0, sc[r][0], sc[r][1], sc[r][2], sc[r][3]);
+                } else {
+                    reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(sc[r][0]), Num<WT>::bits(sc[r][1]),
+                                                                   Num<WT>::bits(sc[r][2]), Num<WT>::bits(sc[r][3]));
+                    n_pass += (uint32_t)passes(sc[r][0], doc0) + (uint32_t)passes(sc[r][1], doc0 + 1) +
+                              (uint32_t)passes(sc[r][2], doc0 + 2) + (uint32_t)passes(sc[r][3], doc0 + 3);
+                }
+            }
         }
     }
     if (!filter) return;
@@ -209,6 +261,7 @@ __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams 
     uint32_t pos = 0;
     if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b], total);
     pos = __shfl_sync(0xFFFFFFFFu, pos, 0) + incl - n_pass;
+    if (n_pass == 0u) return;
     uint64_t* cand = p.sink.cand + b * p.sink.cand_cap;
     for (int dq = lane; dq < quads; dq += 32) {
         const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
@@ -225,12 +278,63 @@ __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams 
     }
 }
 
+// small batches: a warp takes ONE cell row; consecutive warps take consecutive queries of the same tile
+template <int WT>
+__global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams p) {
+    using A = typename Num<WT>::A;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t item = (int64_t)blockIdx.x * p.warps + warp;
+    if (item >= (int64_t)p.ts.count * p.nq) return;
+    const int j = (int)(item / p.nq);                       // position in the tile set
+    const int64_t b = p.q0 + (item - (int64_t)j * p.nq);
+    A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * p.Ts;
+    process_item<WT, false>(p, row, nullptr, j, b, lane);
+}
+
+// batches: a CTA of kWarpsStaged warps takes ONE doc tile and a chunk of up to p.chunk queries; it stages the tile's
+// strips in shared memory once (without this every cell row re-reads its strips from L2: CTAs of one tile land on
+// different SMs, so L1 does not help — measured 191 GB of L2 reads per batch), then every warp walks its share of the
+// chunk's queries on its own, with no barrier after the staging.
+constexpr int kWarpsStaged = 32;
+
+template <int WT>
+__global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(const TermParams p) {
+    using W = typename Num<WT>::W;
+    using A = typename Num<WT>::A;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Ts = p.Ts;
+    const int j = (int)(blockIdx.x / p.n_chunks);
+    const int chunk = (int)(blockIdx.x - (unsigned)j * p.n_chunks);
+    A* rows = reinterpret_cast<A*>(smem_raw);                                   // [kWarpsStaged][Ts]
+    W* s_strip = reinterpret_cast<W*>(rows + (size_t)kWarpsStaged * Ts);         // [H][Ts]
+    {
+        const int tile = p.ts.first + j * p.ts.stride;
+        const W* __restrict__ g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * Ts;
+        const int per = Ts / (16 / (int)sizeof(W));                            // 16-byte pieces per strip (Ts % 32 == 0)
+        for (int i = threadIdx.x; i < p.H * per; i += kWarpsStaged * 32) {
+            const int h = i / per, c = i - h * per;
+            reinterpret_cast<int4*>(s_strip + (size_t)h * Ts)[c] =
+                __ldg(reinterpret_cast<const int4*>(g + (size_t)h * p.N_pad) + c);
+        }
+    }
+    __syncthreads();
+    const int q_end = min(p.nq, (chunk + 1) * p.chunk);
+    for (int q = chunk * p.chunk + warp; q < q_end; q += kWarpsStaged)
+        process_item<WT, true>(p, rows + (size_t)warp * Ts, s_strip, j, p.q0 + q, lane);
+}
+
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
 template <int WT>
-gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t s) {
-    GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    {
+gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged, cudaStream_t s) {
+    if (staged) {
+        GS_CUDA(cudaFuncSetAttribute(k_score_term_staged<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GsProfScope ps(GS_K_SCORE_TERM, s);
+        k_score_term_staged<WT><<<grid, kWarpsStaged * 32, smem, s>>>(p);
+    } else {
+        GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         GsProfScope ps(GS_K_SCORE_TERM, s);
         k_score_term<WT><<<grid, p.warps * 32, smem, s>>>(p);
     }
@@ -239,10 +343,13 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, cudaStream_t
     return GS_OK;
 }
 
+constexpr int kStagedMinQueries = 32;     // below this a CTA of 32 warps has idle warps and stages strips nobody reads
+constexpr int kStagedChunk = 512;         // queries per CTA of the staged kernel
+
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    (void)ix; (void)nq; (void)use_head;
+    if (group <= 0 && nq >= kStagedMinQueries && use_head && ix->H > 0) return kWarpsStaged;
     return norm_warps(group);
 }
 
@@ -262,10 +369,22 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     int dev = 0, smem_max = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const size_t wbytes = ix->wtype == GS_W_F32 ? 4 : 1;
+    const size_t smem_staged = (size_t)kWarpsStaged * ix->Ts * 4 + (size_t)p.H * ix->Ts * wbytes;
+    // query_group > 0 pins the small-batch kernel (that many cell rows per CTA)
+    if (group <= 0 && nq >= kStagedMinQueries && p.H > 0 && smem_staged <= (size_t)smem_max) {
+        p.chunk = kStagedChunk;
+        p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
+        const int64_t grid = (int64_t)ts.count * p.n_chunks;
+        if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+        return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, smem_staged, true, s)
+                                     : launch<GS_W_U8>(p, (unsigned)grid, smem_staged, true, s);
+    }
     while (p.warps > 1 && (size_t)p.warps * ix->Ts * 4 > (size_t)smem_max) p.warps >>= 1;
     const size_t smem = (size_t)p.warps * ix->Ts * 4;
     if (smem > (size_t)smem_max) return GS_ERR_OOM;                 // one accumulator row does not fit: tile_docs too large
     const int64_t grid = ((int64_t)ts.count * nq + p.warps - 1) / p.warps;
     if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-    return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, smem, s) : launch<GS_W_U8>(p, (unsigned)grid, smem, s);
+    return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, smem, false, s)
+                                 : launch<GS_W_U8>(p, (unsigned)grid, smem, false, s);
 }
