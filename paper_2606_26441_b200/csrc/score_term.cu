@@ -37,6 +37,7 @@ template <> struct Num<GS_W_F32> {
     static __device__ __forceinline__ A mac(A acc, A q, A w) { return fmaf(q, w, acc); }
     static __device__ __forceinline__ A widen(W w) { return w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return __float_as_uint(a); }
+    static __device__ __forceinline__ A lowest() { return __uint_as_float(0xFF800000u); }      // -inf
 };
 template <> struct Num<GS_W_U8> {
     using W = uint8_t;
@@ -46,6 +47,7 @@ template <> struct Num<GS_W_U8> {
     static __device__ __forceinline__ A mac(A acc, A q, A w) { return acc + q * w; }
     static __device__ __forceinline__ A widen(W w) { return (int32_t)w; }
     static __device__ __forceinline__ uint32_t bits(A a) { return (uint32_t)a; }
+    static __device__ __forceinline__ A lowest() { return (int32_t)0x80000000; }
 };
 
 struct TermParams {
@@ -189,21 +191,22 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
     const size_t strip_ld = STAGED ? (size_t)Ts : (size_t)p.N_pad;
     const bool filter = p.sink.thr != nullptr;
     const uint64_t thr = filter ? p.sink.thr[b] : 0ull;
-    // score of the threshold key: a cell above it passes, a cell equal to it is decided by the full key (doc id)
-    const A thr_s = Num<WT>::from_bits((int)(WT == GS_W_F32 ? gs_unord_f32((uint32_t)(thr >> 32)) : ((uint32_t)(thr >> 32) ^ 0x80000000u)));
-    const bool accept_all = thr == 0ull;
-    auto passes = [&](A sc, int64_t doc) -> bool {
-        if (doc >= p.N) return false;
-        if (accept_all || sc > thr_s) return true;
-        return sc == thr_s && gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc)), (uint32_t)doc) >= thr;
-    };
-    uint32_t n_pass = 0;
+    // Score and doc id of the threshold key: key >= threshold key  <=>  score > its score, or equal and doc id <= its doc
+    // id (two or three compares per cell instead of building the 64-bit key).  Threshold key 0 = accept everything.
+    const A thr_s = thr == 0ull ? Num<WT>::lowest()
+                                : Num<WT>::from_bits((int)(WT == GS_W_F32 ? gs_unord_f32((uint32_t)(thr >> 32))
+                                                                          : ((uint32_t)(thr >> 32) ^ 0x80000000u)));
+    const int n_live = (int)min((int64_t)Ts, p.N - (int64_t)base);      // documents of this tile that exist
+    const int64_t thr_cell = (int64_t)(0xFFFFFFFFu - (uint32_t)thr) - (int64_t)base;   // threshold doc as a cell of this tile
+    const int tie_cells = (int)max((int64_t)-1, min((int64_t)Ts, thr_cell));           // cells <= this index win a score tie
+    uint64_t* cand = filter ? p.sink.cand + b * p.sink.cand_cap : nullptr;
     for (int dq0 = 0; dq0 < quads; dq0 += 32 * kQuadRounds) {
+        const bool whole = dq0 + 32 * kQuadRounds <= quads;             // uniform: no quad of this chunk is out of range
         A sc[kQuadRounds][4];
 #pragma unroll
         for (int r = 0; r < kQuadRounds; ++r) {
             const int dq = dq0 + 32 * r + lane;
-            const int4 a4 = dq < quads ? reinterpret_cast<const int4*>(row)[dq] : make_int4(0, 0, 0, 0);
+            const int4 a4 = (whole || dq < quads) ? reinterpret_cast<const int4*>(row)[dq] : make_int4(0, 0, 0, 0);
             sc[r][0] = Num<WT>::from_bits(a4.x); sc[r][1] = Num<WT>::from_bits(a4.y);
             sc[r][2] = Num<WT>::from_bits(a4.z); sc[r][3] = Num<WT>::from_bits(a4.w);
         }
@@ -214,7 +217,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
             int4 v[kQuadRounds];
 #pragma unroll
             for (int r = 0; r < kQuadRounds; ++r) {
-                if (dq0 + 32 * r + lane < quads) {
+                if (whole || dq0 + 32 * r + lane < quads) {
                     if (WT == GS_W_F32) {
                         v[r] = STAGED ? *reinterpret_cast<const int4*>(src + 128 * r) : __ldg(reinterpret_cast<const int4*>(src + 128 * r));
                     } else {
@@ -234,46 +237,47 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                 sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
             }
         }
+        if (!filter) {
+#pragma unroll
+            for (int r = 0; r < kQuadRounds; ++r) {
+                const int dq = dq0 + 32 * r + lane;
+                if (whole || dq < quads) store_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, sc[r][0], sc[r][1], sc[r][2], sc[r][3]);
+            }
+            continue;
+        }
+        // filter: bit (4r + u) of `mask` = cell u of the lane's quad in round r passes; the finished scores go back to the row
+        uint32_t mask = 0;
 #pragma unroll
         for (int r = 0; r < kQuadRounds; ++r) {
             const int dq = dq0 + 32 * r + lane;
-            if (dq < quads) {
-                const int64_t doc0 = (int64_t)base + 4 * dq;
-                if (!filter) {
-                    store_quad<WT>(p, b, j, dq, doc0, sc[r][0], sc[r][1], sc[r][2], sc[r][3]);
-                } else {
-                    reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(sc[r][0]), Num<WT>::bits(sc[r][1]),
-                                                                   Num<WT>::bits(sc[r][2]), Num<WT>::bits(sc[r][3]));
-                    n_pass += (uint32_t)passes(sc[r][0], doc0) + (uint32_t)passes(sc[r][1], doc0 + 1) +
-                              (uint32_t)passes(sc[r][2], doc0 + 2) + (uint32_t)passes(sc[r][3], doc0 + 3);
-                }
+            if (whole || dq < quads) {
+                reinterpret_cast<uint4*>(row)[dq] = make_uint4(Num<WT>::bits(sc[r][0]), Num<WT>::bits(sc[r][1]),
+                                                               Num<WT>::bits(sc[r][2]), Num<WT>::bits(sc[r][3]));
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if ((sc[r][u] > thr_s || (sc[r][u] == thr_s && 4 * dq + u <= tie_cells)) && 4 * dq + u < n_live)
+                        mask |= 1u << (4 * r + u);
             }
         }
-    }
-    if (!filter) return;
-    uint32_t incl = n_pass;
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-        if (lane >= o) incl += v;
-    }
-    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    if (total == 0u) return;
-    uint32_t pos = 0;
-    if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b], total);
-    pos = __shfl_sync(0xFFFFFFFFu, pos, 0) + incl - n_pass;
-    if (n_pass == 0u) return;
-    uint64_t* cand = p.sink.cand + b * p.sink.cand_cap;
-    for (int dq = lane; dq < quads; dq += 32) {
-        const int4 a4 = reinterpret_cast<const int4*>(row)[dq];
-        const A sc[4] = {Num<WT>::from_bits(a4.x), Num<WT>::from_bits(a4.y), Num<WT>::from_bits(a4.z), Num<WT>::from_bits(a4.w)};
-        const int64_t doc0 = (int64_t)base + 4 * dq;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (passes(sc[u], doc0 + u)) {
-                if ((int64_t)pos < p.sink.cand_cap)
-                    cand[pos] = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc[u])), (uint32_t)(doc0 + u));
-                ++pos;
-            }
+        if (__ballot_sync(0xFFFFFFFFu, mask != 0u) == 0u) continue;     // no candidate in this chunk (the common case)
+        // the warp reserves its slice of the query's candidate list with ONE atomic
+        const uint32_t mine = (uint32_t)__popc(mask);
+        uint32_t incl = mine;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        uint32_t pos = 0;
+        if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b], total);
+        pos = __shfl_sync(0xFFFFFFFFu, pos, 0) + incl - mine;
+        while (mask) {
+            const int bit = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const int cell = 4 * (dq0 + 32 * (bit >> 2) + lane) + (bit & 3);
+            if ((int64_t)pos < p.sink.cand_cap)
+                cand[pos] = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(row[cell])), (uint32_t)(base + cell));
+            ++pos;
         }
     }
 }
