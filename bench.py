@@ -451,10 +451,21 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
                     "strips_used_per_pass_mean": float(np.mean(sp)) if sp else 0.0, "bytes_one_pass": one,
                     "frac_one_pass": rf.effective_gbps(one, kms) / peaks["hbm_gbs"]})
     else:
-        alg = rf.term_parallel_bytes(ts["U"], wtype, share)
-        out.update({"query_group": st["query_group"], "bytes_per_step": alg,
-                    "bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
-                    "bytes_paper_model": rf.term_parallel_bytes(ts["W"], wtype)})
+        # not HBM bound by construction: the roof is the shared-memory pipeline.  HBM figures kept beside it.
+        hbm = rf.term_parallel_bytes(ts["U"], wtype, share)
+        ht = rf.head_tail_work(lens, queries.terms, head_terms)
+        alg = rf.term_parallel_smem_bytes(ht["W_head"], ht["W_tail"], info["num_tiles"] * B, info["tile_docs"], share)
+        peak = rf.smem_peak_gbs(peaks["sm_max_mhz"])
+        out.update({"bound": "alu", "peak": peak,
+                    "peak_source": f"derived: 148 SMs x 128 B/clk shared memory x {peaks['sm_max_mhz']:.0f} MHz (B200_PROFILING.md unit counts and clocks)",
+                    "cell_rows_per_cta": st["query_group"], "bytes_per_step": alg, "W_head": ht["W_head"], "W_tail": ht["W_tail"],
+                    "bytes_model": "shared-memory traffic: (4*W_head + 8*W_tail + 8*Ts*tiles*B)*(1+sample share)",
+                    "hbm_bytes_per_step": hbm, "hbm_bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
+                    "hbm_achieved": rf.effective_gbps(hbm, kms), "hbm_frac": rf.effective_gbps(hbm, kms) / peaks["hbm_gbs"],
+                    "hbm_bytes_paper_model": rf.term_parallel_bytes(ts["W"], wtype)})
+        out["achieved"] = rf.effective_gbps(alg, kms)
+        out["frac"] = out["achieved"] / peak
+        return out
     out["achieved"] = rf.effective_gbps(alg, kms)
     out["frac"] = out["achieved"] / peaks["hbm_gbs"]
     return out

@@ -94,3 +94,34 @@ def doc_parallel_bytes(N: int, P_tail: int, wtype: str, B: int, query_tile: int,
 
 def term_parallel_bytes(U: int, wtype: str, sample_share: float = 0.0) -> float:
     return (4 + weight_bytes(wtype)) * U * (1.0 + sample_share)
+
+
+# ---- term-parallel kernel: the shared-memory roof ----------------------------------------------------
+# The term-parallel kernel is not HBM bound by construction (it reads each posting of the batch's terms from
+# HBM/L2 and then does one shared-memory access or read-modify-write per multiply-add): its roof is the
+# shared-memory pipeline.  SM counts and clocks: /opt/skills/guides/B200_PROFILING.md (148 SMs, 1965 MHz);
+# 32 banks x 4 bytes per SM per clock is the architectural shared-memory width.
+B200_SMS = 148
+SMEM_BYTES_PER_CLK_PER_SM = 128
+
+
+def smem_peak_gbs(sm_mhz: float = 1965.0, sms: int = B200_SMS) -> float:
+    """Shared-memory bandwidth of the chip in GB/s: SMs x 128 B/clk x clock (37 226 GB/s at 1965 MHz)."""
+    return sms * SMEM_BYTES_PER_CLK_PER_SM * sm_mhz * 1e6 / 1e9
+
+
+def head_tail_work(list_lengths: np.ndarray, query_terms: np.ndarray, head_terms: np.ndarray) -> dict:
+    """Useful multiply-adds of a batch split into head (dense-strip) terms and tail (scattered) terms."""
+    L = np.asarray(list_lengths, dtype=np.int64)
+    t = np.asarray(query_terms)
+    t = t[(t >= 0) & (t < L.shape[0])]
+    is_head = np.zeros(L.shape[0], dtype=bool)
+    is_head[np.asarray(head_terms, dtype=np.int64)] = True
+    return {"W_head": int(L[t[is_head[t]]].sum()), "W_tail": int(L[t[~is_head[t]]].sum())}
+
+
+def term_parallel_smem_bytes(W_head: int, W_tail: int, cell_rows: int, tile_docs: int, sample_share: float = 0.0) -> float:
+    """Algorithmic shared-memory traffic of the term-parallel kernel per batch:
+    4 B per head multiply-add (the strip value read from the staged strip), 8 B per tail multiply-add (accumulator
+    read + write), and per (doc tile, query) cell row 4*Ts to zero it and 4*Ts to read it back."""
+    return (4.0 * W_head + 8.0 * W_tail + 8.0 * cell_rows * tile_docs) * (1.0 + sample_share)

@@ -4,6 +4,7 @@ import json
 import os
 
 import numpy as np
+import pytest
 
 from paper_2606_26441_b200 import roofline as rf
 
@@ -49,3 +50,14 @@ def test_our_models_closed_forms():
     terms = np.array([5, 1, 9, 1, 2, 7], np.int32)
     assert rf.strips_per_pass(indptr, terms, np.array([1, 2, 3]), query_tile=2) == [1, 2]
     assert rf.doc_parallel_bytes(3, 5, "f32", B=3, query_tile=2, strips_by_pass=[1, 2]) == (16 + 40 + 12) + (16 + 40 + 24)
+
+
+def test_term_parallel_shared_memory_roof():
+    assert rf.smem_peak_gbs(1965.0) == pytest.approx(148 * 128 * 1.965e9 / 1e9)
+    L = np.array([10, 0, 7, 3], np.int64)
+    q_terms = np.array([0, 2, 2, 3, 9, -1], np.int32)
+    ht = rf.head_tail_work(L, q_terms, np.array([0, 3]))
+    assert ht == {"W_head": 13, "W_tail": 14}                    # head: terms 0 and 3 once each; tail: term 2 twice
+    assert ht["W_head"] + ht["W_tail"] == rf.batch_term_stats(L, q_terms)["W"]
+    assert rf.term_parallel_smem_bytes(13, 14, cell_rows=6, tile_docs=512) == 4 * 13 + 8 * 14 + 8 * 6 * 512
+    assert rf.term_parallel_smem_bytes(13, 14, 6, 512, sample_share=0.5) == 1.5 * (4 * 13 + 8 * 14 + 8 * 6 * 512)
