@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--also", default="term,doc", help="extra algos timed after the main one ('' = none)")
     ap.add_argument("--doc-query-tile", type=int, default=0)
     ap.add_argument("--query-group", type=int, default=0)
+    ap.add_argument("--sample-shift", type=int, default=0, help="threshold sample = 1/2^shift of the doc tiles (0 = auto)")
     ap.add_argument("--tile-docs", type=int, default=0)
     ap.add_argument("--head-max", type=int, default=0, help="dense strips kept by the index (0 = default 64, -1 = none)")
     ap.add_argument("--head-density", type=float, default=0.0, help="list density from which a strip is kept (0 = default)")
@@ -272,7 +273,7 @@ def run_ours(args):
     sdt = torch.float32 if c["wtype"] == "f32" else torch.int32
     out_ids = torch.empty((B, k), dtype=torch.int32, device=dev)
     out_sc = torch.empty((B, k), dtype=sdt, device=dev)
-    opt_common = dict(doc_query_tile=args.doc_query_tile, query_group=args.query_group)
+    opt_common = dict(doc_query_tile=args.doc_query_tile, query_group=args.query_group, sample_shift=args.sample_shift)
 
     def measure(algo):
         ws_bytes = ix.workspace_bytes(B, queries.nnz, k, algo=algo, **opt_common)
@@ -419,6 +420,19 @@ def suite_entry(torch, gs, wl, name, args, peaks):
     return res
 
 
+def measured_traffic(kernel: str, info, B: int):
+    """DRAM bytes per launch of a scoring kernel from the committed ncu capture (profiles/traffic.csv), for the headline
+    workload only (8.8M docs, B=500); None otherwise."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if info["num_docs"] != 8_800_000 or B != 500 or not os.path.exists(path):
+        return None
+    for r in csv.DictReader(open(path)):
+        if r["kernel"] == kernel and r["workload"] == "paper":
+            return {"bytes_per_launch": int(r["dram_bytes_per_launch"]), "launch": r["launch"], "source": r["source"]}
+    return None
+
+
 def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
     """Roofline of the dominant scoring kernel of the step (SURVEY §8d byte models).
 
@@ -439,8 +453,9 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
     ntiles = max(info["num_tiles"], 1)
     share = st["sample_tiles"] / ntiles if st["sample_tiles"] < ntiles else 0.0
     ts = rf.batch_term_stats(lens, queries.terms)
+    tr = measured_traffic(name, info, B) if wtype == "f32" else None
     out = {"kernel": name, "kernel_ms_per_step": kms, "launches_per_step": nl, "share_of_step": kms / res["ms_per_step"],
-           "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": None,
+           "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": tr["bytes_per_launch"] if tr else None, "traffic_detail": tr,
            "useful_mac_per_step": ts["W"], "mac_per_s": ts["W"] / (kms * 1e-3)}
     if name == "score_doc":
         sp = rf.strips_per_pass(queries.indptr, queries.terms, head_terms, st["doc_query_tile"])

@@ -149,14 +149,15 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
     if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : 16;   // doc-parallel: queries per pass; 16 is the largest tile that stays HBM bound
     p.use_head = !(p.flags & GS_FLAG_NO_HEAD_STRIPS);
     // Threshold sample = 1/2^shift of the doc tiles.  The select phases read the sample (N/2^shift cells per query) and
-    // the candidates (about k*2^shift per query): for a few queries, where they are what a search spends its time on,
-    // balance the two (2^shift ~ sqrt(N/k)); large batches keep 1/32 (candidate lists of 8*k*32 keys per query).
+    // the candidates (about k*2^shift per query), so the balance is 2^shift ~ sqrt(N/k); the candidate lists
+    // (8*k*2^shift keys per query) are kept under 2 GiB for the batch, and never below the 1/32 sample.
     int shift = 5;
     if (o && o->sample_shift > 0) {
         shift = o->sample_shift;
-    } else if (B <= 16 && ix->N > 0) {
+    } else if (ix->N > 0) {
         const double r = std::sqrt((double)ix->N / (double)k);
         while (shift < 10 && (double)(1 << (shift + 1)) <= r * 1.4142) ++shift;
+        while (shift > 5 && (double)B * 8.0 * (double)k * (double)(1 << shift) * 8.0 > 2147483648.0) --shift;
     }
     // the sample must hold comfortably more than k documents, else its k-th key is a weak bound
     while (shift > 0 && ((int64_t)(ix->ntiles >> shift)) * ix->Ts < 4 * (int64_t)k) --shift;
