@@ -342,6 +342,25 @@ def run_ours(args):
     if world == 1 and args.latency_queries > 0:
         latency = {a: latency_leg(torch, ix, queries, k, args.latency_queries, a) for a in ("term", "doc")}
 
+    # ---- batch-size sweep on the same index (Table 3 L262-271 analogue), with --suite
+    sweep = None
+    if world == 1 and args.suite:
+        sweep = []
+        for Bs in (1, 2, 4, 8, 16, 32, 64, 128, 256, B):
+            if Bs > B:
+                continue
+            qb_ = queries.slice_rows(0, Bs)
+            qd_ = [torch.from_numpy(a).to(dev) for a in (qb_.indptr, qb_.terms, qb_.weights)]
+            row = {"batch": Bs}
+            for a in ("term", "doc"):
+                ws_ = torch.empty(ix.workspace_bytes(Bs, qb_.nnz, k, algo=a), dtype=torch.uint8, device=dev)
+                oi = torch.empty((Bs, k), dtype=torch.int32, device=dev)
+                osc = torch.empty((Bs, k), dtype=sdt, device=dev)
+                ms_ = timed_steps(torch, None, lambda: ix.search(*qd_, k, out_ids=oi, out_scores=osc, workspace=ws_, algo=a), 5, 3, 1)
+                row[a] = {"ms_per_batch": ms_ / 5, "qps": Bs * 5 / (ms_ * 1e-3)}
+                del ws_
+            sweep.append(row)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         full, _ = time_oracle(docs, queries, wl.VOCAB, k, args.cpu_sample_queries)
@@ -352,7 +371,7 @@ def run_ours(args):
                 "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32" if c["wtype"] == "f32" else "u8", "data": "synthetic",
                 "config": config_dict(args, c, n_docs, B, k, f"{args.algo}->{main['algo_used']}"),
-                "ms_per_query": main["ms_per_query"], "clocks": main["clocks"], "e2e": e2e, "latency_b1": latency,
+                "ms_per_query": main["ms_per_query"], "clocks": main["clocks"], "e2e": e2e, "latency_b1": latency, "batch_sweep": sweep,
                 "gpu_launches": int(main["launches_per_step"] * args.steps), "roofline": main["roofline"],
                 "cpu_baseline": cpu, "kernels": main["kernels"], "candidates_per_query": main["candidates_per_query"],
                 "overflow_queries": main["overflow_queries"], "other_algos": others,
@@ -361,6 +380,10 @@ def run_ours(args):
                           "bytes_meta": info["bytes_inverted_meta"], "head_terms": info["head_terms"], "head_terms_term_parallel": info["head_terms_term_parallel"],
                           "forward_tail_postings": info["forward_tail_nnz"], "forward_padded_postings": info["forward_padded_nnz"], "tile_docs": info["tile_docs"],
                           "build_s": t_build, "generate_s": t_gen},
+                "data_checksums": {"docs_indptr": f"{wl.checksum(docs.indptr):016x}", "docs_terms": f"{wl.checksum(docs.terms):016x}",
+                                   "docs_weights": f"{wl.checksum(docs.weights):016x}", "query_terms": f"{wl.checksum(queries.terms):016x}",
+                                   "query_weights": f"{wl.checksum(queries.weights):016x}",
+                                   "note": "64-bit checksums of the generated arrays (workload.checksum): same seed -> same inputs on every box"},
                 "context": {"paper_h100_qps": 787, "paper_h100_doc_parallel_hbm_frac": 0.626,
                             "note": "paper numbers are H100 + MS MARCO/SPLADE (PAPER.md L292, L340): context, not a baseline"}}
     ix.close()
@@ -483,6 +506,9 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
         return out
     out["achieved"] = rf.effective_gbps(alg, kms)
     out["frac"] = out["achieved"] / peaks["hbm_gbs"]
+    # context: the nominal HBM3e figure of B200_PROFILING.md (7.7 TB/s, HGX); the fraction that counts is of the measured peak
+    out["peak_nominal"] = 7700.0
+    out["frac_of_nominal"] = out["achieved"] / 7700.0
     return out
 
 
