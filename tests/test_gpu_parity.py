@@ -423,6 +423,31 @@ def test_mid_prefix_full_compare(gs, mode, algo):
     ix.close()
 
 
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+@pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=5), dict(head_max=-1), dict(tile_docs=1024, head_density=0.05)])
+def test_batch_of_80_takes_the_staged_term_kernel(gs, mode, build_kw):
+    """From 64 queries on the term-parallel kernel runs as a persistent CTA per doc tile with the strips staged in shared
+    memory (unless the index has no strips): every score of 80 queries x 20 011 docs, and the top-50, against the oracle."""
+    docs = wl.make_docs("mid", n_docs=20_011)
+    queries = wl.make_queries("mid", n_queries=80)
+    if mode == "u8":
+        docs, queries = docs.to_u8(), queries.to_u8()
+    ix = gs.Index.from_numpy(docs, wl.VOCAB, **build_kw)
+    S = ix.score_dense(*dev(queries), algo="term").cpu().numpy()[:, :docs.rows]
+    R_d, R_q = oracle.as_rows(docs, wl.VOCAB), oracle.as_rows(queries, wl.VOCAB)
+    _, _, A = oracle.search(R_q, R_d, 1, all_scores=True)
+    if mode == "u8":
+        assert np.array_equal(S.astype(np.int64), A.astype(np.int64))
+    else:
+        assert np.all(np.abs(S.astype(np.float64) - A) <= parity.tol(A))
+    st_expect = 32 if build_kw.get("head_max", 0) != -1 else 2            # cell rows per CTA: staged shape or small shape
+    for opt in (dict(algo="term"), dict(algo="auto"), dict(algo="term", flags=gs.GS_FLAG_FORCE_DENSE_TOPK)):
+        ids, sc = gpu_search(gs, ix, queries, 50, **opt)
+        assert ix.stats()["query_group"] == st_expect and ix.stats()["algo_used"] == 1
+        compare(gs, docs, queries, wl.VOCAB, 50, ids, sc)
+    ix.close()
+
+
 # ----------------------------------------------------------------------------------------------------
 # paper scale (BASELINE.json configs[2] and [3]) in the launch configuration bench.py times
 # ----------------------------------------------------------------------------------------------------
