@@ -202,6 +202,7 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
     c.qb.tail_term = (int32_t*)take((size_t)nnz * 4);
     c.qb.tail_w = (uint32_t*)take((size_t)nnz * 4);
     c.qb.tail_cnt = (int32_t*)take((size_t)B * 4);
+    c.qb.tail32 = (uint2*)take((size_t)B * GS_TAIL32 * 8);
     c.thr = (uint64_t*)take((size_t)B * 8);
     c.cand_cnt = (uint32_t*)take((size_t)B * 4);
     c.overflow_list = (int32_t*)take((size_t)B * 4);
@@ -380,7 +381,7 @@ void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
     void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
-                    ix->seg, ix->head_slot, ix->head_strip, ix->host_ws, ix->host_stage};
+                    ix->seg, ix->seg2, ix->head_slot, ix->head_strip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
 }

@@ -10,6 +10,7 @@
 #define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
 #define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings
+#define GS_TAIL32 32            // tail terms of a query kept in the fixed-stride prefetch table
 #define GS_SEL_BINS 2048        // radix-select digit: 11 bits
 #define GS_SEL_BITS 11
 
@@ -57,6 +58,7 @@ struct gs_index {
     void* inv_w = nullptr;           // [P_pad] float | uint8, 0 in the padding
     // per-(term, tile) segment table: seg[t*(ntiles+1)+j] = number of postings of t with doc < j*Ts
     uint32_t* seg = nullptr;         // [V][ntiles+1]
+    uint2* seg2 = nullptr;           // [V][ntiles] (first slot, end slot) of term t inside tile j, absolute (P_pad < 2^32 only)
     // dense strips of the densest lists ("head" terms)
     int32_t H = 0;                   // strips (<= GS_STRIP_MAX), densest list first
     int32_t head_terms_host[GS_STRIP_MAX];
@@ -109,6 +111,8 @@ struct gs_qbatch {
     int32_t* tail_term = nullptr;      // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]
     uint32_t* tail_w = nullptr;        // [nnz] accumulator-typed
     int32_t* tail_cnt = nullptr;       // [B]
+    uint2* tail32 = nullptr;           // [B][32] the first 32 tail terms as (term id or -1, weight bits): a fixed-stride
+                                       // copy the batch kernel can prefetch without reading indptr first
     int32_t* status = nullptr;         // device status word: first validation error (gs_status_t) or 0
 };
 

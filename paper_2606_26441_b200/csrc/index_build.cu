@@ -124,6 +124,19 @@ __global__ void k_segments(const int64_t* __restrict__ inv_off, const int32_t* _
         for (int32_t j = tile_cur + 1; j <= ntiles; ++j) row[j] = (uint32_t)len;
 }
 
+// Pair form of the segment table for the batch kernel: seg2[t][j] = (first slot, one past the last slot) of the postings
+// of term t inside doc tile j, as absolute posting slots (needs P_pad < 2^32): one aligned 64-bit load per probe
+// instead of two table loads and a list-offset load.
+__global__ void k_segment_pairs(const int64_t* __restrict__ inv_off, const uint32_t* __restrict__ seg, int32_t V,
+                                int32_t ntiles, uint2* __restrict__ seg2) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= (int64_t)V * ntiles) return;
+    const int32_t t = (int32_t)(i / ntiles), j = (int32_t)(i - (int64_t)t * ntiles);
+    const uint32_t off = (uint32_t)inv_off[t];
+    const uint32_t* row = seg + (size_t)t * (ntiles + 1);
+    seg2[i] = make_uint2(off + row[j], off + row[j + 1]);
+}
+
 template <typename W>
 __global__ void k_fill_strip(const int32_t* __restrict__ inv_doc, const W* __restrict__ inv_w, int64_t off, int32_t len,
                              W* __restrict__ strip) {
@@ -393,6 +406,14 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         GS_CUDA(cudaStreamSynchronize(s));
         GS_CUDA(cudaGetLastError());
         if (h_err && o.validate) return (gs_status_t)h_err;
+    }
+    if (ix->P_pad < (int64_t)0xFFFFFFFFLL && ix->ntiles > 0) {
+        const size_t pair_elems = (size_t)V * (size_t)ix->ntiles;
+        ix->seg2 = (uint2*)gs_dev_alloc(ix, sizeof(uint2) * pair_elems, s);
+        if (!ix->seg2) return GS_ERR_OOM;
+        k_segment_pairs<<<grid_for((int64_t)pair_elems), kThreads, 0, s>>>(ix->inv_off, ix->seg, V, ix->ntiles, ix->seg2);
+        GS_CUDA(cudaGetLastError());
+        ix->bytes_meta += (int64_t)(sizeof(uint2) * pair_elems);
     }
 
     // ---- dense strips of the head lists

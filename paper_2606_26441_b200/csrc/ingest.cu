@@ -16,12 +16,15 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
                          const void* __restrict__ weights, int64_t B, int32_t V, const int16_t* __restrict__ head_slot,
                          int h_term, int validate, uint2* __restrict__ head_pair, int32_t* __restrict__ head_cnt,
                          int32_t* __restrict__ tail_term,
-                         uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, int32_t* __restrict__ status) {
+                         uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, uint2* __restrict__ tail32,
+                         int32_t* __restrict__ status) {
     const int lane = threadIdx.x & 31;
     const int64_t b = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     if (b >= B) return;
     const int64_t a = indptr[b], e = indptr[b + 1];
     int32_t n_tail = 0, n_head = 0;
+    tail32[b * GS_TAIL32 + lane] = make_uint2(0xFFFFFFFFu, 0u);
+    __syncwarp();
     for (int64_t i0 = a; i0 < e; i0 += 32) {
         const int64_t i = i0 + lane;
         int32_t t = -1;
@@ -60,6 +63,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
             const int64_t dst = a + n_tail + __popc(m & ((1u << lane) - 1u));
             tail_term[dst] = t;
             tail_w[dst] = w;
+            if (dst - a < GS_TAIL32) tail32[b * GS_TAIL32 + (dst - a)] = make_uint2((uint32_t)t, w);
         }
         n_tail += __popc(m);
         __syncwarp();
@@ -80,11 +84,11 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
                                                    use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
-                                                   qb->tail_w, qb->tail_cnt, qb->status);
+                                                   qb->tail_w, qb->tail_cnt, qb->tail32, qb->status);
     else
         k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
                                                   use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
-                                                  qb->tail_w, qb->tail_cnt, qb->status);
+                                                  qb->tail_w, qb->tail_cnt, qb->tail32, qb->status);
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;

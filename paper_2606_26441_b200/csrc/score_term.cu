@@ -52,11 +52,11 @@ template <> struct Num<GS_W_U8> {
 
 struct TermParams {
     // index
-    const int64_t* inv_off; const int32_t* inv_doc; const void* inv_w; const uint32_t* seg;
+    const int64_t* inv_off; const int32_t* inv_doc; const void* inv_w; const uint32_t* seg; const uint2* seg2;
     const void* head_strip; int32_t H; int64_t N; int64_t N_pad; int32_t Ts; int32_t ntiles;
     // queries
     const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
-    const uint32_t* tail_w; const int32_t* tail_cnt;
+    const uint32_t* tail_w; const int32_t* tail_cnt; const uint2* tail32;
     int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
     int32_t warps;                              // cell rows (warps) per CTA (small-batch kernel)
     int32_t chunk, n_chunks;                    // staged kernel: queries per CTA, CTAs per doc tile
@@ -329,6 +329,339 @@ __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(cons
         process_item<WT, true>(p, rows + (size_t)warp * Ts, s_strip, j, p.q0 + q, lane);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Batch kernel (Ts == 512, >= kStagedMinQueries queries, < 2^32 posting slots): same ownership as above — a persistent
+// CTA per doc tile stages the tile's strips once, a warp owns one (query, tile) cell row at a time — with the three
+// per-row phases rebuilt around what the ncu source view of the staged kernel showed (profiles/r01d_term_kernel.md:
+// the tail scatter, 8 % of the multiply-adds, took half of the instructions and 57 % of the stall samples):
+//   * tail: the row's non-empty segments are FLATTENED into one posting stream.  An exclusive scan of the segment
+//     lengths gives every segment its start in the stream; in a round of 32 flat postings a lane finds its segment
+//     with one warp OR-reduction (bit i = "a segment starts at flat position f0+i") and a popcount, fetches
+//     (segment start - stream start, query weight) from a 32-entry per-warp table in shared memory, and loads its
+//     posting: every lane is busy, and the loads of kRounds rounds are in flight together.  The read-modify-writes
+//     of a round are issued segment by segment (two lists may hit the same document; one list never does), so the
+//     order of the additions into a cell is the query's term order: deterministic, no atomics;
+//   * the probes (query terms -> segment table -> list offsets) of the NEXT TWO queries of the warp are prefetched
+//     (two-stage software pipeline) from the fixed-stride tail32 table;
+//   * head: a lane keeps its 16 documents in registers, one 128-bit shared-memory load feeds two FFMA2;
+//   * filter: one max over the lane's 16 scores and one ballot reject a row chunk that holds no candidate (the common
+//     case) before any per-cell test or write-back.
+// ------------------------------------------------------------------------------------------------
+constexpr int kBT = 512;          // documents per tile
+#ifndef GS_BWARPS
+#define GS_BWARPS 32
+#endif
+#ifndef GS_ROUNDS
+#define GS_ROUNDS 2
+#endif
+#ifndef GS_HEAD_UNROLL
+#define GS_HEAD_UNROLL 2
+#endif
+constexpr int kBWarps = GS_BWARPS;   // warps (cell rows in flight) per CTA
+constexpr int kRounds = GS_ROUNDS;   // flat posting rounds whose loads are issued together
+constexpr int kHeadUnroll = GS_HEAD_UNROLL;
+
+__device__ __forceinline__ unsigned long long pack_f32x2(float lo, float hi) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack_f32x2(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+// (a.lo * b.lo + c.lo, a.hi * b.hi + c.hi): one FFMA2, each half an IEEE fp32 fma (same result as two fmaf)
+__device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+template <int WT> __device__ __forceinline__ typename Num<WT>::A num_max(typename Num<WT>::A a, typename Num<WT>::A b);
+template <> __device__ __forceinline__ float num_max<GS_W_F32>(float a, float b) { return fmaxf(a, b); }
+template <> __device__ __forceinline__ int32_t num_max<GS_W_U8>(int32_t a, int32_t b) { return max(a, b); }
+
+struct Probe1 { uint32_t t, wq; };                                    // query terms (first 32 tail terms, one per lane)
+struct Probe2 { uint32_t lo, hi, wq; int32_t cnt_nh; uint64_t thr; };   // + the terms' segments inside the tile, and
+                                                                           // tail count | head count << 16, threshold key
+
+__device__ __forceinline__ Probe1 probe_terms(const TermParams& p, int64_t b, int lane) {
+    const uint2 e = __ldg(p.tail32 + b * GS_TAIL32 + lane);
+    return Probe1{e.x, e.y};
+}
+__device__ __forceinline__ Probe2 probe_segments(const TermParams& p, const Probe1& a, int tile) {
+    Probe2 r;
+    r.lo = r.hi = 0u;
+    r.wq = a.wq; r.cnt_nh = 0; r.thr = 0ull;
+    if (a.t != 0xFFFFFFFFu) {
+        const uint2 e = __ldg(p.seg2 + (size_t)a.t * p.ntiles + tile);      // (first slot, end slot), absolute
+        r.lo = e.x; r.hi = e.y;
+    }
+    return r;
+}
+__device__ __forceinline__ void probe_query(const TermParams& p, int64_t b, bool filter, Probe2& r) {
+    r.cnt_nh = __ldg(p.tail_cnt + b) | (__ldg(p.head_cnt + b) << 16);
+    r.thr = filter ? __ldg(p.sink.thr + b) : 0ull;
+}
+
+__device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
+    uint2 v;
+    asm("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+
+// Applies up to 32 posting-list segments (lane s: n postings from slot `start`, query weight bits wq) to `row`.
+// `desc_s` = shared-window address of the warp's 32-entry descriptor table.
+template <int WT>
+__device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<WT>::A* row, uint32_t desc_s, int n,
+                                             uint32_t start, uint32_t wq, int32_t base, int lane) {
+    using W = typename Num<WT>::W;
+    using A = typename Num<WT>::A;
+    const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
+    const int32_t* __restrict__ inv_doc = p.inv_doc;
+    int incl = n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int T = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    if (T == 0) return;
+    const int excl = incl - n;
+    const unsigned nz = __ballot_sync(0xFFFFFFFFu, n > 0);
+    const unsigned lt = (1u << lane) - 1u, le = lt | (1u << lane);
+    if (n > 0)
+        asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(desc_s + 8u * (uint32_t)__popc(nz & lt)), "r"(start - (uint32_t)excl), "r"(wq) : "memory");
+    __syncwarp();
+    const int last_sg = __popc(nz) - 1;
+    const int my_start = n > 0 ? excl : -0x40000000;   // flat position where the lane's segment starts (never matches when empty)
+    int c0 = -1;                                   // (segments that start before the current round) - 1
+    for (int f0 = 0; f0 < T; f0 += 32 * kRounds) {
+        int32_t doc[kRounds];
+        W wraw[kRounds];
+        uint32_t qv[kRounds];
+        unsigned sm[kRounds];
+        int ord[kRounds];
+        // loads of up to kRounds rounds, no use of a loaded value in this loop (their latencies overlap); a lane past the
+        // end of the stream re-reads the last posting and is switched off by ord = -1
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const int fr = f0 + 32 * r;
+            if (fr < T) {                           // uniform
+                const uint32_t d = (uint32_t)(my_start - fr);
+                sm[r] = __reduce_or_sync(0xFFFFFFFFu, d < 32u ? (1u << d) : 0u);
+                const int o = __popc(sm[r] & le);
+                const bool valid = fr + lane < T;
+                const int sg = valid ? c0 + o : last_sg;
+                const int f = valid ? fr + lane : T - 1;
+                ord[r] = valid ? o : -1;
+                c0 += __popc(sm[r]);
+                const uint2 de = lds_u2(desc_s + 8u * (uint32_t)sg);
+                const uint32_t idx = de.x + (uint32_t)f;
+                doc[r] = __ldg(inv_doc + idx);
+                wraw[r] = __ldg(inv_w + idx);
+                qv[r] = de.y;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            if (f0 + 32 * r < T) {                  // uniform
+                A* cell = row + (doc[r] - base);
+                const A q = Num<WT>::qw(qv[r]), w = Num<WT>::widen(wraw[r]);
+                const int o_hi = __popc(sm[r]);
+                // segment by segment: two lists may hit the same document, one list never does
+                for (int o = (int)(sm[r] & 1u); o <= o_hi; ++o) {
+                    if (ord[r] == o) *cell = Num<WT>::mac(*cell, q, w);
+                    __syncwarp();
+                }
+            }
+        }
+    }
+}
+
+constexpr int kCandBuf = 2560;   // candidate keys a CTA collects in shared memory before it appends them to the queries' lists
+
+template <int WT>
+__global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const TermParams p) {
+    using W = typename Num<WT>::W;
+    using A = typename Num<WT>::A;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int j = (int)(blockIdx.x / p.n_chunks);
+    const int chunk = (int)(blockIdx.x - (unsigned)j * p.n_chunks);
+    const int tile = p.ts.first + j * p.ts.stride;
+    const int32_t base = tile * kBT;
+    // shared memory: rows [kBWarps][kBT] | descriptors [kBWarps][32] uint2 | candidate keys [kCandBuf] u64 |
+    // candidate queries [kCandBuf] u16 | counter (16 bytes) | strips [H][kBT]
+    constexpr size_t kOffDesc = (size_t)kBWarps * kBT * 4;
+    constexpr size_t kOffKey = kOffDesc + (size_t)kBWarps * 32 * 8;
+    constexpr size_t kOffQ = kOffKey + (size_t)kCandBuf * 8;
+    constexpr size_t kOffCnt = kOffQ + (size_t)kCandBuf * 2;
+    constexpr size_t kOffStrip = kOffCnt + 16;
+    A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
+    const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
+    uint64_t* s_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey);
+    uint16_t* s_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ);
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt);
+    uint32_t* s_next = s_cnt + 1;
+    W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
+    if (threadIdx.x == 0) { *s_cnt = 0u; *s_next = 2u * kBWarps; }
+    {
+        const W* __restrict__ g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * kBT;
+        constexpr int per = kBT / (16 / (int)sizeof(W));
+        for (int i = threadIdx.x; i < p.H * per; i += kBWarps * 32) {
+            const int h = i / per, c = i - h * per;
+            reinterpret_cast<int4*>(s_strip + (size_t)h * kBT)[c] = __ldg(reinterpret_cast<const int4*>(g + (size_t)h * p.N_pad) + c);
+        }
+    }
+    const bool filter = p.sink.thr != nullptr;
+    // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
+    // warp and warp + kBWarps of the chunk and claims further ones from a shared-memory counter, two rows ahead of the
+    // row it works on (the probes of the next two rows are in flight).
+    const int q_end = min(p.nq, (chunk + 1) * p.chunk);
+    int q = chunk * p.chunk + warp;             // row being processed
+    int q_n1 = q + kBWarps;                     // next row (segments probed)
+    int q_n2 = q_end;                           // row after that (terms probed)
+    int q_n3 = q_end;                           // claimed, not yet probed
+    Probe1 s1{0xFFFFFFFFu, 0u};
+    Probe2 s2{0u, 0u, 0u, 0, 0ull};
+    if (q < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile); probe_query(p, p.q0 + q, filter, s2); }
+    if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
+    __syncthreads();
+    {
+        int c = 0;
+        if (lane == 0) c = (int)atomicAdd(s_next, 1u);
+        q_n2 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;
+    }
+    const int n_live = (int)min((int64_t)kBT, p.N - (int64_t)base);                    // documents of this tile that exist
+    const W* srow = s_strip + 4 * lane;
+    for (; q < q_end; q = q_n1, q_n1 = q_n2, q_n2 = q_n3) {
+        const int64_t b = p.q0 + q;
+        const Probe2 cur = s2;
+        if (q_n1 < q_end) { s2 = probe_segments(p, s1, tile); probe_query(p, p.q0 + q_n1, filter, s2); }
+        if (q_n2 < q_end) s1 = probe_terms(p, p.q0 + q_n2, lane);
+        {
+            int c = 0;
+            if (lane == 0) c = (int)atomicAdd(s_next, 1u);
+            q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
+        }
+        const int nh = cur.cnt_nh >> 16, cnt = cur.cnt_nh & 0xFFFF;
+        const uint64_t thr = cur.thr;
+
+#pragma unroll
+        for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
+        __syncwarp();
+        scatter_flat<WT>(p, row, desc_s, (int)(cur.hi - cur.lo), cur.lo, cur.wq, base, lane);
+        if (cnt > GS_TAIL32) {                      // rare: more than 32 tail terms, probed in line
+            const int64_t qa = p.q_indptr[b];
+            for (int i0 = GS_TAIL32; i0 < cnt; i0 += 32) {
+                __syncwarp();                       // the descriptor table is reused
+                Probe1 a{0xFFFFFFFFu, 0u};
+                if (i0 + lane < cnt) { a.t = (uint32_t)p.tail_term[qa + i0 + lane]; a.wq = p.tail_w[qa + i0 + lane]; }
+                const Probe2 e = probe_segments(p, a, tile);
+                scatter_flat<WT>(p, row, desc_s, (int)(e.hi - e.lo), e.lo, e.wq, base, lane);
+            }
+        }
+        __syncwarp();
+
+        // head strips: the lane's 16 documents (quads lane, lane+32, lane+64, lane+96) stay in registers
+        const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
+        A sc[4][4];
+        if constexpr (WT == GS_W_F32) {
+            unsigned long long acc[4][2];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const ulonglong2 a2 = reinterpret_cast<const ulonglong2*>(row)[lane + 32 * r];
+                acc[r][0] = a2.x; acc[r][1] = a2.y;
+            }
+#pragma unroll kHeadUnroll
+            for (int i = 0; i < nh; ++i) {
+                const uint2 e = __ldg(hl + i);
+                const float qf = __uint_as_float(e.y);
+                const unsigned long long q2 = pack_f32x2(qf, qf);
+                const ulonglong2* src = reinterpret_cast<const ulonglong2*>(srow + (size_t)e.x * kBT);
+                ulonglong2 v[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) v[r] = src[32 * r];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    acc[r][0] = fma_f32x2(v[r].x, q2, acc[r][0]);
+                    acc[r][1] = fma_f32x2(v[r].y, q2, acc[r][1]);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                unpack_f32x2(acc[r][0], sc[r][0], sc[r][1]);
+                unpack_f32x2(acc[r][1], sc[r][2], sc[r][3]);
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int4 a4 = reinterpret_cast<const int4*>(row)[lane + 32 * r];
+                sc[r][0] = a4.x; sc[r][1] = a4.y; sc[r][2] = a4.z; sc[r][3] = a4.w;
+            }
+#pragma unroll kHeadUnroll
+            for (int i = 0; i < nh; ++i) {
+                const uint2 e = __ldg(hl + i);
+                const int32_t qi = (int32_t)e.y;
+                const uchar4* src = reinterpret_cast<const uchar4*>(srow + (size_t)e.x * kBT);
+                uchar4 v[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) v[r] = src[32 * r];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    sc[r][0] += qi * (int32_t)v[r].x; sc[r][1] += qi * (int32_t)v[r].y;
+                    sc[r][2] += qi * (int32_t)v[r].z; sc[r][3] += qi * (int32_t)v[r].w;
+                }
+            }
+        }
+
+        if (!filter) {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int dq = lane + 32 * r;
+                store_quad<WT>(p, b, j, dq, (int64_t)base + 4 * dq, sc[r][0], sc[r][1], sc[r][2], sc[r][3]);
+            }
+            continue;
+        }
+        // Score and doc id of the threshold key: key >= threshold key  <=>  score > its score, or equal and doc id <= its
+        // doc id.  Threshold key 0 = accept everything.  A cell that passes goes to the CTA's candidate buffer in shared
+        // memory (one shared-memory atomic per candidate; the global append — an atomic whose result must come back —
+        // happens once per CTA, all entries in flight together); when the buffer is full the cell is appended directly.
+        const A thr_s = thr == 0ull ? Num<WT>::lowest()
+                                    : Num<WT>::from_bits((int)(WT == GS_W_F32 ? gs_unord_f32((uint32_t)(thr >> 32))
+                                                                              : ((uint32_t)(thr >> 32) ^ 0x80000000u)));
+        const int64_t thr_cell = (int64_t)(0xFFFFFFFFu - (uint32_t)thr) - (int64_t)base;   // threshold doc as a cell of this tile
+        const int tie_cells = (int)max((int64_t)-1, min((int64_t)kBT, thr_cell));           // cells <= this index win a score tie
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (sc[r][u] >= thr_s) {                                 // rare (a few cells per row)
+                    const int cell = 4 * (lane + 32 * r) + u;
+                    if (cell < n_live && (sc[r][u] > thr_s || cell <= tie_cells)) {
+                        const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc[r][u])), (uint32_t)(base + cell));
+                        const uint32_t slot = atomicAdd(s_cnt, 1u);
+                        if (slot < (uint32_t)kCandBuf) {
+                            s_key[slot] = key;
+                            s_q[slot] = (uint16_t)(q - chunk * p.chunk);
+                        } else {
+                            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                            if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (!filter) return;
+    __syncthreads();
+    const uint32_t n_buf = min(*s_cnt, (uint32_t)kCandBuf);
+    for (uint32_t i = threadIdx.x; i < n_buf; i += kBWarps * 32) {
+        const int64_t b = p.q0 + (int64_t)chunk * p.chunk + s_q[i];
+        const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+        if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = s_key[i];
+    }
+}
+
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
 template <int WT>
@@ -353,6 +686,8 @@ constexpr int kStagedChunk = 512;         // queries per CTA of the staged kerne
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
+    if (group == 0 && nq >= kStagedMinQueries && use_head && ix->H > 0 && ix->Ts == kBT && ix->seg2 != nullptr)
+        return kBWarps;                                                 // batch kernel
     if (group <= 0 && nq >= kStagedMinQueries && use_head && ix->H > 0) return kWarpsStaged;
     return norm_warps(group);
 }
@@ -361,11 +696,11 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     TermParams p{};
-    p.inv_off = ix->inv_off; p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg = ix->seg;
+    p.inv_off = ix->inv_off; p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg = ix->seg; p.seg2 = ix->seg2;
     p.head_strip = ix->head_strip; p.H = use_head ? ix->H : 0; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
     p.ntiles = ix->ntiles;
     p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_term = qb.tail_term;
-    p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt;
+    p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt; p.tail32 = qb.tail32;
     p.q0 = q0; p.nq = (int32_t)nq;
     p.warps = norm_warps(group);
     p.ts = ts; p.sink = sink;
@@ -375,12 +710,24 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t wbytes = ix->wtype == GS_W_F32 ? 4 : 1;
     const size_t smem_staged = (size_t)kWarpsStaged * ix->Ts * 4 + (size_t)p.H * ix->Ts * wbytes;
-    // query_group > 0 pins the small-batch kernel (that many cell rows per CTA)
+    // query_group > 0 pins the small-batch kernel (that many cell rows per CTA); -1 pins the generic staged kernel
     if (group <= 0 && nq >= kStagedMinQueries && p.H > 0 && smem_staged <= (size_t)smem_max) {
         p.chunk = kStagedChunk;
         p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + 16;
+        if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max) {
+            auto go = [&](auto kern) -> gs_status_t {
+                GS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch));
+                GsProfScope ps(GS_K_SCORE_TERM, s);
+                kern<<<(unsigned)grid, kBWarps * 32, smem_batch, s>>>(p);
+                ++gs_tls_launches;
+                GS_CUDA(cudaGetLastError());
+                return GS_OK;
+            };
+            return ix->wtype == GS_W_F32 ? go(k_score_term_batch<GS_W_F32>) : go(k_score_term_batch<GS_W_U8>);
+        }
         return ix->wtype == GS_W_F32 ? launch<GS_W_F32>(p, (unsigned)grid, smem_staged, true, s)
                                      : launch<GS_W_U8>(p, (unsigned)grid, smem_staged, true, s);
     }

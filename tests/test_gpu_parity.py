@@ -423,6 +423,9 @@ def test_mid_prefix_full_compare(gs, mode, algo):
     ix.close()
 
 
+BATCH_KERNEL_WARPS = 32   # kBWarps of score_term.cu
+
+
 @pytest.mark.parametrize("mode", ["f32", "u8"])
 @pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=5), dict(head_max=-1), dict(tile_docs=1024, head_density=0.05)])
 def test_batch_of_80_takes_the_staged_term_kernel(gs, mode, build_kw):
@@ -440,7 +443,8 @@ def test_batch_of_80_takes_the_staged_term_kernel(gs, mode, build_kw):
         assert np.array_equal(S.astype(np.int64), A.astype(np.int64))
     else:
         assert np.all(np.abs(S.astype(np.float64) - A) <= parity.tol(A))
-    st_expect = 32 if build_kw.get("head_max", 0) != -1 else 2            # cell rows per CTA: staged shape or small shape
+    # cell rows per CTA: batch kernel (512-doc tiles), generic staged shape (other tilings) or small shape (no strips)
+    st_expect = 2 if build_kw.get("head_max", 0) == -1 else (32 if "tile_docs" in build_kw else BATCH_KERNEL_WARPS)
     for opt in (dict(algo="term"), dict(algo="auto"), dict(algo="term", flags=gs.GS_FLAG_FORCE_DENSE_TOPK)):
         ids, sc = gpu_search(gs, ix, queries, 50, **opt)
         assert ix.stats()["query_group"] == st_expect and ix.stats()["algo_used"] == 1
