@@ -36,6 +36,10 @@
 
 #include "gs_internal.cuh"
 
+#ifndef GS_DOC_PF
+#define GS_DOC_PF 2      // chunks of the posting stream in flight per warp
+#endif
+
 namespace {
 
 constexpr uint32_t kTermMask = (1u << GS_FWD_DOC_SHIFT) - 1u;
@@ -303,11 +307,19 @@ __device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ mya
 #pragma unroll
         for (int q = 0; q < QT / 2; ++q)
             asm("mov.b64 %0, {%1, %2};" : "=l"(acc[q]) : "f"(myacc[2 * q]), "f"(myacc[2 * q + 1]));
+        // the strip values of the next group of 4 are loaded before the multiply-adds of the current one
+        float xn[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) xn[u] = sp[(size_t)c_tile.hl[u] * N_pad];
 #pragma unroll 1
         for (int i0 = 0; i0 < nh; i0 += 4) {
             float x[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) x[u] = sp[(size_t)c_tile.hl[i0 + u] * N_pad];
+            for (int u = 0; u < 4; ++u) x[u] = xn[u];
+            if (i0 + 4 < nh) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) xn[u] = sp[(size_t)c_tile.hl[i0 + 4 + u] * N_pad];
+            }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
 #pragma unroll
@@ -446,13 +458,19 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
 
     int64_t sb = (int64_t)blockIdx.x * NW + warp;
     int64_t doc0 = 0, c0 = 0, c1 = 0;              // chunk range of the current block
-    uint4 tc = make_uint4(0, 0, 0, 0), wc = tc;
+    uint4 tc = make_uint4(0, 0, 0, 0), wc = tc;      // chunk c of the current block
+#if GS_DOC_PF >= 2
+    uint4 td = tc, wd = tc;                          // chunk c + 1
+#endif
     if (sb < n_subs) {
         const int64_t blk = block_of(sb, doc0);
         if (blk >= 0) {
             c0 = p.fwd_blk[blk] / GS_FWD_CHUNK;
             c1 = p.fwd_blk[blk + 1] / GS_FWD_CHUNK;
             if (c0 < c1) load_chunk(c0, tc, wc);
+#if GS_DOC_PF >= 2
+            if (c0 + 1 < c1) load_chunk(c0 + 1, td, wd);
+#endif
         } else {
             c0 = c1 = -1;
         }
@@ -466,6 +484,9 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         if (c0 < 0) {                              // block beyond the collection
             doc0 = doc0n; c0 = c0n; c1 = c1n;
             if (c0 >= 0 && c0 < c1) load_chunk(c0, tc, wc);
+#if GS_DOC_PF >= 2
+            if (c0 >= 0 && c0 + 1 < c1) load_chunk(c0 + 1, td, wd);
+#endif
             continue;
         }
         for (int i = lane; i < 32 * AST; i += 32) s_acc[i] = A(0);
@@ -474,7 +495,11 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         int cnt = 0;
         for (int64_t c = c0; c < c1; ++c) {
             uint4 tn = make_uint4(0, 0, 0, 0), wn = tn;
+#if GS_DOC_PF >= 2
+            if (c + 2 < c1) load_chunk(c + 2, tn, wn);                       // prefetch, two chunks ahead
+#else
             if (c + 1 < c1) load_chunk(c + 1, tn, wn);                       // prefetch
+#endif
             if (cnt + GS_FWD_CHUNK > QCAP) { walk(cnt); cnt = 0; }
             const uint32_t tw[4] = {tc.x, tc.y, tc.z, tc.w};
             const uint32_t ww[4] = {wc.x, wc.y, wc.z, wc.w};
@@ -493,11 +518,18 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
                 }
                 cnt += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
+#if GS_DOC_PF >= 2
+            tc = td; wc = wd; td = tn; wd = wn;
+#else
             tc = tn; wc = wn;
+#endif
         }
         walk(cnt);
-        // first chunk of the next block: in flight during the contraction
+        // first chunk(s) of the next block: in flight during the contraction
         if (c0n >= 0 && c0n < c1n) load_chunk(c0n, tc, wc);
+#if GS_DOC_PF >= 2
+        if (c0n >= 0 && c0n + 1 < c1n) load_chunk(c0n + 1, td, wd);
+#endif
 
         // ---- head strips: thread = document, QT accumulators in registers, weights as uniform constant operands
         const int64_t doc = doc0 + lane;
