@@ -4,7 +4,8 @@
 // L146-152).  Here one warp per query splits its terms into
 //   * head terms (the H densest lists, kept as dense strips): compact list head_pair[b][..] of (strip number, weight);
 //   * tail terms: compacted (row b starts at indptr[b]) into tail_term/tail_w, weights converted to the
-//     accumulator type (float, or int32 for uint8 impacts).
+//     accumulator type (float, or int32 for uint8 impacts); the first 32 of them are also written to the
+//     fixed-stride table tail32[b][32] (term id or -1, weight), which the batch kernel prefetches two rows ahead.
 // Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
 // (out of range / duplicate / non-finite) is recorded in a status word the host reads back.
 #include "gs_internal.cuh"

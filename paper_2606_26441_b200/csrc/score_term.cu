@@ -19,9 +19,10 @@
 //   4. hand the finished cells to the sink: dense score matrix, or threshold filter -> candidate
 //      list, where the warp reserves its slice of the list with ONE atomic.
 //
-// An earlier version gave a CTA a group of 64 queries and staged the tile's strips in shared memory;
-// measured on B200 it was slower at every batch size (barrier stalls, idle warps, strips nobody
-// used): DESIGN.md §7.
+// Three kernels share this ownership rule: k_score_term (small batches, a warp per cell row, strips from
+// global memory), k_score_term_staged (batches, any tile size: persistent CTA per doc tile, strips staged in
+// shared memory) and k_score_term_batch (batches, 512-doc tiles: the same CTA shape with the tail walked as one
+// flat posting stream, FFMA2 strips and a shared-memory candidate buffer — see its own comment).
 #include <algorithm>
 
 #include "gs_internal.cuh"
