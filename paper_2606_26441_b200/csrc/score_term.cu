@@ -478,7 +478,12 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
     }
 }
 
-constexpr int kCandBuf = 2560;   // candidate keys a CTA collects in shared memory before it appends them to the queries' lists
+constexpr int kWarpBuf = 80;                  // candidate keys a warp collects in shared memory before it appends them
+#ifndef GS_FLUSH_AT
+#define GS_FLUSH_AT 40
+#endif
+constexpr int kFlushAt = GS_FLUSH_AT;                  // ... which it does at the end of a row once it holds more than this many
+constexpr int kCandBuf = kBWarps * kWarpBuf;
 
 template <int WT>
 __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const TermParams p) {
@@ -490,21 +495,35 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     const int chunk = (int)(blockIdx.x - (unsigned)j * p.n_chunks);
     const int tile = p.ts.first + j * p.ts.stride;
     const int32_t base = tile * kBT;
-    // shared memory: rows [kBWarps][kBT] | descriptors [kBWarps][32] uint2 | candidate keys [kCandBuf] u64 |
-    // candidate queries [kCandBuf] u16 | counter (16 bytes) | strips [H][kBT]
+    // shared memory: rows [kBWarps][kBT] | descriptors [kBWarps][32] uint2 | candidate keys [kBWarps][kWarpBuf] u64 |
+    // candidate queries [kBWarps][kWarpBuf] u16 | counters [kBWarps] + query counter | strips [H][kBT]
     constexpr size_t kOffDesc = (size_t)kBWarps * kBT * 4;
     constexpr size_t kOffKey = kOffDesc + (size_t)kBWarps * 32 * 8;
     constexpr size_t kOffQ = kOffKey + (size_t)kCandBuf * 8;
     constexpr size_t kOffCnt = kOffQ + (size_t)kCandBuf * 2;
-    constexpr size_t kOffStrip = kOffCnt + 16;
+    constexpr size_t kOffStrip = kOffCnt + (size_t)(kBWarps + 4) * 4;
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
     const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
-    uint64_t* s_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey);
-    uint16_t* s_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ);
-    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt);
-    uint32_t* s_next = s_cnt + 1;
+    uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey) + warp * kWarpBuf;     // the warp's candidate buffer
+    uint16_t* w_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ) + warp * kWarpBuf;
+    uint32_t* w_cnt = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + warp;
+    uint32_t* s_next = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + kBWarps;
     W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
-    if (threadIdx.x == 0) { *s_cnt = 0u; *s_next = 2u * kBWarps; }
+    if (lane == 0) *w_cnt = 0u;
+    if (threadIdx.x == 0) *s_next = 2u * kBWarps;
+    // the warp appends its buffered candidates to the queries' lists (all the atomics of a round in flight together)
+    auto flush = [&]() {
+        __syncwarp();
+        const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)kWarpBuf);
+        for (uint32_t i = lane; i < n_buf; i += 32) {
+            const int64_t bb = p.q0 + (int64_t)chunk * p.chunk + w_q[i];
+            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[bb], 1u);
+            if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[bb * p.sink.cand_cap + pos] = w_key[i];
+        }
+        __syncwarp();
+        if (lane == 0) *w_cnt = 0u;
+        __syncwarp();
+    };
     {
         const W* __restrict__ g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * kBT;
         constexpr int per = kBT / (16 / (int)sizeof(W));
@@ -640,11 +659,11 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                     const int cell = 4 * (lane + 32 * r) + u;
                     if (cell < n_live && (sc[r][u] > thr_s || cell <= tie_cells)) {
                         const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc[r][u])), (uint32_t)(base + cell));
-                        const uint32_t slot = atomicAdd(s_cnt, 1u);
-                        if (slot < (uint32_t)kCandBuf) {
-                            s_key[slot] = key;
-                            s_q[slot] = (uint16_t)(q - chunk * p.chunk);
-                        } else {
+                        const uint32_t slot = atomicAdd(w_cnt, 1u);
+                        if (slot < (uint32_t)kWarpBuf) {
+                            w_key[slot] = key;
+                            w_q[slot] = (uint16_t)(q - chunk * p.chunk);
+                        } else {                                         // buffer full: append directly
                             const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
                             if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                         }
@@ -652,15 +671,10 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 }
             }
         }
+        __syncwarp();
+        if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt) flush();
     }
-    if (!filter) return;
-    __syncthreads();
-    const uint32_t n_buf = min(*s_cnt, (uint32_t)kCandBuf);
-    for (uint32_t i = threadIdx.x; i < n_buf; i += kBWarps * 32) {
-        const int64_t b = p.q0 + (int64_t)chunk * p.chunk + s_q[i];
-        const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
-        if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = s_key[i];
-    }
+    if (filter) flush();
 }
 
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
@@ -681,8 +695,15 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged,
     return GS_OK;
 }
 
-constexpr int kStagedMinQueries = 64;     // below this the warp-per-row shape is as fast or faster (measured batch sweep)
-constexpr int kStagedChunk = 512;         // queries per CTA of the staged kernel
+#ifndef GS_STAGED_MIN
+#define GS_STAGED_MIN 192
+#endif
+constexpr int kStagedMinQueries = GS_STAGED_MIN;     // below this the warp-per-row shape is as fast or faster (batch sweep at 8.8M docs: 64 queries 3.9 vs 7.3 ms, 128: 7.2 vs 7.2, 256: 13.7 vs 13.2, 500: 25.9 vs 21.8)
+constexpr int kStagedChunk = 512;         // most queries per CTA of the staged / batch kernels
+#ifndef GS_CHUNK_WAVES
+#define GS_CHUNK_WAVES 16
+#endif
+constexpr int kChunkWaves = GS_CHUNK_WAVES;   // CTAs per SM a launch aims for before it stops splitting the queries
 
 }  // namespace
 
@@ -713,11 +734,19 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     const size_t smem_staged = (size_t)kWarpsStaged * ix->Ts * 4 + (size_t)p.H * ix->Ts * wbytes;
     // query_group > 0 pins the small-batch kernel (that many cell rows per CTA); -1 pins the generic staged kernel
     if (group <= 0 && nq >= kStagedMinQueries && p.H > 0 && smem_staged <= (size_t)smem_max) {
-        p.chunk = kStagedChunk;
+        // queries per CTA: all of them (up to kStagedChunk) when the doc tiles alone fill the machine many times over;
+        // a launch over few tiles (the threshold sample, a small collection) splits the queries so that the grid still
+        // has about kChunkWaves CTAs per SM, down to one cell row per warp
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const int64_t want = ((int64_t)kChunkWaves * sms + ts.count - 1) / ts.count;
+        const int64_t most = std::max<int64_t>(1, nq / kWarpsStaged);
+        int64_t n_chunks = std::max<int64_t>((nq + kStagedChunk - 1) / kStagedChunk, std::min(want, most));
+        p.chunk = (int32_t)((nq + n_chunks - 1) / n_chunks);
         p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + 16;
+        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4;
         if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max) {
             auto go = [&](auto kern) -> gs_status_t {
                 GS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch));
