@@ -524,14 +524,23 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         if (lane == 0) *w_cnt = 0u;
         __syncwarp();
     };
-    {
-        const W* __restrict__ g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * kBT;
-        constexpr int per = kBT / (16 / (int)sizeof(W));
-        for (int i = threadIdx.x; i < p.H * per; i += kBWarps * 32) {
-            const int h = i / per, c = i - h * per;
-            reinterpret_cast<int4*>(s_strip + (size_t)h * kBT)[c] = __ldg(reinterpret_cast<const int4*>(g + (size_t)h * p.N_pad) + c);
-        }
+    // The tile's strips come in by TMA: one thread issues a 1-D bulk copy per strip (kBT weights, contiguous in the strip)
+    // that completes on an mbarrier; a warp waits for it only before its first head phase, so the copy runs under the
+    // probes and the tail scatter of every warp's first row.
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffCnt + (size_t)(kBWarps + 2) * 4);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_s) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        const uint32_t row_bytes = (uint32_t)(kBT * sizeof(W));
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_s), "r"(row_bytes * (uint32_t)p.H) : "memory");
+        const W* g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * kBT;
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_strip);
+        for (int h = 0; h < p.H; ++h)
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(dst + (uint32_t)h * row_bytes), "l"(g + (size_t)h * p.N_pad), "r"(row_bytes), "r"(mbar_s) : "memory");
     }
+    bool strips_ready = false;
     const bool filter = p.sink.thr != nullptr;
     // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
     // warp and warp + kBWarps of the chunk and claims further ones from a shared-memory counter, two rows ahead of the
@@ -582,6 +591,14 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         }
         __syncwarp();
 
+        if (!strips_ready) {                        // once per warp: the bulk copies of the tile's strips have landed
+            uint32_t ok = 0;
+            do {
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(ok) : "r"(mbar_s) : "memory");
+            } while (!ok);
+            strips_ready = true;
+        }
         // head strips: the lane's 16 documents (quads lane, lane+32, lane+64, lane+96) stay in registers
         const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
         A sc[4][4];
