@@ -515,10 +515,26 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     auto flush = [&]() {
         __syncwarp();
         const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)kWarpBuf);
-        for (uint32_t i = lane; i < n_buf; i += 32) {
-            const int64_t bb = p.q0 + (int64_t)chunk * p.chunk + w_q[i];
-            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[bb], 1u);
-            if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[bb * p.sink.cand_cap + pos] = w_key[i];
+        // The buffer holds one run of entries per row the warp has finished: the first lane of a run reserves the whole
+        // run in its query's list with ONE atomic (same-address atomics of one warp instruction are served one after the
+        // other, each a round trip: 32 lanes on two or three counters cost tens of microseconds per flush).
+        const unsigned le_ = 0xFFFFFFFFu >> (31 - lane);
+        for (uint32_t i0 = 0; i0 < n_buf; i0 += 32) {
+            const uint32_t i = i0 + lane;
+            const bool valid = i < n_buf;
+            const uint32_t qi = valid ? (uint32_t)w_q[i] : 0xFFFFFFFFu;
+            const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, qi, 1);
+            const bool head = valid && (lane == 0 || qi != prev);
+            const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
+            const int n_valid = __popc(__ballot_sync(0xFFFFFFFFu, valid));
+            const int start = 31 - __clz((int)(heads & le_));                 // first lane of this lane's run
+            const unsigned later = heads & ~le_;
+            const int end = later ? __ffs((int)later) - 1 : n_valid;          // one past the run's last lane
+            const int64_t bb = p.q0 + (int64_t)chunk * p.chunk + (valid ? qi : 0u);
+            uint32_t pos = 0;
+            if (head) pos = atomicAdd(&p.sink.cand_cnt[bb], (uint32_t)(end - lane));
+            pos = __shfl_sync(0xFFFFFFFFu, pos, start & 31) + (uint32_t)(lane - start);
+            if (valid && (int64_t)pos < p.sink.cand_cap) p.sink.cand[bb * p.sink.cand_cap + pos] = w_key[i];
         }
         __syncwarp();
         if (lane == 0) *w_cnt = 0u;
@@ -712,22 +728,31 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged,
     return GS_OK;
 }
 
+// From how many queries on the CTA-per-doc-tile kernels are used.  Batch sweep on B200 (ms per batch, warp-per-row shape vs
+// batch kernel): 8.8M docs 64: 3.87 / 4.01, 96: 5.58 / 5.33, 128: 7.23 / 6.64, 256: 13.7 / 11.8, 500: 25.9 / 20.9;
+// 1M docs 128: 1.03 / 1.09, 192: 1.48 / 1.53, 256: 1.85 / 1.83, 500: 3.40 / 3.19 — the fixed cost of a CTA (staging, first-row
+// probes) is amortised over fewer rows when the collection has few doc tiles.
 #ifndef GS_STAGED_MIN
-#define GS_STAGED_MIN 192
+#define GS_STAGED_MIN 256
 #endif
-constexpr int kStagedMinQueries = GS_STAGED_MIN;     // below this the warp-per-row shape is as fast or faster (batch sweep at 8.8M docs: 64 queries 3.9 vs 7.3 ms, 128: 7.2 vs 7.2, 256: 13.7 vs 13.2, 500: 25.9 vs 21.8)
+constexpr int kStagedMinQueries = GS_STAGED_MIN;
+constexpr int kStagedMinQueriesLarge = GS_STAGED_MIN < 96 ? GS_STAGED_MIN : 96;     // collections of >= kLargeTiles doc tiles
+constexpr int kLargeTiles = 8192;
 constexpr int kStagedChunk = 512;         // most queries per CTA of the staged / batch kernels
 #ifndef GS_CHUNK_WAVES
 #define GS_CHUNK_WAVES 16
 #endif
 constexpr int kChunkWaves = GS_CHUNK_WAVES;   // CTAs per SM a launch aims for before it stops splitting the queries
+static inline bool cta_per_tile(const gs_index* ix, int64_t nq) {
+    return nq >= (ix->ntiles >= kLargeTiles ? kStagedMinQueriesLarge : kStagedMinQueries);
+}
 
 }  // namespace
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    if (group == 0 && nq >= kStagedMinQueries && use_head && ix->H > 0 && ix->Ts == kBT && ix->seg2 != nullptr)
+    if (group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->Ts == kBT && ix->seg2 != nullptr)
         return kBWarps;                                                 // batch kernel
-    if (group <= 0 && nq >= kStagedMinQueries && use_head && ix->H > 0) return kWarpsStaged;
+    if (group <= 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0) return kWarpsStaged;
     return norm_warps(group);
 }
 
@@ -750,7 +775,7 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     const size_t wbytes = ix->wtype == GS_W_F32 ? 4 : 1;
     const size_t smem_staged = (size_t)kWarpsStaged * ix->Ts * 4 + (size_t)p.H * ix->Ts * wbytes;
     // query_group > 0 pins the small-batch kernel (that many cell rows per CTA); -1 pins the generic staged kernel
-    if (group <= 0 && nq >= kStagedMinQueries && p.H > 0 && smem_staged <= (size_t)smem_max) {
+    if (group <= 0 && cta_per_tile(ix, nq) && p.H > 0 && smem_staged <= (size_t)smem_max) {
         // queries per CTA: all of them (up to kStagedChunk) when the doc tiles alone fill the machine many times over;
         // a launch over few tiles (the threshold sample, a small collection) splits the queries so that the grid still
         // has about kChunkWaves CTAs per SM, down to one cell row per warp

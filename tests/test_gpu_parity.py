@@ -429,13 +429,13 @@ BATCH_KERNEL_WARPS = 32   # kBWarps of score_term.cu
 @pytest.mark.parametrize("mode", ["f32", "u8"])
 @pytest.mark.parametrize("qcfg", ["mid", "skew_b32"])
 @pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=5), dict(head_max=-1), dict(tile_docs=1024, head_density=0.05)])
-def test_batch_of_200_takes_the_cta_per_tile_term_kernels(gs, mode, build_kw, qcfg):
-    """From 192 queries on the term-parallel kernel runs as a persistent CTA per doc tile with the strips staged in shared
+def test_batch_of_256_takes_the_cta_per_tile_term_kernels(gs, mode, build_kw, qcfg):
+    """From 256 queries on (96 on collections of at least 8192 doc tiles) the term-parallel kernel runs as a persistent CTA per doc tile with the strips staged in shared
     memory (unless the index has no strips) — the batch kernel on 512-doc tiles, the generic staged kernel on other tile sizes:
-    every score of 200 queries x 20 011 docs, and the top-50, against the oracle.  The "skew_b32" queries (5..256 terms,
+    every score of 256 queries x 20 011 docs, and the top-50, against the oracle.  The "skew_b32" queries (5..256 terms,
     Zipf 1.3) have more than 32 tail terms, which the batch kernel probes in line after the prefetched first 32."""
     docs = wl.make_docs("mid", n_docs=20_011)
-    queries = wl.make_queries(qcfg, n_queries=200)
+    queries = wl.make_queries(qcfg, n_queries=256)
     if mode == "u8":
         docs, queries = docs.to_u8(), queries.to_u8()
     ix = gs.Index.from_numpy(docs, wl.VOCAB, **build_kw)
