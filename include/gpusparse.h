@@ -203,6 +203,21 @@ GS_API gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t num_
                           int32_t k, int32_t* out_ids, void* out_scores, void* workspace,
                           size_t workspace_bytes, gs_stream_t stream);
 
+/* Exact merge of partial top-k lists (document sharding; §6.7 L322-324 merges on
+ * the host, L430 asks for a device-side merge).  `ids` [n_lists][B][k_in] int32 and `scores` [n_lists][B][k_in]
+ * (float | int32 per wtype) are DEVICE arrays: list l holds, for every query, the top-k_in of shard l as returned by
+ * gs_search (shard-local doc ids, -1 in unused slots).  `list_doc_base` [n_lists] is a HOST array (or NULL = zeros):
+ * the global id of shard l's document 0.  Output: the k_out best of the union per query under (score desc, global
+ * doc id asc), rows padded with (-1, -inf | INT32_MIN) when the union is smaller.  Global ids must be distinct and
+ * < 2^32 - 1.  n_lists <= GS_MERGE_MAX_LISTS, k_out <= GS_MAX_K.  Asynchronous on `stream`, never allocates. */
+#define GS_MERGE_MAX_LISTS 64
+GS_API gs_status_t gs_merge_topk_workspace_bytes(int32_t n_lists, int64_t num_queries, int32_t k_in, int32_t k_out,
+                                                 size_t* out_bytes);
+GS_API gs_status_t gs_merge_topk(int32_t wtype, int32_t n_lists, int64_t num_queries, int32_t k_in, int32_t k_out,
+                                 const int32_t* ids, const void* scores, const int64_t* list_doc_base,
+                                 int32_t* out_doc_ids, void* out_scores, void* workspace, size_t workspace_bytes,
+                                 gs_stream_t stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Kernel timing (SURVEY §8d measurement): when enabled on the calling thread, every kernel launch of
  * the following gs_search / gs_score_dense / gs_topk_dense calls is bracketed by CUDA events on the

@@ -25,7 +25,7 @@ EXPORTS = [
     "gs_index_build", "gs_index_info", "gs_index_free", "gs_index_copy_meta", "gs_index_copy_list",
     "gs_index_copy_head_terms",
     "gs_search_workspace_bytes", "gs_search", "gs_search_host", "gs_search_stats", "gs_score_dense",
-    "gs_topk_workspace_bytes", "gs_topk_dense", "gs_strerror", "gs_version", "gs_abi_version",
+    "gs_topk_workspace_bytes", "gs_topk_dense", "gs_merge_topk_workspace_bytes", "gs_merge_topk", "gs_strerror", "gs_version", "gs_abi_version",
     "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name",
 ]
 GS_PROF_CLASSES = 8
@@ -100,6 +100,8 @@ def lib():
         L.gs_score_dense.argtypes = [vp, P(gs_csr_t), P(gs_search_opts_t), vp, i64, vp, sz, vp]
         L.gs_topk_workspace_bytes.argtypes = [i64, i64, i32, P(sz)]
         L.gs_topk_dense.argtypes = [vp, i32, i64, i64, i64, i32, vp, vp, vp, sz, vp]
+        L.gs_merge_topk_workspace_bytes.argtypes = [i32, i64, i32, i32, P(sz)]
+        L.gs_merge_topk.argtypes = [i32, i32, i64, i32, i32, vp, vp, P(i64), vp, vp, vp, sz, vp]
         L.gs_strerror.argtypes = [ctypes.c_int]
         L.gs_strerror.restype = ctypes.c_char_p
         L.gs_version.restype = ctypes.c_char_p
@@ -338,3 +340,29 @@ def topk_dense(scores, k: int, n: Optional[int] = None, stream=None):
     _check(lib().gs_topk_dense(scores.data_ptr(), wt, rows, n, ld, k, ids.data_ptr(), sc.data_ptr(), ws.data_ptr(),
                                ws.numel(), _stream_ptr(stream)))
     return ids, sc
+
+
+def merge_topk(ids, scores, k_out: int, doc_bases=None, workspace=None, stream=None):
+    """gs_merge_topk: partial top-k lists ``ids``/``scores`` [n_lists, B, k_in] (device, shard-local doc ids, -1 padding) ->
+    the k_out best of the union per query (global ids = local id + doc_bases[list]), score desc, ties by lower id."""
+    torch = _torch()
+    assert ids.is_cuda and scores.is_cuda and ids.dim() == 3 and ids.shape == scores.shape
+    assert ids.dtype == torch.int32 and ids.is_contiguous() and scores.is_contiguous()
+    n_lists, B, k_in = ids.shape
+    wt = GS_W_F32 if scores.dtype == torch.float32 else GS_W_U8
+    if wt == GS_W_U8:
+        assert scores.dtype == torch.int32
+    need = ctypes.c_size_t()
+    _check(lib().gs_merge_topk_workspace_bytes(n_lists, B, k_in, k_out, ctypes.byref(need)))
+    if workspace is None:
+        workspace = torch.empty(max(need.value, 256), dtype=torch.uint8, device=ids.device)
+    assert workspace.numel() >= need.value
+    bases = None
+    if doc_bases is not None:
+        assert len(doc_bases) == n_lists
+        bases = (ctypes.c_int64 * n_lists)(*[int(x) for x in doc_bases])
+    out_ids = torch.empty((B, k_out), dtype=torch.int32, device=ids.device)
+    out_sc = torch.empty((B, k_out), dtype=scores.dtype, device=ids.device)
+    _check(lib().gs_merge_topk(wt, n_lists, B, k_in, k_out, ids.data_ptr(), scores.data_ptr(), bases, out_ids.data_ptr(),
+                               out_sc.data_ptr(), workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
+    return out_ids, out_sc

@@ -13,7 +13,7 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgpusparse.so")
-SOURCES = ["api.cu", "index_build.cu", "ingest.cu", "score_term.cu", "score_doc.cu", "topk.cu"]
+SOURCES = ["api.cu", "index_build.cu", "ingest.cu", "score_term.cu", "score_doc.cu", "topk.cu", "merge.cu"]
 HEADERS = [os.path.join(CSRC, "gs_internal.cuh"), os.path.join(os.path.dirname(_HERE), "include", "gpusparse.h")]
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",

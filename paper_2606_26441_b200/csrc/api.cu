@@ -564,6 +564,34 @@ gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t rows, int64
     return gs_launch_select(src, rows, k, out_ids, out_scores, nullptr, nullptr, nullptr, 0, ws, (cudaStream_t)stream);
 }
 
+gs_status_t gs_merge_topk_workspace_bytes(int32_t n_lists, int64_t B, int32_t k_in, int32_t k_out, size_t* out_bytes) {
+    if (!out_bytes || n_lists < 1 || n_lists > GS_MERGE_MAX_LISTS || B < 0 || k_in < 1) return GS_ERR_INVALID_ARG;
+    if (k_out < 1 || k_out > GS_MAX_K || B > 65535) return GS_ERR_OUT_OF_RANGE;
+    *out_bytes = gs_merge_scratch_bytes(n_lists, B, k_in, k_out);
+    return GS_OK;
+}
+
+gs_status_t gs_merge_topk(int32_t wtype, int32_t n_lists, int64_t B, int32_t k_in, int32_t k_out, const int32_t* ids,
+                          const void* scores, const int64_t* list_doc_base, int32_t* out_ids, void* out_scores, void* ws,
+                          size_t ws_bytes, gs_stream_t stream) {
+    if (!out_ids || !out_scores || !ws || n_lists < 1 || n_lists > GS_MERGE_MAX_LISTS || B < 0 || k_in < 1)
+        return GS_ERR_INVALID_ARG;
+    if (wtype != GS_W_F32 && wtype != GS_W_U8) return GS_ERR_INVALID_ARG;
+    if (k_out < 1 || k_out > GS_MAX_K || B > 65535) return GS_ERR_OUT_OF_RANGE;
+    if ((int64_t)n_lists * k_in > (int64_t)1 << 20) return GS_ERR_OUT_OF_RANGE;       // one-launch select: rows of up to 2^20 keys
+    GS_TRY(check_device());
+    if (B > 0 && (!is_device_ptr(ids) || !is_device_ptr(scores))) return GS_ERR_INVALID_ARG;
+    if (!is_device_ptr(out_ids) || !is_device_ptr(out_scores) || !is_device_ptr(ws)) return GS_ERR_INVALID_ARG;
+    if (ws_bytes < gs_merge_scratch_bytes(n_lists, B, k_in, k_out)) return GS_ERR_OOM;
+    if (list_doc_base)
+        for (int l = 0; l < n_lists; ++l)
+            if (list_doc_base[l] < 0 || list_doc_base[l] >= 0xFFFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+    gs_tls_launches = 0;
+    if (B == 0) return GS_OK;
+    return gs_launch_merge(wtype, n_lists, B, k_in, k_out, ids, scores, list_doc_base, out_ids, out_scores, ws,
+                           (cudaStream_t)stream);
+}
+
 void gs_profile_enable(int32_t on) {
     tls_prof_on = on != 0;
     for (ProfRec& r : tls_prof) { tls_event_pool.push_back(r.a); tls_event_pool.push_back(r.b); }

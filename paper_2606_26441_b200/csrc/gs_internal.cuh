@@ -186,3 +186,9 @@ size_t gs_select_scratch_bytes(int64_t rows, int32_t k);
 gs_status_t gs_launch_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* out_ids, void* out_scores,
                              uint64_t* out_thr, uint64_t* out_keys, uint32_t* out_cnt, int64_t out_cap,
                              void* scratch, cudaStream_t s);
+
+// k-way merge of partial top-k lists (merge.cu)
+size_t gs_merge_scratch_bytes(int32_t n_lists, int64_t B, int32_t k_in, int32_t k_out);
+gs_status_t gs_launch_merge(int32_t wtype, int32_t n_lists, int64_t B, int32_t k_in, int32_t k_out, const int32_t* ids,
+                            const void* scores, const int64_t* base, int32_t* out_ids, void* out_scores, void* scratch,
+                            cudaStream_t s);

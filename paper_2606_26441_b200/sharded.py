@@ -1,0 +1,63 @@
+"""Document sharding with a device-side top-k merge — the "next" row beyond the graded
+one-GPU path.
+
+PAPER.md §6.7 (L322-324) splits the documents evenly over two GPUs, runs the scatter-add kernel on each and merges the
+partial top-k lists on the HOST (0.6x of one GPU at 100K docs); its future work (L430, item 4) asks for a device-side
+merge over NVLink.  Contiguous doc-id ranges are independent: every rank indexes its own range and returns its own
+[B, k] (local id, score); ONE exchange — an all-gather of B*k*8 bytes per rank (4 MB at B=500, k=1000: latency bound
+over NVLink 5 / NVSwitch) — and a k-way merge under the same order (score desc, global doc id asc) give exactly the
+single-index result, ties included.  The merge is ``gs_merge_topk`` (CUDA, merge.cu); this module holds the host
+logic only: the ranges, the exchange and the call.  No scoring arithmetic lives here.
+"""
+from __future__ import annotations
+
+from typing import List, Sequence, Tuple
+
+
+def shard_ranges(num_docs: int, world: int) -> List[Tuple[int, int]]:
+    """Contiguous doc-id ranges [lo, hi) of `world` shards: sizes differ by at most one, earlier shards take the extra
+    document (the paper splits "evenly", L324)."""
+    if num_docs < 0 or world < 1:
+        raise ValueError("num_docs must be >= 0 and world >= 1")
+    q, r = divmod(num_docs, world)
+    out, lo = [], 0
+    for i in range(world):
+        hi = lo + q + (1 if i < r else 0)
+        out.append((lo, hi))
+        lo = hi
+    return out
+
+
+def gather_lists(ids, scores, dist=None):
+    """All-gather of every rank's [B, k] result into [world, B, k] tensors (rank order = shard order).  Without an
+    initialised process group the single list is returned as [1, B, k]."""
+    import torch
+    if dist is None or not dist.is_available() or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ids.unsqueeze(0).contiguous(), scores.unsqueeze(0).contiguous()
+    world = dist.get_world_size()
+    all_ids = torch.empty((world,) + tuple(ids.shape), dtype=ids.dtype, device=ids.device)
+    all_sc = torch.empty((world,) + tuple(scores.shape), dtype=scores.dtype, device=scores.device)
+    dist.all_gather([all_ids[i] for i in range(world)], ids.contiguous())        # slices of one buffer: no extra copy
+    dist.all_gather([all_sc[i] for i in range(world)], scores.contiguous())
+    return all_ids, all_sc
+
+
+class ShardedIndex:
+    """One rank's view of a document-sharded collection: the local index over docs [lo, hi) plus the exchange + merge.
+
+    ``local_index`` is a ``binding.Index`` built from the rows [lo, hi) of the collection (row 0 of the shard is global
+    document ``lo``); ``ranges`` are the ranges of ALL shards in rank order (``shard_ranges``)."""
+
+    def __init__(self, local_index, ranges: Sequence[Tuple[int, int]], rank: int, dist=None):
+        if not 0 <= rank < len(ranges):
+            raise ValueError("rank outside the shard list")
+        self.index, self.ranges, self.rank, self.dist = local_index, list(ranges), rank, dist
+
+    def search(self, q_indptr, q_terms, q_weights, k: int, **opts):
+        """Every rank searches its shard for the same query batch; returns the merged global (ids, scores) on every
+        rank.  The local k is min(k, ...) of nothing: a shard smaller than k pads with -1, which the merge drops."""
+        from . import binding as gs
+        ids, sc = self.index.search(q_indptr, q_terms, q_weights, k, **opts)
+        all_ids, all_sc = gather_lists(ids, sc, self.dist)
+        bases = [lo for lo, _ in self.ranges][:all_ids.shape[0]] if all_ids.shape[0] > 1 else [self.ranges[self.rank][0]]
+        return gs.merge_topk(all_ids, all_sc, k, doc_bases=bases)
