@@ -455,6 +455,22 @@ def test_batch_of_256_takes_the_cta_per_tile_term_kernels(gs, mode, build_kw, qc
     ix.close()
 
 
+def test_batch_kernel_is_deterministic_run_to_run(gs):
+    """DESIGN.md R2: every (query, doc) cell is owned by one warp and its additions keep the query's term order, so the fp32
+    scores of the batch kernel are bitwise identical from run to run (the candidate lists are not ordered, the results are)."""
+    docs = wl.make_docs("mid", n_docs=20_011)
+    queries = wl.make_queries("skew_b32", n_queries=256)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    S0 = ix.score_dense(*dev(queries), algo="term").cpu().numpy()
+    ids0, sc0 = gpu_search(gs, ix, queries, 100, algo="term")
+    assert ix.stats()["query_group"] == BATCH_KERNEL_WARPS
+    for _ in range(3):
+        assert np.array_equal(ix.score_dense(*dev(queries), algo="term").cpu().numpy().view(np.uint32), S0.view(np.uint32))
+        ids, sc = gpu_search(gs, ix, queries, 100, algo="term")
+        assert np.array_equal(ids, ids0) and np.array_equal(sc.view(np.uint32), sc0.view(np.uint32))
+    ix.close()
+
+
 # ----------------------------------------------------------------------------------------------------
 # paper scale (BASELINE.json configs[2] and [3]) in the launch configuration bench.py times
 # ----------------------------------------------------------------------------------------------------
