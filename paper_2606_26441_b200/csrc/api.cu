@@ -203,6 +203,8 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
     c.qb.tail_w = (uint32_t*)take((size_t)nnz * 4);
     c.qb.tail_cnt = (int32_t*)take((size_t)B * 4);
     c.qb.tail32 = (uint2*)take((size_t)B * GS_TAIL32 * 8);
+    c.qb.xpair = (uint2*)take((size_t)B * GS_XSTRIP_MAX * 8);
+    c.qb.xcnt = (int32_t*)take((size_t)B * 4);
     c.thr = (uint64_t*)take((size_t)B * 8);
     c.cand_cnt = (uint32_t*)take((size_t)B * 4);
     c.overflow_list = (int32_t*)take((size_t)B * 4);
@@ -256,7 +258,8 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     GS_CUDA(cudaMemsetAsync(c.sb, 0, sizeof(StatsBlock), s));
     if (B == 0) return GS_OK;
     const bool validate = p.flags & GS_FLAG_VALIDATE_QUERIES;
-    GS_TRY(gs_launch_ingest(ix, q, validate, p.use_head, &c.qb, s));
+    GS_TRY(gs_launch_ingest(ix, q, validate, p.use_head,
+                            p.algo == GS_ALGO_TERM_PARALLEL && gs_score_term_wants_x(ix, B, p.group, p.use_head), &c.qb, s));
     if (validate) {
         int32_t st = 0;
         GS_CUDA(cudaMemcpyAsync(&st, &c.sb->status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
@@ -381,7 +384,7 @@ void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
     void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
-                    ix->seg, ix->seg2, ix->head_slot, ix->head_strip, ix->host_ws, ix->host_stage};
+                    ix->seg, ix->seg2, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
 }
@@ -393,7 +396,7 @@ gs_status_t gs_index_info(const gs_index_t* ix, gs_info_t* out) {
     out->num_tiles = ix->ntiles; out->head_terms = ix->H;
     out->bytes_inverted = ix->bytes_inverted; out->bytes_inverted_meta = ix->bytes_meta;
     out->bytes_forward = ix->bytes_forward; out->bytes_head = ix->bytes_head;
-    out->head_terms_term_parallel = ix->H; out->forward_tail_nnz = ix->P_tail;
+    out->head_terms_term_parallel = ix->H + ix->HX; out->forward_tail_nnz = ix->P_tail;
     out->forward_padded_nnz = ix->P_fwd; out->reserved = 0;
     out->bytes_total = ix->bytes_inverted + ix->bytes_meta + ix->bytes_forward + ix->bytes_head;
     return GS_OK;
@@ -533,7 +536,8 @@ gs_status_t gs_score_dense(const gs_index_t* ix, const gs_csr_t* q, const gs_sea
     if (ws_bytes < c.fixed_bytes) return GS_ERR_OOM;
     c.qb.B = q->rows; c.qb.nnz = q->nnz; c.qb.indptr = q->indptr;
     if (q->rows == 0 || ix->N == 0) return GS_OK;
-    GS_TRY(gs_launch_ingest(ix, q, false, p.use_head, &c.qb, s));
+    GS_TRY(gs_launch_ingest(ix, q, false, p.use_head,
+                            p.algo == GS_ALGO_TERM_PARALLEL && gs_score_term_wants_x(ix, q->rows, p.group, p.use_head), &c.qb, s));
     gs_tileset all{0, 1, ix->ntiles};
     gs_sink sink{};
     sink.dense = (uint32_t*)out_scores;

@@ -8,6 +8,13 @@
 
 #define GS_STRIP_MAX 64         // dense strips kept by the index
 #define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
+#ifndef GS_XSTRIP_MAX
+#define GS_XSTRIP_MAX 64
+#endif
+#ifndef GS_XDENS
+#define GS_XDENS 0.10f
+#endif
+// GS_XSTRIP_MAX: second tier of dense strips, read from global memory by the term-parallel kernels only
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
 #define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings
 #define GS_TAIL32 32            // tail terms of a query kept in the fixed-stride prefetch table
@@ -64,6 +71,12 @@ struct gs_index {
     int32_t head_terms_host[GS_STRIP_MAX];
     int16_t* head_slot = nullptr;    // [V]: strip number of a term or -1
     void* head_strip = nullptr;      // [H][N_pad] float | uint8 (0 where the doc is not in the list)
+    // second tier ("x strips"): the next densest lists (density >= 0.10), a dense copy used by the term-parallel kernels
+    // only — there they replace the scatter of a 50-130-posting segment per doc tile by four 128-bit loads and eight
+    // FFMA2; the lists stay tail terms everywhere else (forward index, document-parallel kernel)
+    int32_t HX = 0;
+    int16_t* xslot = nullptr;        // [V]: x-strip number of a term or -1
+    void* xstrip = nullptr;          // [HX][N_pad]
     // allocator
     gs_alloc_t alloc{};
     bool has_alloc = false;
@@ -108,6 +121,9 @@ struct gs_qbatch {
     const int64_t* indptr = nullptr;   // caller's CSR indptr (device)
     uint2* head_pair = nullptr;        // [B][GS_HEAD_MAX] compact (strip number, accumulator-typed weight bits)
     int32_t* head_cnt = nullptr;       // [B] number of head terms of the query
+    uint2* xpair = nullptr;            // [B][GS_XSTRIP_MAX] compact (x-strip number, weight bits); used when x_on
+    int32_t* xcnt = nullptr;           // [B]
+    bool x_on = false;                 // the batch's x-strip terms are in xpair (and NOT in the tail lists)
     int32_t* tail_term = nullptr;      // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]
     uint32_t* tail_w = nullptr;        // [nnz] accumulator-typed
     int32_t* tail_cnt = nullptr;       // [B]
@@ -149,8 +165,9 @@ struct GsProfScope {
     cudaStream_t stream = nullptr;
 };
 
-gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head,
+gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head, bool use_x,
                              gs_qbatch* qb, cudaStream_t s);
+bool gs_score_term_wants_x(const gs_index* ix, int64_t nq, int group, bool use_head);   // the batch kernel will run
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);

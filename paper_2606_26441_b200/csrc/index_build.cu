@@ -310,6 +310,25 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     if (!ix->head_slot) return GS_ERR_OOM;
     GS_CUDA(cudaMemcpyAsync(ix->head_slot, h_slot.data(), sizeof(int16_t) * (size_t)V, cudaMemcpyHostToDevice, s));
 
+    // ---- second tier of strips for the term-parallel kernels (512-doc tiles only: the batch kernel is their user)
+    std::vector<int32_t> xorder;
+    if (o.head_max >= 0 && ix->Ts == 512 && N > 0) {
+        const float xdens = std::min(dens, GS_XDENS);
+        for (int32_t t = 0; t < V; ++t)
+            if (h_slot[t] < 0 && h_len[t] > 0 && (double)h_len[t] >= (double)xdens * (double)N) xorder.push_back(t);
+        std::stable_sort(xorder.begin(), xorder.end(), [&](int32_t a, int32_t b) { return h_len[a] > h_len[b]; });
+        if ((int)xorder.size() > GS_XSTRIP_MAX) xorder.resize(GS_XSTRIP_MAX);
+    }
+    ix->HX = (int32_t)xorder.size();
+    if (ix->HX > 0) {
+        std::vector<int16_t> x_slot(V, (int16_t)-1);
+        for (int h = 0; h < ix->HX; ++h) x_slot[xorder[h]] = (int16_t)h;
+        ix->xslot = (int16_t*)gs_dev_alloc(ix, sizeof(int16_t) * (size_t)V, s);
+        if (!ix->xslot) return GS_ERR_OOM;
+        GS_CUDA(cudaMemcpyAsync(ix->xslot, x_slot.data(), sizeof(int16_t) * (size_t)V, cudaMemcpyHostToDevice, s));
+        GS_CUDA(cudaStreamSynchronize(s));        // x_slot is a local
+    }
+
     // ---- forward index, hybrid: strips for the H densest lists + a block CSR of every other posting
     {
         int64_t p_tail = P;
@@ -428,6 +447,18 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
                                                                    (W*)ix->head_strip + (size_t)h * (size_t)ix->N_pad);
         }
         ix->bytes_head = (int64_t)strip_bytes;
+    }
+    if (ix->HX > 0) {
+        size_t xbytes = sizeof(W) * (size_t)ix->HX * (size_t)ix->N_pad;
+        ix->xstrip = gs_dev_alloc(ix, xbytes, s);
+        if (!ix->xstrip) return GS_ERR_OOM;
+        GS_CUDA(cudaMemsetAsync(ix->xstrip, 0, xbytes, s));
+        for (int h = 0; h < ix->HX; ++h) {
+            int32_t t = xorder[h];
+            k_fill_strip<W><<<grid_for(h_len[t]), kThreads, 0, s>>>(ix->inv_doc, (const W*)ix->inv_w, h_off[t], h_len[t],
+                                                                   (W*)ix->xstrip + (size_t)h * (size_t)ix->N_pad);
+        }
+        ix->bytes_head += (int64_t)xbytes;
     }
     GS_CUDA(cudaStreamSynchronize(s));
     GS_CUDA(cudaGetLastError());

@@ -15,7 +15,9 @@ namespace {
 template <int WT>
 __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __restrict__ terms,
                          const void* __restrict__ weights, int64_t B, int32_t V, const int16_t* __restrict__ head_slot,
-                         int h_term, int validate, uint2* __restrict__ head_pair, int32_t* __restrict__ head_cnt,
+                         int h_term, const int16_t* __restrict__ xslot, int h_x, uint2* __restrict__ xpair,
+                         int32_t* __restrict__ xcnt, int validate, uint2* __restrict__ head_pair,
+                         int32_t* __restrict__ head_cnt,
                          int32_t* __restrict__ tail_term,
                          uint32_t* __restrict__ tail_w, int32_t* __restrict__ tail_cnt, uint2* __restrict__ tail32,
                          int32_t* __restrict__ status) {
@@ -23,7 +25,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
     const int64_t b = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     if (b >= B) return;
     const int64_t a = indptr[b], e = indptr[b + 1];
-    int32_t n_tail = 0, n_head = 0;
+    int32_t n_tail = 0, n_head = 0, n_x = 0;
     tail32[b * GS_TAIL32 + lane] = make_uint2(0xFFFFFFFFu, 0u);
     __syncwarp();
     for (int64_t i0 = a; i0 < e; i0 += 32) {
@@ -58,7 +60,16 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
             if (dst < GS_HEAD_MAX) head_pair[b * GS_HEAD_MAX + dst] = make_uint2((uint32_t)slot, w);
         }
         n_head = min(GS_HEAD_MAX, n_head + __popc(mh));
-        const bool is_tail = ok && slot < 0;
+        // second-tier strips (term-parallel batch searches): their own compact list, not the tail
+        int xs = (ok && slot < 0 && h_x > 0) ? (int)xslot[t] : -1;
+        if (xs >= h_x) xs = -1;
+        const unsigned mx = __ballot_sync(0xFFFFFFFFu, xs >= 0);
+        if (xs >= 0) {
+            const int dst = n_x + __popc(mx & ((1u << lane) - 1u));
+            if (dst < GS_XSTRIP_MAX) xpair[b * GS_XSTRIP_MAX + dst] = make_uint2((uint32_t)xs, w);
+        }
+        n_x = min(GS_XSTRIP_MAX, n_x + __popc(mx));
+        const bool is_tail = ok && slot < 0 && xs < 0;
         const unsigned m = __ballot_sync(0xFFFFFFFFu, is_tail);
         if (is_tail) {
             const int64_t dst = a + n_tail + __popc(m & ((1u << lane) - 1u));
@@ -69,14 +80,16 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
         n_tail += __popc(m);
         __syncwarp();
     }
-    if (lane == 0) { tail_cnt[b] = n_tail; head_cnt[b] = n_head; }
+    if (lane == 0) { tail_cnt[b] = n_tail; head_cnt[b] = n_head; xcnt[b] = n_x; }
 }
 
 }  // namespace
 
-gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head, gs_qbatch* qb,
-                             cudaStream_t s) {
+gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validate, bool use_head, bool use_x,
+                             gs_qbatch* qb, cudaStream_t s) {
     const int64_t B = q->rows;
+    const int h_x = (use_head && use_x && ix->HX > 0) ? ix->HX : 0;
+    qb->x_on = h_x > 0;
     GS_CUDA(cudaMemsetAsync(qb->status, 0, sizeof(int32_t), s));
     if (B == 0) return GS_OK;
     const int threads = 128;
@@ -84,11 +97,11 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
     GsProfScope ps(GS_K_INGEST, s);
     if (ix->wtype == GS_W_F32)
         k_ingest<GS_W_F32><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                   use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                   use_head ? ix->H : 0, ix->xslot, h_x, qb->xpair, qb->xcnt, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                    qb->tail_w, qb->tail_cnt, qb->tail32, qb->status);
     else
         k_ingest<GS_W_U8><<<grid, threads, 0, s>>>(q->indptr, q->term_ids, q->weights, B, ix->V, ix->head_slot,
-                                                  use_head ? ix->H : 0, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
+                                                  use_head ? ix->H : 0, ix->xslot, h_x, qb->xpair, qb->xcnt, validate, qb->head_pair, qb->head_cnt, qb->tail_term,
                                                   qb->tail_w, qb->tail_cnt, qb->tail32, qb->status);
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());

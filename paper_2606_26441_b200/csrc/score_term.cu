@@ -58,6 +58,7 @@ struct TermParams {
     // queries
     const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
     const uint32_t* tail_w; const int32_t* tail_cnt; const uint2* tail32;
+    const void* xstrip; const uint2* xpair; const int32_t* xcnt;      // second-tier strips (null when the batch has none)
     int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
     int32_t warps;                              // cell rows (warps) per CTA (small-batch kernel)
     int32_t chunk, n_chunks;                    // staged kernel: queries per CTA, CTAs per doc tile
@@ -236,6 +237,32 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                 sc[r][1] = Num<WT>::mac(sc[r][1], q, Num<WT>::from_bits(v[r].y));
                 sc[r][2] = Num<WT>::mac(sc[r][2], q, Num<WT>::from_bits(v[r].z));
                 sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
+            }
+        }
+        if (p.xcnt != nullptr) {                // second-tier strips, from global memory
+            const int nx = p.xcnt[b];
+            const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
+            const W* __restrict__ gx = reinterpret_cast<const W*>(p.xstrip) + base;
+            for (int i = 0; i < nx; ++i) {
+                const uint2 e = __ldg(xl + i);
+                const A q = Num<WT>::qw(e.y);
+                const W* src = gx + (size_t)e.x * (size_t)p.N_pad + 4 * (dq0 + lane);
+#pragma unroll
+                for (int r = 0; r < kQuadRounds; ++r) {
+                    if (whole || dq0 + 32 * r + lane < quads) {
+                        int4 v;
+                        if (WT == GS_W_F32) {
+                            v = __ldg(reinterpret_cast<const int4*>(src + 128 * r));
+                        } else {
+                            const uchar4 u = __ldg(reinterpret_cast<const uchar4*>(src + 128 * r));
+                            v = make_int4(u.x, u.y, u.z, u.w);
+                        }
+                        sc[r][0] = Num<WT>::mac(sc[r][0], q, Num<WT>::from_bits(v.x));
+                        sc[r][1] = Num<WT>::mac(sc[r][1], q, Num<WT>::from_bits(v.y));
+                        sc[r][2] = Num<WT>::mac(sc[r][2], q, Num<WT>::from_bits(v.z));
+                        sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v.w));
+                    }
+                }
             }
         }
         if (!filter) {
@@ -589,6 +616,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
         }
         const int nh = cur.cnt_nh >> 16, cnt = cur.cnt_nh & 0xFFFF;
+        const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
         const uint64_t thr = cur.thr;
 
 #pragma unroll
@@ -640,6 +668,25 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                     acc[r][1] = fma_f32x2(v[r].y, q2, acc[r][1]);
                 }
             }
+            if (nx > 0) {                          // second-tier strips: same contraction, the strip read from global memory
+                const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
+                const float* gx = reinterpret_cast<const float*>(p.xstrip) + (size_t)base + 4 * lane;
+#pragma unroll 1
+                for (int i = 0; i < nx; ++i) {
+                    const uint2 e = __ldg(xl + i);
+                    const float qf = __uint_as_float(e.y);
+                    const unsigned long long q2 = pack_f32x2(qf, qf);
+                    const ulonglong2* src = reinterpret_cast<const ulonglong2*>(gx + (size_t)e.x * (size_t)p.N_pad);
+                    ulonglong2 v[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) v[r] = __ldg(src + 32 * r);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        acc[r][0] = fma_f32x2(v[r].x, q2, acc[r][0]);
+                        acc[r][1] = fma_f32x2(v[r].y, q2, acc[r][1]);
+                    }
+                }
+            }
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 unpack_f32x2(acc[r][0], sc[r][0], sc[r][1]);
@@ -663,6 +710,24 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 for (int r = 0; r < 4; ++r) {
                     sc[r][0] += qi * (int32_t)v[r].x; sc[r][1] += qi * (int32_t)v[r].y;
                     sc[r][2] += qi * (int32_t)v[r].z; sc[r][3] += qi * (int32_t)v[r].w;
+                }
+            }
+            if (nx > 0) {
+                const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
+                const uint8_t* gx = reinterpret_cast<const uint8_t*>(p.xstrip) + (size_t)base + 4 * lane;
+#pragma unroll 1
+                for (int i = 0; i < nx; ++i) {
+                    const uint2 e = __ldg(xl + i);
+                    const int32_t qi = (int32_t)e.y;
+                    const uchar4* src = reinterpret_cast<const uchar4*>(gx + (size_t)e.x * (size_t)p.N_pad);
+                    uchar4 v[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) v[r] = __ldg(src + 32 * r);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        sc[r][0] += qi * (int32_t)v[r].x; sc[r][1] += qi * (int32_t)v[r].y;
+                        sc[r][2] += qi * (int32_t)v[r].z; sc[r][3] += qi * (int32_t)v[r].w;
+                    }
                 }
             }
         }
@@ -749,6 +814,10 @@ static inline bool cta_per_tile(const gs_index* ix, int64_t nq) {
 
 }  // namespace
 
+bool gs_score_term_wants_x(const gs_index* ix, int64_t nq, int group, bool use_head) {
+    return group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->HX > 0 && ix->Ts == kBT && ix->seg2 != nullptr;
+}
+
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
     if (group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->Ts == kBT && ix->seg2 != nullptr)
         return kBWarps;                                                 // batch kernel
@@ -765,6 +834,7 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
     p.ntiles = ix->ntiles;
     p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_term = qb.tail_term;
     p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt; p.tail32 = qb.tail32;
+    p.xstrip = qb.x_on ? ix->xstrip : nullptr; p.xpair = qb.x_on ? qb.xpair : nullptr; p.xcnt = qb.x_on ? qb.xcnt : nullptr;
     p.q0 = q0; p.nq = (int32_t)nq;
     p.warps = norm_warps(group);
     p.ts = ts; p.sink = sink;
