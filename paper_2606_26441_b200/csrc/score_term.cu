@@ -119,7 +119,7 @@ constexpr int kQuadRounds = 2;    // rounds of 32 quads (128 documents) a lane k
 
 // One (doc tile, query) cell row, done by one warp.  STAGED: the tile's strips are in shared memory (s_strip, [H][Ts]);
 // otherwise they are read from the global strips.
-template <int WT, bool STAGED>
+template <int WT, bool STAGED, bool XS>
 __device__ __forceinline__ void process_item(const TermParams& p, typename Num<WT>::A* row,
                                              const typename Num<WT>::W* s_strip, int j, int64_t b, int lane) {
     using W = typename Num<WT>::W;
@@ -239,7 +239,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                 sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
             }
         }
-        if (p.xcnt != nullptr) {                // second-tier strips, from global memory
+        if (XS) {                               // second-tier strips, from global memory
             const int nx = p.xcnt[b];
             const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
             const W* __restrict__ gx = reinterpret_cast<const W*>(p.xstrip) + base;
@@ -311,7 +311,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
 }
 
 // small batches: a warp takes ONE cell row; consecutive warps take consecutive queries of the same tile
-template <int WT>
+template <int WT, bool XS>
 __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams p) {
     using A = typename Num<WT>::A;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -321,7 +321,7 @@ __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams 
     const int j = (int)(item / p.nq);                       // position in the tile set
     const int64_t b = p.q0 + (item - (int64_t)j * p.nq);
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * p.Ts;
-    process_item<WT, false>(p, row, nullptr, j, b, lane);
+    process_item<WT, false, XS>(p, row, nullptr, j, b, lane);
 }
 
 // batches: a CTA of kWarpsStaged warps takes ONE doc tile and a chunk of up to p.chunk queries; it stages the tile's
@@ -330,7 +330,7 @@ __global__ void __launch_bounds__(kWarpsMax * 32) k_score_term(const TermParams 
 // chunk's queries on its own, with no barrier after the staging.
 constexpr int kWarpsStaged = 32;
 
-template <int WT>
+template <int WT, bool XS>
 __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(const TermParams p) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(cons
     __syncthreads();
     const int q_end = min(p.nq, (chunk + 1) * p.chunk);
     for (int q = chunk * p.chunk + warp; q < q_end; q += kWarpsStaged)
-        process_item<WT, true>(p, rows + (size_t)warp * Ts, s_strip, j, p.q0 + q, lane);
+        process_item<WT, true, XS>(p, rows + (size_t)warp * Ts, s_strip, j, p.q0 + q, lane);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -777,20 +777,25 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
 
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
-template <int WT>
-gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged, cudaStream_t s) {
+template <int WT, bool XS>
+gs_status_t launch_x(const TermParams& p, unsigned grid, size_t smem, bool staged, cudaStream_t s) {
     if (staged) {
-        GS_CUDA(cudaFuncSetAttribute(k_score_term_staged<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GS_CUDA(cudaFuncSetAttribute(k_score_term_staged<WT, XS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term_staged<WT><<<grid, kWarpsStaged * 32, smem, s>>>(p);
+        k_score_term_staged<WT, XS><<<grid, kWarpsStaged * 32, smem, s>>>(p);
     } else {
-        GS_CUDA(cudaFuncSetAttribute(k_score_term<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GS_CUDA(cudaFuncSetAttribute(k_score_term<WT, XS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term<WT><<<grid, p.warps * 32, smem, s>>>(p);
+        k_score_term<WT, XS><<<grid, p.warps * 32, smem, s>>>(p);
     }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
     return GS_OK;
+}
+// the second-tier strip loop is compiled in only when the batch carries x lists (it costs the small kernel 16 registers)
+template <int WT>
+gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged, cudaStream_t s) {
+    return p.xcnt != nullptr ? launch_x<WT, true>(p, grid, smem, staged, s) : launch_x<WT, false>(p, grid, smem, staged, s);
 }
 
 // From how many queries on the CTA-per-doc-tile kernels are used.  Batch sweep on B200 (ms per batch, warp-per-row shape vs
