@@ -491,6 +491,9 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
     else:
         # not HBM bound by construction: the roof is the shared-memory pipeline.  HBM figures kept beside it.
         hbm = rf.term_parallel_bytes(ts["U"], wtype, share)
+        # batch kernel: the second tier of dense strips is read in full (w bytes per document per strip) on top of the postings
+        x_strips = info["head_terms_term_parallel"] - info["head_terms"] if st["query_group"] >= 32 else 0
+        hbm += rf.weight_bytes(wtype) * float(info["num_docs"]) * x_strips * (1.0 + share)
         ht = rf.head_tail_work(lens, queries.terms, head_terms)
         alg = rf.term_parallel_smem_bytes(ht["W_head"], ht["W_tail"], info["num_tiles"] * B, info["tile_docs"], share)
         peak = rf.smem_peak_gbs(peaks["sm_max_mhz"])
@@ -498,7 +501,7 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
                     "peak_source": f"derived: 148 SMs x 128 B/clk shared memory x {peaks['sm_max_mhz']:.0f} MHz (B200_PROFILING.md unit counts and clocks)",
                     "cell_rows_per_cta": st["query_group"], "bytes_per_step": alg, "W_head": ht["W_head"], "W_tail": ht["W_tail"],
                     "bytes_model": "shared-memory traffic: (4*W_head + 8*W_tail + 8*Ts*tiles*B)*(1+sample share)",
-                    "hbm_bytes_per_step": hbm, "hbm_bytes_model": "(4+w)*U*(1+sample share), U=postings of distinct batch terms",
+                    "hbm_bytes_per_step": hbm, "hbm_bytes_model": "((4+w)*U + w*N*x_strips)*(1+sample share), U=postings of distinct batch terms, x_strips=second-tier strips (batch kernel)", "x_strips": x_strips,
                     "hbm_achieved": rf.effective_gbps(hbm, kms), "hbm_frac": rf.effective_gbps(hbm, kms) / peaks["hbm_gbs"],
                     "hbm_bytes_paper_model": rf.term_parallel_bytes(ts["W"], wtype)})
         out["achieved"] = rf.effective_gbps(alg, kms)
