@@ -9,10 +9,10 @@
 #define GS_STRIP_MAX 64         // dense strips kept by the index
 #define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
 #ifndef GS_XSTRIP_MAX
-#define GS_XSTRIP_MAX 64
+#define GS_XSTRIP_MAX 128
 #endif
 #ifndef GS_XDENS
-#define GS_XDENS 0.10f
+#define GS_XDENS 0.05f
 #endif
 // GS_XSTRIP_MAX: second tier of dense strips, read from global memory by the term-parallel kernels only
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
@@ -71,7 +71,7 @@ struct gs_index {
     int32_t head_terms_host[GS_STRIP_MAX];
     int16_t* head_slot = nullptr;    // [V]: strip number of a term or -1
     void* head_strip = nullptr;      // [H][N_pad] float | uint8 (0 where the doc is not in the list)
-    // second tier ("x strips"): the next densest lists (density >= 0.10), a dense copy used by the term-parallel kernels
+    // second tier ("x strips"): the next densest lists (up to 128 of density >= 0.05), a dense copy used by the term-parallel kernels
     // only — there they replace the scatter of a 50-130-posting segment per doc tile by four 128-bit loads and eight
     // FFMA2; the lists stay tail terms everywhere else (forward index, document-parallel kernel)
     int32_t HX = 0;

@@ -380,10 +380,10 @@ constexpr int kBT = 512;          // documents per tile
 #define GS_BWARPS 32
 #endif
 #ifndef GS_ROUNDS
-#define GS_ROUNDS 2
+#define GS_ROUNDS 1
 #endif
 #ifndef GS_HEAD_UNROLL
-#define GS_HEAD_UNROLL 2
+#define GS_HEAD_UNROLL 4
 #endif
 constexpr int kBWarps = GS_BWARPS;   // warps (cell rows in flight) per CTA
 constexpr int kRounds = GS_ROUNDS;   // flat posting rounds whose loads are issued together
