@@ -799,14 +799,14 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged,
 }
 
 // From how many queries on the CTA-per-doc-tile kernels are used.  Batch sweep on B200 (ms per batch, warp-per-row shape vs
-// batch kernel): 8.8M docs 64: 3.87 / 4.01, 96: 5.58 / 5.33, 128: 7.23 / 6.64, 256: 13.7 / 11.8, 500: 25.9 / 20.9;
-// 1M docs 128: 1.03 / 1.09, 192: 1.48 / 1.53, 256: 1.85 / 1.83, 500: 3.40 / 3.19 — the fixed cost of a CTA (staging, first-row
-// probes) is amortised over fewer rows when the collection has few doc tiles.
+// batch kernel): 8.8M docs 48: 3.03 / 3.19, 64: 3.89 / 3.37, 128: 7.25 / 5.51, 256: 13.7 / 9.49, 500: 25.9 / 16.6;
+// 1M docs 64: 0.61 / 0.62, 96: 0.84 / 0.88, 128: 1.04 / 0.98, 256: 1.87 / 1.53, 500: 3.41 / 2.59 — the fixed cost of a CTA
+// (staging, first-row probes) is amortised over fewer rows when the collection has few doc tiles.
 #ifndef GS_STAGED_MIN
-#define GS_STAGED_MIN 256
+#define GS_STAGED_MIN 128
 #endif
 constexpr int kStagedMinQueries = GS_STAGED_MIN;
-constexpr int kStagedMinQueriesLarge = GS_STAGED_MIN < 96 ? GS_STAGED_MIN : 96;     // collections of >= kLargeTiles doc tiles
+constexpr int kStagedMinQueriesLarge = GS_STAGED_MIN < 64 ? GS_STAGED_MIN : 64;     // collections of >= kLargeTiles doc tiles
 constexpr int kLargeTiles = 8192;
 constexpr int kStagedChunk = 512;         // most queries per CTA of the staged / batch kernels
 #ifndef GS_CHUNK_WAVES

@@ -430,7 +430,7 @@ BATCH_KERNEL_WARPS = 32   # kBWarps of score_term.cu
 @pytest.mark.parametrize("qcfg", ["mid", "skew_b32"])
 @pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=5), dict(head_max=-1), dict(tile_docs=1024, head_density=0.05)])
 def test_batch_of_256_takes_the_cta_per_tile_term_kernels(gs, mode, build_kw, qcfg):
-    """From 256 queries on (96 on collections of at least 8192 doc tiles) the term-parallel kernel runs as a persistent CTA per doc tile with the strips staged in shared
+    """From 128 queries on (64 on collections of at least 8192 doc tiles) the term-parallel kernel runs as a persistent CTA per doc tile with the strips staged in shared
     memory (unless the index has no strips) — the batch kernel on 512-doc tiles, the generic staged kernel on other tile sizes:
     every score of 256 queries x 20 011 docs, and the top-50, against the oracle.  The "skew_b32" queries (5..256 terms,
     Zipf 1.3) have more than 32 tail terms, which the batch kernel probes in line after the prefetched first 32."""
