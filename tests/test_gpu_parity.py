@@ -455,6 +455,31 @@ def test_batch_of_256_takes_the_cta_per_tile_term_kernels(gs, mode, build_kw, qc
     ix.close()
 
 
+@pytest.mark.parametrize("mode", ["f32", "u8"])
+def test_candidate_overflow_of_a_batch_falls_back_to_the_dense_path_with_second_tier_strips(gs, mode):
+    """130 queries over 200 000 docs built so that the threshold sample (every 64th doc tile at this N and k) sees none of the
+    high-scoring documents: every candidate list overflows and the queries are re-run through the dense path in sub-batches
+    (the warp-per-row kernel) while the batch still carries its second-tier strip lists (term 1: density 0.2).  Exact
+    against the oracle."""
+    n = 200_000
+    dt = np.float32 if mode == "f32" else np.uint8
+    d = np.arange(n)
+    has1, has2 = (d % 5 == 3) & ((d // 512) % 64 != 0), d % 50 == 7
+    nnz = 1 + has1.astype(np.int64) + has2.astype(np.int64)
+    indptr = np.concatenate([[0], np.cumsum(nnz)]).astype(np.int64)
+    terms = np.zeros(indptr[-1], np.int32)
+    terms[indptr[:-1][has1] + 1] = 1
+    terms[indptr[1:][has2] - 1] = 2
+    docs = wl.Csr(indptr, terms, np.ones(indptr[-1], dt))
+    queries = csr_from_dicts([{0: 1, 1: 1, 2: 1 + (b % 3)} for b in range(130)], dt)
+    ix = gs.Index.from_numpy(docs, 8)
+    assert ix.info()["head_terms_term_parallel"] > ix.info()["head_terms"]          # term 1 is a second-tier strip
+    ids, sc = gpu_search(gs, ix, queries, 50, algo="term")
+    assert ix.stats()["overflow_queries"] > 0
+    compare(gs, docs, queries, 8, 50, ids, sc)
+    ix.close()
+
+
 def test_batch_kernel_is_deterministic_run_to_run(gs):
     """DESIGN.md R2: every (query, doc) cell is owned by one warp and its additions keep the query's term order, so the fp32
     scores of the batch kernel are bitwise identical from run to run (the candidate lists are not ordered, the results are)."""
