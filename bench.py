@@ -392,9 +392,35 @@ def run_ours(args):
         if args.suite and world == 1:
             line["suite"] = {name: suite_entry(torch, gs, wl, name, args, peaks)
                              for name in ("tiny", "mid", "paper_u8", "skew_b1", "skew_b32")}
+            line["sparsity_sweep"] = sparsity_sweep(torch, gs, wl)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def sparsity_sweep(torch, gs, wl):
+    """Analogue of the paper's synthetic sparsity sweep (Table 5: 500K docs, 64 queries, mean doc nnz
+    10..500; the paper does not state its generator, so only the shape is comparable): ms per 64-query batch of both kernels,
+    top-10, docs from the seeded generator with nnz ~ N(m, m/3) clipped to [m/6, 4m]."""
+    dev = torch.device("cuda:0")
+    queries = wl.make_queries("mid", n_queries=64)
+    q_dev = [torch.from_numpy(a).to(dev) for a in (queries.indptr, queries.terms, queries.weights)]
+    out = []
+    for m in (10, 50, 120, 250, 500):
+        docs = wl.make_rows(500_000, seed=0, stream=wl.STREAM_DOCS, vocab=wl.VOCAB, zipf_s=1.1, nnz_law=wl.NNZ_NORMAL,
+                            mu=float(m), sigma=m / 3.0, lo=max(1, m // 6), hi=4 * m)
+        ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev)
+        row = {"mean_doc_nnz": m, "postings": int(docs.indptr[-1])}
+        for algo in ("term", "doc"):
+            ws = torch.empty(ix.workspace_bytes(64, queries.nnz, 10, algo=algo), dtype=torch.uint8, device=dev)
+            oi = torch.empty((64, 10), dtype=torch.int32, device=dev)
+            osc = torch.empty((64, 10), dtype=torch.float32, device=dev)
+            ms = timed_steps(torch, None, lambda: ix.search(*q_dev, 10, out_ids=oi, out_scores=osc, workspace=ws, algo=algo), 5, 3, 1)
+            row[algo + "_ms_per_batch"] = ms / 5
+            del ws
+        ix.close()
+        out.append(row)
+    return out
 
 
 def suite_entry(torch, gs, wl, name, args, peaks):
