@@ -110,7 +110,8 @@ typedef struct gs_info {
     int64_t bytes_head;        /* dense strips                                                        */
     int64_t bytes_total;
     int64_t forward_tail_nnz;  /* postings held by the CSR part of the forward index                  */
-    int32_t head_terms_term_parallel; /* strips the term-parallel kernel reads (= head_terms)          */
+    int32_t head_terms_term_parallel; /* strips the term-parallel kernels can read: head_terms + the second tier (up to
+                                       * 128 more lists of density >= 0.05, 512-doc tiles only; bytes in bytes_head) */
     int32_t reserved;
     int64_t forward_padded_nnz; /* slots of the CSR part: forward_tail_nnz + block padding             */
 } gs_info_t;
