@@ -518,26 +518,24 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     using A = typename Num<WT>::A;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int j = (int)(blockIdx.x / p.n_chunks);
-    const int chunk = (int)(blockIdx.x - (unsigned)j * p.n_chunks);
-    const int tile = p.ts.first + j * p.ts.stride;
-    const int32_t base = tile * kBT;
     // shared memory: rows [kBWarps][kBT] | descriptors [kBWarps][32] uint2 | candidate keys [kBWarps][kWarpBuf] u64 |
-    // candidate queries [kBWarps][kWarpBuf] u16 | counters [kBWarps] + query counter | strips [H][kBT]
+    // candidate queries [kBWarps][kWarpBuf] u16 | counters (per-warp candidate counts, query counters and "warps done"
+    // counters of the even / odd work items) | mbarrier | strips [H][kBT]
     constexpr size_t kOffDesc = (size_t)kBWarps * kBT * 4;
     constexpr size_t kOffKey = kOffDesc + (size_t)kBWarps * 32 * 8;
     constexpr size_t kOffQ = kOffKey + (size_t)kCandBuf * 8;
     constexpr size_t kOffCnt = kOffQ + (size_t)kCandBuf * 2;
-    constexpr size_t kOffStrip = kOffCnt + (size_t)(kBWarps + 4) * 4;
+    constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;
+    constexpr size_t kOffStrip = kOffBar + 16;
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
     const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
     uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey) + warp * kWarpBuf;     // the warp's candidate buffer
     uint16_t* w_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ) + warp * kWarpBuf;
     uint32_t* w_cnt = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + warp;
-    uint32_t* s_next = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + kBWarps;
+    uint32_t* s_next = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + kBWarps;           // [2]
+    uint32_t* s_done = s_next + 2;                                                            // [2]
     W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
-    if (lane == 0) *w_cnt = 0u;
-    if (threadIdx.x == 0) *s_next = 2u * kBWarps;
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffBar);
     // the warp appends its buffered candidates to the queries' lists (all the atomics of a round in flight together)
     auto flush = [&]() {
         __syncwarp();
@@ -557,7 +555,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             const int start = 31 - __clz((int)(heads & le_));                 // first lane of this lane's run
             const unsigned later = heads & ~le_;
             const int end = later ? __ffs((int)later) - 1 : n_valid;          // one past the run's last lane
-            const int64_t bb = p.q0 + (int64_t)chunk * p.chunk + (valid ? qi : 0u);
+            const int64_t bb = p.q0 + (valid ? (int64_t)qi : 0);
             uint32_t pos = 0;
             if (head) pos = atomicAdd(&p.sink.cand_cnt[bb], (uint32_t)(end - lane));
             pos = __shfl_sync(0xFFFFFFFFu, pos, start & 31) + (uint32_t)(lane - start);
@@ -567,24 +565,51 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         if (lane == 0) *w_cnt = 0u;
         __syncwarp();
     };
-    // The tile's strips come in by TMA: one thread issues a 1-D bulk copy per strip (kBT weights, contiguous in the strip)
-    // that completes on an mbarrier; a warp waits for it only before its first head phase, so the copy runs under the
-    // probes and the tail scatter of every warp's first row.
-    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffCnt + (size_t)(kBWarps + 2) * 4);
-    if (threadIdx.x == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_s) : "memory");
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    // A work item = (doc tile, chunk of queries).  The CTA is persistent: it takes items blockIdx.x, blockIdx.x + gridDim.x, ...
+    // The item's strips come in by TMA: one thread issues a 1-D bulk copy per strip (kBT weights, contiguous in the
+    // strip) that completes on an mbarrier (one phase per item); a warp waits for it only before its first head phase.
+    // A warp that finds no more rows in the item moves on to the next item's probes and tail scatter at once; the LAST
+    // warp out of an item (shared-memory counter) starts the copy of the next item's strips — nobody reads the old ones
+    // any more — so the copy, the item prologue and the slow warps' last rows overlap with the other warps' work.
+    const int n_items = p.ts.count * p.n_chunks;
+    auto issue_strips = [&](int item) {                 // one thread
+        const int tile_ = p.ts.first + (item / p.n_chunks) * p.ts.stride;
         const uint32_t row_bytes = (uint32_t)(kBT * sizeof(W));
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_s), "r"(row_bytes * (uint32_t)p.H) : "memory");
-        const W* g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile * kBT;
+        const W* g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile_ * kBT;
         const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_strip);
         for (int h = 0; h < p.H; ++h)
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                          ::"r"(dst + (uint32_t)h * row_bytes), "l"(g + (size_t)h * p.N_pad), "r"(row_bytes), "r"(mbar_s) : "memory");
+    };
+    if (lane == 0) *w_cnt = 0u;
+    if (threadIdx.x == 0) {
+        s_next[0] = s_next[1] = 2u * kBWarps;
+        s_done[0] = s_done[1] = 0u;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_s) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    bool strips_ready = false;
+    __syncthreads();
+    if (threadIdx.x == 0 && (int)blockIdx.x < n_items) issue_strips((int)blockIdx.x);
     const bool filter = p.sink.thr != nullptr;
+    const W* srow = s_strip + 4 * lane;
+    int it = 0;
+    for (int item = (int)blockIdx.x; item < n_items; item += (int)gridDim.x, ++it) {
+    const int par = it & 1;
+    const int j = item / p.n_chunks;
+    const int chunk = item - j * p.n_chunks;
+    const int tile = p.ts.first + j * p.ts.stride;
+    const int32_t base = tile * kBT;
+    bool strips_ready = false;
+    auto wait_strips = [&]() {                          // the bulk copies of this item's strips have landed
+        uint32_t ok = 0;
+        do {
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(ok) : "r"(mbar_s), "r"((uint32_t)par) : "memory");
+        } while (!ok);
+        strips_ready = true;
+    };
     // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
     // warp and warp + kBWarps of the chunk and claims further ones from a shared-memory counter, two rows ahead of the
     // row it works on (the probes of the next two rows are in flight).
@@ -597,14 +622,12 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     Probe2 s2{0u, 0u, 0u, 0, 0ull};
     if (q < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile); probe_query(p, p.q0 + q, filter, s2); }
     if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
-    __syncthreads();
     {
         int c = 0;
-        if (lane == 0) c = (int)atomicAdd(s_next, 1u);
+        if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
         q_n2 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;
     }
     const int n_live = (int)min((int64_t)kBT, p.N - (int64_t)base);                    // documents of this tile that exist
-    const W* srow = s_strip + 4 * lane;
     for (; q < q_end; q = q_n1, q_n1 = q_n2, q_n2 = q_n3) {
         const int64_t b = p.q0 + q;
         const Probe2 cur = s2;
@@ -612,7 +635,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         if (q_n2 < q_end) s1 = probe_terms(p, p.q0 + q_n2, lane);
         {
             int c = 0;
-            if (lane == 0) c = (int)atomicAdd(s_next, 1u);
+            if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
             q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
         }
         const int nh = cur.cnt_nh >> 16, cnt = cur.cnt_nh & 0xFFFF;
@@ -635,14 +658,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         }
         __syncwarp();
 
-        if (!strips_ready) {                        // once per warp: the bulk copies of the tile's strips have landed
-            uint32_t ok = 0;
-            do {
-                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                             : "=r"(ok) : "r"(mbar_s) : "memory");
-            } while (!ok);
-            strips_ready = true;
-        }
+        if (!strips_ready) wait_strips();           // once per warp and item
         // head strips: the lane's 16 documents (quads lane, lane+32, lane+64, lane+96) stay in registers
         const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
         A sc[4][4];
@@ -760,7 +776,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                         const uint32_t slot = atomicAdd(w_cnt, 1u);
                         if (slot < (uint32_t)kWarpBuf) {
                             w_key[slot] = key;
-                            w_q[slot] = (uint16_t)(q - chunk * p.chunk);
+                            w_q[slot] = (uint16_t)q;
                         } else {                                         // buffer full: append directly
                             const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
                             if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
@@ -771,6 +787,20 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         }
         __syncwarp();
         if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt) flush();
+    }
+    // out of rows in this item.  Every warp observes every phase of the mbarrier (a warp without rows too: a wait for the
+    // NEXT phase issued while this one is still pending would be satisfied at once), then reports itself done.
+    if (!strips_ready) wait_strips();
+    __syncwarp();
+    if (lane == 0) {
+        __threadfence_block();
+        if (atomicAdd(s_done + par, 1u) == (uint32_t)(kBWarps - 1)) {       // last warp out: the strips buffer is free
+            s_done[par] = 0u;
+            s_next[par] = 2u * kBWarps;                                    // for the item after the next
+            if (item + (int)gridDim.x < n_items) issue_strips(item + (int)gridDim.x);
+        }
+    }
+    __syncwarp();
     }
     if (filter) flush();
 }
@@ -863,12 +893,13 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
         p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4;
-        if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max) {
+        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 16;
+        if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max && nq <= 65535) {
             auto go = [&](auto kern) -> gs_status_t {
                 GS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch));
                 GsProfScope ps(GS_K_SCORE_TERM, s);
-                kern<<<(unsigned)grid, kBWarps * 32, smem_batch, s>>>(p);
+                // persistent: one CTA per SM walks the (doc tile, query chunk) items
+                kern<<<(unsigned)std::min<int64_t>(grid, sms), kBWarps * 32, smem_batch, s>>>(p);
                 ++gs_tls_launches;
                 GS_CUDA(cudaGetLastError());
                 return GS_OK;
