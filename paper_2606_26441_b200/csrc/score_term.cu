@@ -388,6 +388,10 @@ constexpr int kBT = 512;          // documents per tile
 constexpr int kBWarps = GS_BWARPS;   // warps (cell rows in flight) per CTA
 constexpr int kRounds = GS_ROUNDS;   // flat posting rounds whose loads are issued together
 constexpr int kHeadUnroll = GS_HEAD_UNROLL;
+#ifndef GS_X_UNROLL
+#define GS_X_UNROLL 1
+#endif
+constexpr int kXUnroll = GS_X_UNROLL;     // second-tier strip terms whose loads are issued together
 
 __device__ __forceinline__ unsigned long long pack_f32x2(float lo, float hi) {
     unsigned long long d;
@@ -687,7 +691,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (nx > 0) {                          // second-tier strips: same contraction, the strip read from global memory
                 const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
                 const float* gx = reinterpret_cast<const float*>(p.xstrip) + (size_t)base + 4 * lane;
-#pragma unroll 1
+#pragma unroll kXUnroll
                 for (int i = 0; i < nx; ++i) {
                     const uint2 e = __ldg(xl + i);
                     const float qf = __uint_as_float(e.y);
