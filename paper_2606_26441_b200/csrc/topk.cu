@@ -13,6 +13,10 @@
 
 #include "gs_internal.cuh"
 
+#ifndef GS_SEL_TARGET
+#define GS_SEL_TARGET 128     // CTAs a select launch aims for before it stops splitting rows over clusters
+#endif
+
 namespace {
 
 constexpr int kSelThreads = 512;
@@ -413,7 +417,7 @@ gs_status_t run_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* 
         GS_CUDA(cudaFuncSetAttribute(k_sel_row<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         // CTAs per row: enough to spread a few rows over the chip, one when there are rows to spare
         int C = 1;
-        while (C < 8 && rows * C < 128 && max_items > (int64_t)C * 8192) C <<= 1;
+        while (C < 8 && rows * C < GS_SEL_TARGET && max_items > (int64_t)C * 8192) C <<= 1;
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3((unsigned)(rows * C));
         cfg.blockDim = dim3(kRowThreads);
