@@ -721,16 +721,17 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
 #pragma unroll kHeadUnroll
             for (int i = 0; i < nh; ++i) {
                 const uint2 e = __ldg(hl + i);
-                const int32_t qi = (int32_t)e.y;
-                const uchar4* src = reinterpret_cast<const uchar4*>(srow + (size_t)e.x * kBT);
-                uchar4 v[4];
+                // one IDP4A per cell: the impact byte of the query (<= 255) placed in byte u of the second operand picks
+                // byte u of the strip word — no unpacking
+                const uint32_t qi = e.y & 0xFFu;
+                const uint32_t* src = reinterpret_cast<const uint32_t*>(srow + (size_t)e.x * kBT);
+                uint32_t v[4];
 #pragma unroll
                 for (int r = 0; r < 4; ++r) v[r] = src[32 * r];
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    sc[r][0] += qi * (int32_t)v[r].x; sc[r][1] += qi * (int32_t)v[r].y;
-                    sc[r][2] += qi * (int32_t)v[r].z; sc[r][3] += qi * (int32_t)v[r].w;
-                }
+                for (int r = 0; r < 4; ++r)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) sc[r][u] = (int32_t)__dp4a(v[r], qi << (8 * u), (uint32_t)sc[r][u]);
             }
             if (nx > 0) {
                 const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
@@ -738,16 +739,15 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
 #pragma unroll 1
                 for (int i = 0; i < nx; ++i) {
                     const uint2 e = __ldg(xl + i);
-                    const int32_t qi = (int32_t)e.y;
-                    const uchar4* src = reinterpret_cast<const uchar4*>(gx + (size_t)e.x * (size_t)p.N_pad);
-                    uchar4 v[4];
+                    const uint32_t qi = e.y & 0xFFu;
+                    const uint32_t* src = reinterpret_cast<const uint32_t*>(gx + (size_t)e.x * (size_t)p.N_pad);
+                    uint32_t v[4];
 #pragma unroll
                     for (int r = 0; r < 4; ++r) v[r] = __ldg(src + 32 * r);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        sc[r][0] += qi * (int32_t)v[r].x; sc[r][1] += qi * (int32_t)v[r].y;
-                        sc[r][2] += qi * (int32_t)v[r].z; sc[r][3] += qi * (int32_t)v[r].w;
-                    }
+                    for (int r = 0; r < 4; ++r)
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) sc[r][u] = (int32_t)__dp4a(v[r], qi << (8 * u), (uint32_t)sc[r][u]);
                 }
             }
         }
