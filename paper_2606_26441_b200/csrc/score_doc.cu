@@ -57,7 +57,8 @@ struct ConstTile {
     uint32_t hl[GS_STRIP_MAX];           // compact position -> strip number (0 beyond nh)
     uint32_t thr_s[kMaxQT];              // threshold as a score (accumulator bits); "accept all" = NaN / INT32_MIN
     unsigned long long thr_key[kMaxQT];  // threshold as a key; queries beyond the tile: all ones
-    uint32_t qh[GS_STRIP_MAX * kMaxQT];  // [compact strip][QT] accumulator-typed head weights, row stride QT
+    uint32_t qh[GS_STRIP_MAX * kMaxQT];  // f32: [compact strip][QT] head weights, row stride QT; u8: [strip / 4][QT] words of
+                                         // four impact bytes (strips 4g .. 4g+3 of query q)
 };
 __constant__ ConstTile c_tile;
 
@@ -245,7 +246,9 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                 const uint32_t below = hs < 32 ? (s_hmask[0] & ((1u << hs) - 1u))
                                                : (s_hmask[1] & ((1u << (hs - 32)) - 1u));
                 const int ci = __popc(below) + (hs >= 32 ? __popc(s_hmask[0]) : 0);
-                ct->qh[(size_t)ci * QT + j] = w;
+                if (WT == GS_W_F32) ct->qh[(size_t)ci * QT + j] = w;
+                else                                       // impacts: byte (ci & 3) of word [ci / 4][j] — four strips per IDP4A
+                    reinterpret_cast<uint8_t*>(ct->qh)[((size_t)(ci >> 2) * QT + j) * 4 + (ci & 3)] = (uint8_t)w;
             } else {
                 const uint32_t word = bm[t >> 5];
                 const uint32_t r = pre[t >> 5] + __popc(word & ((1u << (t & 31)) - 1u));
@@ -341,17 +344,16 @@ __device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ mya
         A acc[QT];
 #pragma unroll
         for (int q = 0; q < QT; ++q) acc[q] = myacc[q];
+        // integer impacts: the document's bytes of four strips packed into one word, the tile's weights of the same four
+        // strips packed per query (k_build_qtile): one IDP4A per (four strips, query)
 #pragma unroll 1
         for (int i0 = 0; i0 < nh; i0 += 4) {
-            A x[4];
+            uint32_t x4 = 0;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) x[u] = NumD<WT>::widen(sp[(size_t)c_tile.hl[i0 + u] * N_pad]);
+            for (int u = 0; u < 4; ++u) x4 |= (uint32_t)sp[(size_t)c_tile.hl[i0 + u] * N_pad] << (8 * u);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-#pragma unroll
-                for (int q = 0; q < QT; ++q)
-                    acc[q] = NumD<WT>::mac(acc[q], NumD<WT>::from_bits(c_tile.qh[(i0 + u) * QT + q]), x[u]);
-            }
+            for (int q = 0; q < QT; ++q)
+                acc[q] = (A)__dp4a(x4, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
         }
 #pragma unroll
         for (int q = 0; q < QT; ++q) myacc[q] = acc[q];
