@@ -223,9 +223,9 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                     if (WT == GS_W_F32) {
                         v[r] = STAGED ? *reinterpret_cast<const int4*>(src + 128 * r) : __ldg(reinterpret_cast<const int4*>(src + 128 * r));
                     } else {
-                        const uchar4 u = STAGED ? *reinterpret_cast<const uchar4*>(src + 128 * r)
-                                                : __ldg(reinterpret_cast<const uchar4*>(src + 128 * r));
-                        v[r] = make_int4(u.x, u.y, u.z, u.w);
+                        // impacts: the four bytes stay packed in v[r].x; one IDP4A per cell below picks its byte
+                        v[r].x = (int)(STAGED ? *reinterpret_cast<const uint32_t*>(src + 128 * r)
+                                              : __ldg(reinterpret_cast<const uint32_t*>(src + 128 * r)));
                     }
                 } else {
                     v[r] = make_int4(0, 0, 0, 0);
@@ -233,10 +233,16 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
             }
 #pragma unroll
             for (int r = 0; r < kQuadRounds; ++r) {
-                sc[r][0] = Num<WT>::mac(sc[r][0], q, Num<WT>::from_bits(v[r].x));
-                sc[r][1] = Num<WT>::mac(sc[r][1], q, Num<WT>::from_bits(v[r].y));
-                sc[r][2] = Num<WT>::mac(sc[r][2], q, Num<WT>::from_bits(v[r].z));
-                sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
+                if (WT == GS_W_F32) {
+                    sc[r][0] = Num<WT>::mac(sc[r][0], q, Num<WT>::from_bits(v[r].x));
+                    sc[r][1] = Num<WT>::mac(sc[r][1], q, Num<WT>::from_bits(v[r].y));
+                    sc[r][2] = Num<WT>::mac(sc[r][2], q, Num<WT>::from_bits(v[r].z));
+                    sc[r][3] = Num<WT>::mac(sc[r][3], q, Num<WT>::from_bits(v[r].w));
+                } else {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        sc[r][u] = Num<WT>::from_bits((int)__dp4a((uint32_t)v[r].x, (e.y & 0xFFu) << (8 * u), Num<WT>::bits(sc[r][u])));
+                }
             }
         }
         if (XS) {                               // second-tier strips, from global memory
