@@ -60,7 +60,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-queries", type=int, default=0, help="oracle sample size (0 = one per core)")
     ap.add_argument("--latency-queries", type=int, default=200, help="single-query searches timed for the batch-1 latency leg (0 = skip)")
-    ap.add_argument("--suite", action="store_true", help="also measure BASELINE.json configs 1,2,4,5 (QPS, latency, roofline) into the line's `suite` key")
+    ap.add_argument("--no-suite", action="store_true", help="skip the other BASELINE.json configs (1, 2, 4, 5: QPS, p50/p99, roofline) in the line's `suite` key")
+    ap.add_argument("--sweeps", action="store_true", help="also run the batch-size sweep and the sparsity sweep (PAPER.md Tables 3 / 5 analogues)")
     return ap.parse_args()
 
 
@@ -171,9 +172,17 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+BJ_INDEX = {"tiny": 0, "mid": 1, "paper": 2, "paper_u8": 3, "skew_b1": 4, "skew_b32": 4}
+
+
+def workload_label(name, c, n_docs, B, k):
+    qlaw = "nnz~U{5..256}" if c["qlaw"]["nnz_law"] == 1 else "nnz~N(25,8) clip [5,64]"
+    return (f"BASELINE.json configs[{BJ_INDEX.get(name, '?')}] '{name}': V=30522, N={n_docs} docs (nnz~N(120,40) clip [20,400], "
+            f"Zipf s={c['s']}, LogNormal(0,0.5) {c['wtype']} weights), B={B} queries ({qlaw}, Zipf s={c['s']}), top-k={k}, seed 0")
+
+
 def config_dict(args, c, n_docs, B, k, algo):
-    return {"workload": f"BASELINE.json configs[2] '{args.config}': V=30522, N={n_docs} docs (nnz~N(120,40) clip [20,400], Zipf s={c['s']}, "
-                        f"LogNormal(0,0.5) {c['wtype']} weights), B={B} queries (nnz~N(25,8) clip [5,64]), top-k={k}, seed 0",
+    return {"workload": workload_label(args.config, c, n_docs, B, k),
             "num_docs": n_docs, "batch": B, "k": k, "vocab": 30522, "wtype": c["wtype"], "algo": algo,
             "l2": "index arrays (GBs) exceed the 126 MB L2; no explicit flush between iterations",
             "parallelism": "replicas only (no sharding, no collectives)"}
@@ -230,9 +239,49 @@ def latency_leg(torch, ix, queries, k, n, algo, batch=1, **opt):
         ms.append(e0.elapsed_time(e1))
     st = ix.stats(ws)
     ms = np.array(ms)
-    return {"batch": batch, "calls": int(n), "algo": algo, "algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"),
-            "p50_ms": float(np.percentile(ms, 50)), "p99_ms": float(np.percentile(ms, 99)), "mean_ms": float(ms.mean()),
-            "p50_ms_per_query": float(np.percentile(ms, 50)) / batch}
+    out = {"batch": batch, "calls": int(n), "algo": algo, "algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"),
+           "p50_ms": float(np.percentile(ms, 50)), "p99_ms": float(np.percentile(ms, 99)), "mean_ms": float(ms.mean()),
+           "p50_ms_per_query": float(np.percentile(ms, 50)) / batch,
+           "protocol": "per call: CUDA event, gs_search + gs_search_finish (stream sync + 64 B read-back), CUDA event"}
+    # the same search captured ONCE into a CUDA graph (gs_search is asynchronous) and replayed for every query: the new
+    # query is copied into the captured buffers before the first event, so the timed region is the graph replay alone
+    if st["algo_used"] == 1 and batch <= 32:
+        try:
+            cap = max_nnz
+            g_ip = torch.zeros(batch + 1, dtype=torch.int64, device=dev)
+            g_t = torch.zeros(max(cap, 1), dtype=torch.int32, device=dev)
+            g_w = torch.zeros(max(cap, 1), dtype=slices[0][0][2].dtype, device=dev)
+
+            def put(q):
+                g_ip.copy_(q[0]); g_t[:q[1].numel()].copy_(q[1]); g_w[:q[2].numel()].copy_(q[2])
+
+            put(slices[0][0])
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                ix.search(g_ip, g_t, g_w, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, finish=False, **opt)
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                ix.search(g_ip, g_t, g_w, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, finish=False, **opt)
+            gms, n_ov = [], 0
+            for (q, _) in slices:
+                put(q)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(s)
+                graph.replay()
+                e1.record(s)
+                e1.synchronize()
+                gms.append(e0.elapsed_time(e1))
+                n_ov += ix.stats(ws)["overflow_queries"]
+            gms = np.array(gms)
+            out.update({"graph_p50_ms": float(np.percentile(gms, 50)), "graph_p99_ms": float(np.percentile(gms, 99)),
+                        "graph_overflow_queries": int(n_ov)})
+            del graph
+        except Exception as e:                                   # report, never hide
+            out["graph_error"] = repr(e)[:200]
+    return out
 
 
 def run_ours(args):
@@ -279,8 +328,8 @@ def run_ours(args):
         ws_bytes = ix.workspace_bytes(B, queries.nnz, k, algo=algo, **opt_common)
         ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
 
-        def step():
-            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, **opt_common)
+        def step():      # asynchronous gs_search; the overflow count of the (identical) steps is read after the timed region
+            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, finish=False, **opt_common)
 
         with ClockSampler(local) as cs:
             ms = timed_steps(torch, dist, step, args.steps, args.warmup, world)
@@ -340,11 +389,11 @@ def run_ours(args):
     # ---- batch-1 latency (BASELINE.json metric: "batch-1 p50 ms/query"), both kernels, on the same index
     latency = None
     if world == 1 and args.latency_queries > 0:
-        latency = {a: latency_leg(torch, ix, queries, k, args.latency_queries, a) for a in ("term", "doc")}
+        latency = {a: latency_leg(torch, ix, queries, k, args.latency_queries, a, **opt_common) for a in ("term", "doc")}
 
     # ---- batch-size sweep on the same index (Table 3 L262-271 analogue), with --suite
     sweep = None
-    if world == 1 and args.suite:
+    if world == 1 and args.sweeps:
         sweep = []
         for Bs in (1, 2, 4, 8, 16, 32, 64, 128, 256, B):
             if Bs > B:
@@ -389,9 +438,9 @@ def run_ours(args):
     ix.close()
     del ix, q_dev, out_ids, out_sc
     if rank == 0:
-        if args.suite and world == 1:
-            line["suite"] = {name: suite_entry(torch, gs, wl, name, args, peaks)
-                             for name in ("tiny", "mid", "paper_u8", "skew_b1", "skew_b32")}
+        if not args.no_suite and world == 1 and args.config == "paper" and args.docs is None:
+            line["suite"] = run_suite(torch, gs, wl, args, peaks)
+        if args.sweeps and world == 1:
             line["sparsity_sweep"] = sparsity_sweep(torch, gs, wl)
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -423,50 +472,77 @@ def sparsity_sweep(torch, gs, wl):
     return out
 
 
-def suite_entry(torch, gs, wl, name, args, peaks):
-    """One BASELINE.json config other than the headline one: QPS of both kernels (CUDA events, queries resident),
-    roofline of the scoring kernel, per-call latency.  Parity of these configs is the business of tests/."""
+def suite_entry(torch, gs, wl, name, args, peaks, docs, ix):
+    """One BASELINE.json config other than the headline one, compact: QPS of both kernels (CUDA events, queries resident),
+    scoring-kernel time and roofline fraction, overflow count, per-call p50/p99 for the latency configs (B <= 32).
+    Parity of these configs is the business of tests/ (test_gpu_golden.py, test_gpu_parity.py)."""
     c = wl.CONFIGS[name]
     dev = torch.device("cuda:0")
     B, k = c["B"], c["k"]
-    docs = wl.make_docs(name)
-    n_lat = max(args.latency_queries, 1) if B <= 32 else 0
+    n_lat = (200 if B == 1 else 50) if (B <= 32 and args.latency_queries > 0) else 0
     queries = wl.make_queries(name, n_queries=max(B, n_lat * B))
     batch = queries.slice_rows(0, B)
-    ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs, head_max=args.head_max,
-                             head_density=args.head_density)
     info, lens, head_terms = ix.info(), ix.meta()[1].astype(np.int64), ix.head_terms()
     q_dev = [torch.from_numpy(a).to(dev) for a in (batch.indptr, batch.terms, batch.weights)]
     sdt = torch.float32 if c["wtype"] == "f32" else torch.int32
     out_ids = torch.empty((B, k), dtype=torch.int32, device=dev)
     out_sc = torch.empty((B, k), dtype=sdt, device=dev)
-    res = {"workload": f"N={docs.rows} docs, Zipf s={c['s']}, {c['wtype']} weights, B={B}, k={k}", "algos": {}}
-    steps = max(args.steps, 3)
-    for algo in ("term", "doc"):
+    res = {"workload": workload_label(name, c, docs.rows, B, k), "dtype": c["wtype"], "algos": {}}
+    steps = max(args.steps, 5)
+    for algo in ("auto", "term", "doc"):
         ws = torch.empty(ix.workspace_bytes(B, batch.nnz, k, algo=algo), dtype=torch.uint8, device=dev)
 
         def step():
-            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo)
+            ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo=algo, finish=False)
 
         ms = timed_steps(torch, None, step, steps, max(args.warmup, 3), 1)
         st = ix.stats(ws)
+        used = {1: "term", 2: "doc"}.get(st["algo_used"], "?")
+        if algo == "auto":
+            res["auto_dispatch"] = used
+            if used in ("term", "doc"):
+                del ws
+                continue
         gs.profile_enable(True)
         for _ in range(steps):
             step()
         torch.cuda.synchronize()
         prof = gs.profile_read()
         gs.profile_enable(False)
-        r = {"algo_used": {1: "term", 2: "doc"}.get(st["algo_used"], "?"), "ms_per_step": ms / steps, "qps": B * steps / (ms * 1e-3),
-             "ms_per_query": ms / steps / B, "overflow_queries": st["overflow_queries"],
+        r = {"algo_used": used, "ms_per_step": ms / steps, "qps": B * steps / (ms * 1e-3), "ms_per_query": ms / steps / B,
+             "overflow_queries": st["overflow_queries"], "launches_per_step": gs.last_launch_count(),
              "kernels": {n: {"launches_per_step": v["launches"] / steps, "ms_per_step": v["ms"] / steps} for n, v in prof.items()}}
-        r["roofline"] = roofline(r, st, info, lens, head_terms, batch, B, k, peaks, c["wtype"])
+        rl = roofline(r, st, info, lens, head_terms, batch, B, k, peaks, c["wtype"])
         del r["kernels"]
+        if rl:
+            r["roofline"] = {kk: rl.get(kk) for kk in ("kernel", "bound", "achieved", "peak", "unit", "frac", "kernel_ms_per_step",
+                                                       "share_of_step", "hbm_frac", "frac_one_pass", "doc_query_tile")
+                             if rl.get(kk) is not None}
         if n_lat:
-            r["latency"] = latency_leg(torch, ix, queries, k, n_lat, algo, batch=B)
+            lat = latency_leg(torch, ix, queries, k, n_lat, algo, batch=B)
+            r["latency"] = {kk: lat[kk] for kk in ("calls", "p50_ms", "p99_ms", "p50_ms_per_query", "graph_p50_ms", "graph_p99_ms") if kk in lat}
         res["algos"][algo] = r
         del ws
-    ix.close()
     return res
+
+
+def run_suite(torch, gs, wl, args, peaks):
+    """BASELINE.json configs 1, 2, 4 and 5 beside the headline config 3 (north_star: QPS, batch-1 p50 latency and roofline
+    fraction for every config).  Collections that share documents are generated and indexed once."""
+    dev = torch.device("cuda:0")
+    out = {}
+    groups = [("tiny", ["tiny"]), ("mid", ["mid"]), ("paper_u8", ["paper_u8"]), ("skew_b32", ["skew_b1", "skew_b32"])]
+    for doc_cfg, names in groups:
+        docs = wl.make_docs(doc_cfg)
+        ix = gs.Index.from_numpy(docs, wl.VOCAB, device=dev, tile_docs=args.tile_docs, head_max=args.head_max,
+                                 head_density=args.head_density)
+        for name in names:
+            out[name] = suite_entry(torch, gs, wl, name, args, peaks, docs, ix)
+        inf = ix.info()
+        out[names[0]]["index_bytes"] = {kk: inf[kk] for kk in ("bytes_inverted", "bytes_inverted_meta", "bytes_forward", "bytes_head", "bytes_total")}
+        ix.close()
+        del docs, ix
+    return out
 
 
 def measured_traffic(kernel: str, info, B: int):
@@ -504,7 +580,10 @@ def roofline(res, st, info, lens, head_terms, queries, B, k, peaks, wtype):
     ts = rf.batch_term_stats(lens, queries.terms)
     tr = measured_traffic(name, info, B) if wtype == "f32" else None
     out = {"kernel": name, "kernel_ms_per_step": kms, "launches_per_step": nl, "share_of_step": kms / res["ms_per_step"],
-           "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"], "traffic": tr["bytes_per_launch"] if tr else None, "traffic_detail": tr,
+           "bound": "hbm", "unit": "GB/s", "peak": peaks["hbm_gbs"], "peak_source": peaks["source"],
+           # `traffic` (ncu dram bytes per launch) cannot be measured inside an un-profiled run: the figure of the committed ncu
+           # capture of the same kernel and workload is quoted under its own name
+           "traffic": None, "traffic_static_from_profiles": tr,
            "useful_mac_per_step": ts["W"], "mac_per_s": ts["W"] / (kms * 1e-3)}
     if name == "score_doc":
         sp = rf.strips_per_pass(queries.indptr, queries.terms, head_terms, st["doc_query_tile"])

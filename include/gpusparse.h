@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define GS_ABI_VERSION 3
+#define GS_ABI_VERSION 4
 #if defined(__GNUC__)
 #define GS_API __attribute__((visibility("default")))
 #else
@@ -131,7 +131,7 @@ typedef struct gs_search_opts {
 /* Counters of the last search that used a workspace (read back with gs_search_stats). */
 typedef struct gs_stats {
     int64_t candidates;        /* (query, doc) cells that passed the threshold filter                  */
-    int32_t overflow_queries;  /* queries re-run through the dense fallback                            */
+    int32_t overflow_queries;  /* queries whose candidate list overflowed (exact only after gs_search_finish) */
     int32_t launches;          /* kernels launched by the call (host-side count)                       */
     int32_t algo_used;         /* gs_algo_t actually run                                               */
     int32_t sample_tiles;      /* doc tiles scored densely to obtain the thresholds                    */
@@ -167,19 +167,36 @@ GS_API gs_status_t gs_index_copy_head_terms(const gs_index_t* index, int32_t cap
 
 /* ------------------------------------------------------------------------------------------------
  * Search (§4-§5).
- * gs_search: queries and outputs are DEVICE pointers.  Asynchronous on `stream` (unless
- * GS_FLAG_VALIDATE_QUERIES), never allocates, re-entrant on different streams with different
- * workspaces.  out_doc_ids [B*k] int32, out_scores [B*k] float (GS_W_F32) or int32_t (GS_W_U8),
- * row-major, each row sorted by (score desc, doc id asc).  If k > N, slots >= N hold id -1 and
- * score -inf / INT32_MIN.  Query term ids outside [0,V) are ignored unless validation is on.
- * B == 0 is legal (nothing is written; the output pointers may then be NULL).
- * workspace: >= gs_search_workspace_bytes(...) bytes, 256-byte aligned.
+ * gs_search: queries and outputs are DEVICE pointers.  ASYNCHRONOUS on `stream`: the call only enqueues work (no
+ * synchronisation, no allocation, no host read-back), so it can be captured into a CUDA graph and is re-entrant on
+ * different streams with different workspaces (document-parallel searches of one device are serialised among
+ * themselves: they share one constant-memory query tile).  The one exception is GS_FLAG_VALIDATE_QUERIES, which
+ * synchronises to return the validation status.
+ * out_doc_ids [B*k] int32, out_scores [B*k] float (GS_W_F32) or int32_t (GS_W_U8), row-major, each row sorted by
+ * (score desc, doc id asc).  If k > N, slots >= N hold id -1 and score -inf / INT32_MIN.  Query term ids outside
+ * [0,V) are ignored unless validation is on.  B == 0 is legal (nothing is written; the output pointers may then be
+ * NULL).  Limits: B <= 65535 queries per call, k <= GS_MAX_K, a query row holds fewer than 2^24 terms.
+ * workspace: >= gs_search_workspace_bytes(...) bytes, 256-byte aligned; it must stay untouched until the search (and
+ * its gs_search_finish) is done.
+ *
+ * Exactness and gs_search_finish.  The search filters every (query, doc) cell against a per-query lower bound of the
+ * k-th best score taken from a sample of the doc tiles, and keeps the survivors in a candidate list of fixed capacity
+ * (8x the expected size).  A query whose list overflows (documents ordered so that the sample is unrepresentative) is
+ * counted in gs_stats_t.overflow_queries and its output row is NOT yet exact.  gs_search_finish synchronises `stream`,
+ * reads that count and re-runs exactly those queries through the dense path (every score materialised, exact), then
+ * synchronises again; with no overflow it costs one stream synchronisation and a 64-byte read-back.  Pass the same
+ * arguments as to gs_search.  *out_resolved (may be NULL) receives the number of queries re-run.  A caller that
+ * skips gs_search_finish (e.g. inside a captured graph) must check overflow_queries == 0 through gs_search_stats.
+ * gs_search_host calls it internally.
  * ---------------------------------------------------------------------------------------------- */
 GS_API gs_status_t gs_search_workspace_bytes(const gs_index_t* index, int64_t num_queries, int64_t query_nnz,
                                       int32_t k, const gs_search_opts_t* opts, size_t* out_bytes);
 GS_API gs_status_t gs_search(const gs_index_t* index, const gs_csr_t* queries, int32_t k,
                       const gs_search_opts_t* opts, int32_t* out_doc_ids, void* out_scores,
                       void* workspace, size_t workspace_bytes, gs_stream_t stream);
+GS_API gs_status_t gs_search_finish(const gs_index_t* index, const gs_csr_t* queries, int32_t k,
+                             const gs_search_opts_t* opts, int32_t* out_doc_ids, void* out_scores,
+                             void* workspace, size_t workspace_bytes, gs_stream_t stream, int32_t* out_resolved);
 
 /* Same search with HOST buffers: queries->* and the outputs are HOST pointers (pinned memory makes
  * the copies asynchronous).  Copies H2D, searches, copies D2H, synchronises `stream`.  Uses a

@@ -24,7 +24,7 @@ ALGOS = {"auto": GS_ALGO_AUTO, "term": GS_ALGO_TERM_PARALLEL, "doc": GS_ALGO_DOC
 EXPORTS = [
     "gs_index_build", "gs_index_info", "gs_index_free", "gs_index_copy_meta", "gs_index_copy_list",
     "gs_index_copy_head_terms",
-    "gs_search_workspace_bytes", "gs_search", "gs_search_host", "gs_search_stats", "gs_score_dense",
+    "gs_search_workspace_bytes", "gs_search", "gs_search_finish", "gs_search_host", "gs_search_stats", "gs_score_dense",
     "gs_topk_workspace_bytes", "gs_topk_dense", "gs_merge_topk_workspace_bytes", "gs_merge_topk", "gs_strerror", "gs_version", "gs_abi_version",
     "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name",
 ]
@@ -55,6 +55,10 @@ class gs_info_t(ctypes.Structure):
                 ("bytes_forward", ctypes.c_int64), ("bytes_head", ctypes.c_int64), ("bytes_total", ctypes.c_int64),
                 ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("reserved", ctypes.c_int32),
                 ("forward_padded_nnz", ctypes.c_int64)]
+
+
+class gs_alloc_t(ctypes.Structure):
+    _fields_ = [("alloc", ctypes.c_void_p), ("free", ctypes.c_void_p), ("user", ctypes.c_void_p)]
 
 
 class gs_search_opts_t(ctypes.Structure):
@@ -95,6 +99,7 @@ def lib():
         L.gs_index_copy_head_terms.argtypes = [vp, i32, vp, P(i32)]
         L.gs_search_workspace_bytes.argtypes = [vp, i64, i64, i32, P(gs_search_opts_t), P(sz)]
         L.gs_search.argtypes = [vp, P(gs_csr_t), i32, P(gs_search_opts_t), vp, vp, vp, sz, vp]
+        L.gs_search_finish.argtypes = [vp, P(gs_csr_t), i32, P(gs_search_opts_t), vp, vp, vp, sz, vp, P(i32)]
         L.gs_search_host.argtypes = [vp, P(gs_csr_t), i32, P(gs_search_opts_t), vp, vp, vp]
         L.gs_search_stats.argtypes = [vp, vp, P(gs_stats_t)]
         L.gs_score_dense.argtypes = [vp, P(gs_csr_t), P(gs_search_opts_t), vp, i64, vp, sz, vp]
@@ -189,13 +194,20 @@ class Index:
     """gs_index_build / gs_index_free: a GPU-resident inverted + forward index (§3)."""
 
     def __init__(self, indptr, terms, weights, vocab_size: int, *, tile_docs: int = 0, head_max: int = 0,
-                 head_density: float = 0.0, validate: bool = True, stream=None):
+                 head_density: float = 0.0, validate: bool = True, stream=None, allocator=None):
+        """``allocator``: optional pair of ctypes callbacks (alloc(bytes, stream, user) -> ptr, free(ptr, stream, user))
+        passed as gs_alloc_t; everything the handle owns then comes from it (default: cudaMalloc)."""
         L = lib()
         csr = _dev_csr(indptr, terms, weights)
         bo = gs_build_opts_t(tile_docs, head_max, head_density, 1 if validate else 0)
         h = ctypes.c_void_p()
         self._h = None
-        _check(L.gs_index_build(ctypes.byref(csr), vocab_size, ctypes.byref(bo), None, _stream_ptr(stream),
+        self._alloc = None
+        if allocator is not None:
+            self._cb = allocator                       # keep the callbacks alive as long as the handle
+            self._alloc = gs_alloc_t(ctypes.cast(allocator[0], ctypes.c_void_p), ctypes.cast(allocator[1], ctypes.c_void_p), None)
+        _check(L.gs_index_build(ctypes.byref(csr), vocab_size, ctypes.byref(bo),
+                                ctypes.byref(self._alloc) if self._alloc is not None else None, _stream_ptr(stream),
                                 ctypes.byref(h)))
         self._h = h
         self.wtype = csr.wtype
@@ -269,8 +281,12 @@ class Index:
         return self._ws
 
     def search(self, q_indptr, q_terms, q_weights, k: int, *, out_ids=None, out_scores=None, workspace=None,
-               stream=None, **opt):
-        """gs_search on DEVICE tensors -> (ids int32 [B,k], scores float32|int32 [B,k]) device tensors."""
+               stream=None, finish: bool = True, **opt):
+        """gs_search on DEVICE tensors -> (ids int32 [B,k], scores float32|int32 [B,k]) device tensors.
+
+        ``finish=True`` (default) follows it with gs_search_finish (one stream synchronisation; re-runs the queries
+        whose candidate list overflowed, so the result is always exact).  ``finish=False`` only enqueues the search
+        (asynchronous, capturable into a CUDA graph); call :meth:`finish` or check ``stats()["overflow_queries"]``."""
         torch = _torch()
         csr = _dev_csr(q_indptr, q_terms, q_weights)
         o = _opts(**opt)
@@ -285,7 +301,24 @@ class Index:
         _check(lib().gs_search(self._h, ctypes.byref(csr), k, ctypes.byref(o), out_ids.data_ptr(), out_scores.data_ptr(),
                                workspace.data_ptr(), workspace.numel(), _stream_ptr(stream)))
         self._last_ws = workspace
+        self.last_resolved = 0
+        if finish:
+            r = ctypes.c_int32()
+            _check(lib().gs_search_finish(self._h, ctypes.byref(csr), k, ctypes.byref(o), out_ids.data_ptr(),
+                                          out_scores.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                          _stream_ptr(stream), ctypes.byref(r)))
+            self.last_resolved = int(r.value)
         return out_ids, out_scores
+
+    def finish(self, q_indptr, q_terms, q_weights, k: int, out_ids, out_scores, workspace, stream=None, **opt) -> int:
+        """gs_search_finish for a search enqueued with ``finish=False``; returns the number of queries re-run."""
+        csr = _dev_csr(q_indptr, q_terms, q_weights)
+        o = _opts(**opt)
+        r = ctypes.c_int32()
+        _check(lib().gs_search_finish(self._h, ctypes.byref(csr), k, ctypes.byref(o), out_ids.data_ptr(),
+                                      out_scores.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                      _stream_ptr(stream), ctypes.byref(r)))
+        return int(r.value)
 
     def search_host(self, q_indptr: np.ndarray, q_terms: np.ndarray, q_weights: np.ndarray, k: int, *,
                     out_ids: Optional[np.ndarray] = None, out_scores: Optional[np.ndarray] = None, stream=None, **opt):

@@ -16,6 +16,8 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <set>
+#include <utility>
 #include <vector>
 
 #include "gs_internal.cuh"
@@ -26,6 +28,26 @@ size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, 
 thread_local int32_t gs_tls_launches = 0;
 static thread_local int32_t tls_cuda_error = 0;
 void gs_set_cuda_error(cudaError_t e) { tls_cuda_error = (int32_t)e; cudaGetLastError(); }
+
+cudaError_t gs_optin_smem_impl(const void* kern) {
+    static std::mutex mu;
+    static std::set<std::pair<const void*, int>> done;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count({kern, dev})) return cudaSuccess;
+    int smem_max = 0;
+    e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa{};
+    e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    // the opt-in limit covers static + dynamic shared memory
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - (int)fa.sharedSizeBytes);
+    if (e == cudaSuccess) done.insert({kern, dev});
+    return e;
+}
 
 // ---- kernel timing (gs_profile_*): thread-local list of event pairs
 namespace {
@@ -153,7 +175,7 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
     // (8*k*2^shift keys per query) are kept under 2 GiB for the batch, and never below the 1/32 sample.
     int shift = 5;
     if (o && o->sample_shift > 0) {
-        shift = o->sample_shift;
+        shift = std::min(o->sample_shift, 16);        // 1 .. 16; larger values would overflow the stride
     } else if (ix->N > 0) {
         const double r = std::sqrt((double)ix->N / (double)k);
         while (shift < 10 && (double)(1 << (shift + 1)) <= r * 1.4142) ++shift;
@@ -169,6 +191,10 @@ Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t*
         p.cand_cap = std::min<int64_t>(p.cand_cap, ix->N_pad);
     }
     return p;
+}
+
+bool plan_wants_x(const gs_index* ix, const Plan& p, int64_t B) {
+    return p.algo == GS_ALGO_TERM_PARALLEL && gs_score_term_wants_x(ix, B, p.group, p.use_head);
 }
 
 PlanStats plan_stats(const gs_index* ix, const Plan& p, int64_t B, int32_t sample_tiles) {
@@ -199,10 +225,9 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
     c.sb = (StatsBlock*)take(sizeof(StatsBlock));
     c.qb.head_pair = (uint2*)take((size_t)B * GS_HEAD_MAX * 8);
     c.qb.head_cnt = (int32_t*)take((size_t)B * 4);
-    c.qb.tail_term = (int32_t*)take((size_t)nnz * 4);
-    c.qb.tail_w = (uint32_t*)take((size_t)nnz * 4);
+    c.qb.tail_desc = (uint4*)take((size_t)nnz * 16);
     c.qb.tail_cnt = (int32_t*)take((size_t)B * 4);
-    c.qb.tail32 = (uint2*)take((size_t)B * GS_TAIL32 * 8);
+    c.qb.tail32 = (uint4*)take((size_t)B * GS_TAIL32 * 16);
     c.qb.xpair = (uint2*)take((size_t)B * GS_XSTRIP_MAX * 8);
     c.qb.xcnt = (int32_t*)take((size_t)B * 4);
     c.thr = (uint64_t*)take((size_t)B * 8);
@@ -258,8 +283,7 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     GS_CUDA(cudaMemsetAsync(c.sb, 0, sizeof(StatsBlock), s));
     if (B == 0) return GS_OK;
     const bool validate = p.flags & GS_FLAG_VALIDATE_QUERIES;
-    GS_TRY(gs_launch_ingest(ix, q, validate, p.use_head,
-                            p.algo == GS_ALGO_TERM_PARALLEL && gs_score_term_wants_x(ix, B, p.group, p.use_head), &c.qb, s));
+    GS_TRY(gs_launch_ingest(ix, q, validate, p.use_head, plan_wants_x(ix, p, B), &c.qb, s));
     if (validate) {
         int32_t st = 0;
         GS_CUDA(cudaMemcpyAsync(&st, &c.sb->status, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
@@ -325,15 +349,26 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
-    // ---- 4. overflowed candidate lists -> dense fallback for those queries (needs the count on the host)
-    int32_t n_ov = 0;
-    GS_CUDA(cudaMemcpyAsync(&n_ov, &c.sb->n_overflow, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
-    GS_CUDA(cudaStreamSynchronize(s));
-    if (n_ov > 0) {
-        std::vector<int32_t> ov(n_ov);
-        GS_CUDA(cudaMemcpyAsync(ov.data(), c.overflow_list, sizeof(int32_t) * (size_t)n_ov, cudaMemcpyDeviceToHost, s));
-        GS_CUDA(cudaStreamSynchronize(s));
-        for (int32_t b : ov) GS_TRY(dense_topk(ix, p, q, c, b, 1, k, out_ids, out_scores, s));
+    // ---- 4. a query whose candidate list overflowed has an inexact row: it is flagged in the stats block (n_overflow, list
+    // of the queries) and re-run through the dense path by gs_search_finish — the only part that needs the host
+    return GS_OK;
+}
+
+// dense fallback for the overflowed queries of the last gs_search on this workspace (n_ov of them, host list `ov`):
+// consecutive query numbers are re-run together, as many at a time as the dense region holds
+gs_status_t resolve_overflow(const gs_index* ix, const gs_csr_t* q, int32_t k, const gs_search_opts_t* opts, int32_t* out_ids,
+                             void* out_scores, void* ws, size_t ws_bytes, std::vector<int32_t>& ov, cudaStream_t s) {
+    Plan p = make_plan(ix, q->rows, k, opts);
+    Carve c = carve_ws(ix, p, q->rows, q->nnz, k, ws, ws_bytes);
+    c.qb.B = q->rows; c.qb.nnz = q->nnz; c.qb.indptr = q->indptr;
+    // the ingest result of the search is still in the workspace (second-tier strip lists included)
+    c.qb.x_on = plan_wants_x(ix, p, q->rows) && ix->HX > 0;
+    std::sort(ov.begin(), ov.end());
+    for (size_t i = 0; i < ov.size();) {
+        size_t j = i + 1;
+        while (j < ov.size() && ov[j] == ov[j - 1] + 1) ++j;
+        GS_TRY(dense_topk(ix, p, q, c, ov[i], (int64_t)(j - i), k, out_ids, (uint32_t*)out_scores, s));
+        i = j;
     }
     return GS_OK;
 }
@@ -384,7 +419,7 @@ void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
     void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
-                    ix->seg, ix->seg2, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
+                    ix->term_meta, ix->seg_tab, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
 }
@@ -464,6 +499,33 @@ gs_status_t gs_search(const gs_index_t* ix, const gs_csr_t* q, int32_t k, const 
     return search_impl(ix, q, k, norm_opts(opts, &tmp), out_ids, out_scores, ws, ws_bytes, (cudaStream_t)stream);
 }
 
+gs_status_t gs_search_finish(const gs_index_t* ix, const gs_csr_t* q, int32_t k, const gs_search_opts_t* opts,
+                             int32_t* out_ids, void* out_scores, void* ws, size_t ws_bytes, gs_stream_t stream,
+                             int32_t* out_resolved) {
+    if (out_resolved) *out_resolved = 0;
+    if (!ix || !ws || !q) return GS_ERR_INVALID_ARG;
+    if (k < 1 || k > GS_MAX_K) return GS_ERR_OUT_OF_RANGE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (q->rows == 0) return GS_OK;
+    StatsBlock sb;
+    GS_CUDA(cudaMemcpyAsync(&sb, ws, sizeof(StatsBlock), cudaMemcpyDeviceToHost, s));
+    GS_CUDA(cudaStreamSynchronize(s));
+    const int32_t n_ov = sb.n_overflow;
+    if (n_ov <= 0) return GS_OK;
+    if (n_ov > q->rows) return GS_ERR_INVALID_ARG;             // not the workspace of a search of this batch
+    gs_search_opts_t tmp;
+    const gs_search_opts_t* o = norm_opts(opts, &tmp);
+    Plan p = make_plan(ix, q->rows, k, o);
+    Carve c = carve_ws(ix, p, q->rows, q->nnz, k, ws, ws_bytes);
+    std::vector<int32_t> ov((size_t)n_ov);
+    GS_CUDA(cudaMemcpyAsync(ov.data(), c.overflow_list, sizeof(int32_t) * (size_t)n_ov, cudaMemcpyDeviceToHost, s));
+    GS_CUDA(cudaStreamSynchronize(s));
+    GS_TRY(resolve_overflow(ix, q, k, o, out_ids, out_scores, ws, ws_bytes, ov, s));
+    GS_CUDA(cudaStreamSynchronize(s));
+    if (out_resolved) *out_resolved = n_ov;
+    return GS_OK;
+}
+
 gs_status_t gs_search_host(gs_index_t* ix, const gs_csr_t* hq, int32_t k, const gs_search_opts_t* opts,
                            int32_t* host_ids, void* host_scores, gs_stream_t stream) {
     static std::mutex mu;
@@ -506,9 +568,19 @@ gs_status_t gs_search_host(gs_index_t* ix, const gs_csr_t* hq, int32_t k, const 
     dq.weights = st + o_w;
     gs_status_t r = gs_search(ix, &dq, k, opts, (int32_t*)(st + o_ids), st + o_sc, ix->host_ws, ix->host_ws_bytes, stream);
     if (r != GS_OK) return r;
+    // results and the overflow count come back together: ONE synchronisation on the common path
+    int32_t n_ov = 0;
+    if (B > 0) GS_CUDA(cudaMemcpyAsync(&n_ov, &((StatsBlock*)ix->host_ws)->n_overflow, sizeof(int32_t), cudaMemcpyDeviceToHost, s));
     GS_CUDA(cudaMemcpyAsync(host_ids, st + o_ids, 4 * (size_t)B * k, cudaMemcpyDeviceToHost, s));
     GS_CUDA(cudaMemcpyAsync(host_scores, st + o_sc, 4 * (size_t)B * k, cudaMemcpyDeviceToHost, s));
     GS_CUDA(cudaStreamSynchronize(s));
+    if (n_ov > 0) {                     // rare: some candidate list overflowed -> dense re-run of those queries, copy again
+        int32_t resolved = 0;
+        GS_TRY(gs_search_finish(ix, &dq, k, opts, (int32_t*)(st + o_ids), st + o_sc, ix->host_ws, ix->host_ws_bytes, stream, &resolved));
+        GS_CUDA(cudaMemcpyAsync(host_ids, st + o_ids, 4 * (size_t)B * k, cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaMemcpyAsync(host_scores, st + o_sc, 4 * (size_t)B * k, cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaStreamSynchronize(s));
+    }
     return GS_OK;
 }
 
@@ -536,8 +608,7 @@ gs_status_t gs_score_dense(const gs_index_t* ix, const gs_csr_t* q, const gs_sea
     if (ws_bytes < c.fixed_bytes) return GS_ERR_OOM;
     c.qb.B = q->rows; c.qb.nnz = q->nnz; c.qb.indptr = q->indptr;
     if (q->rows == 0 || ix->N == 0) return GS_OK;
-    GS_TRY(gs_launch_ingest(ix, q, false, p.use_head,
-                            p.algo == GS_ALGO_TERM_PARALLEL && gs_score_term_wants_x(ix, q->rows, p.group, p.use_head), &c.qb, s));
+    GS_TRY(gs_launch_ingest(ix, q, false, p.use_head, plan_wants_x(ix, p, q->rows), &c.qb, s));
     gs_tileset all{0, 1, ix->ntiles};
     gs_sink sink{};
     sink.dense = (uint32_t*)out_scores;

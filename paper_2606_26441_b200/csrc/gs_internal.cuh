@@ -8,6 +8,7 @@
 
 #define GS_STRIP_MAX 64         // dense strips kept by the index
 #define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
+#define GS_HOT_STRIPS 32        // the densest strips: kept in tensor memory by the fp32 batch kernel
 #ifndef GS_XSTRIP_MAX
 #define GS_XSTRIP_MAX 128
 #endif
@@ -22,6 +23,10 @@
 #define GS_SEL_BITS 11
 
 void gs_set_cuda_error(cudaError_t e);
+// Raises a kernel's dynamic shared-memory limit to the device's opt-in maximum, once per (kernel, device): launches then pass
+// their actual size, and concurrent callers never see a limit smaller than what they launch with.
+cudaError_t gs_optin_smem_impl(const void* kern);
+template <typename K> inline cudaError_t gs_optin_smem(K kern) { return gs_optin_smem_impl(reinterpret_cast<const void*>(kern)); }
 #define GS_CUDA(call)                                   \
     do {                                                \
         cudaError_t e__ = (call);                       \
@@ -35,6 +40,14 @@ void gs_set_cuda_error(cudaError_t e);
         gs_status_t s__ = (call);                       \
         if (s__ != GS_OK) return s__;                   \
     } while (0)
+
+// per-term entry of the compact tile-segment table (16 bytes: one 128-bit load)
+struct __align__(16) gs_term_meta {
+    uint32_t tab_off;     // first entry of the term in seg_tab
+    uint32_t shift;       // log2 of the doc tiles per table entry
+    uint32_t list_blk;    // start of the term's padded posting list / 32 (lists are padded to 32 slots)
+    uint32_t len;         // true list length
+};
 
 // ------------------------------------------------------------------------------------------------
 // The index handle.  All pointers are device pointers owned by the handle.
@@ -63,9 +76,14 @@ struct gs_index {
     int32_t* inv_len = nullptr;      // [V]   true list length
     int32_t* inv_doc = nullptr;      // [P_pad] doc ids, ascending within a list, -1 in the padding
     void* inv_w = nullptr;           // [P_pad] float | uint8, 0 in the padding
-    // per-(term, tile) segment table: seg[t*(ntiles+1)+j] = number of postings of t with doc < j*Ts
-    uint32_t* seg = nullptr;         // [V][ntiles+1]
-    uint2* seg2 = nullptr;           // [V][ntiles] (first slot, end slot) of term t inside tile j, absolute (P_pad < 2^32 only)
+    // Compact tile-segment table.  Term t owns seg_tab[meta.tab_off .. + (ntiles >> meta.shift) + 2): entry g = number of
+    // postings of t whose doc tile is < (g << shift), so the postings of t inside doc tile j lie in the slot range
+    // [tab[j >> shift], tab[(j >> shift) + 1]) of its list — exactly that range when shift == 0, a superset (the tiles of
+    // the same group of 2^shift tiles) otherwise; a reader drops the postings outside its tile by their doc ids.  shift
+    // grows as the list gets shorter (a group holds ~4 postings on average), so the table costs O(postings), not O(V * ntiles).
+    gs_term_meta* term_meta = nullptr;   // [V]
+    uint32_t* seg_tab = nullptr;         // [seg_entries]
+    int64_t seg_entries = 0;
     // dense strips of the densest lists ("head" terms)
     int32_t H = 0;                   // strips (<= GS_STRIP_MAX), densest list first
     int32_t head_terms_host[GS_STRIP_MAX];
@@ -119,16 +137,17 @@ struct gs_qbatch {
     int64_t B = 0;
     int64_t nnz = 0;
     const int64_t* indptr = nullptr;   // caller's CSR indptr (device)
-    uint2* head_pair = nullptr;        // [B][GS_HEAD_MAX] compact (strip number, accumulator-typed weight bits)
-    int32_t* head_cnt = nullptr;       // [B] number of head terms of the query
+    uint2* head_pair = nullptr;        // [B][GS_HEAD_MAX] compact (strip number, accumulator-typed weight bits): the "hot" strips
+                                       // (number < GS_HOT_STRIPS) from entry 0 upwards, the others from the last entry downwards
+    int32_t* head_cnt = nullptr;       // [B] head terms of the query | hot ones << 8
     uint2* xpair = nullptr;            // [B][GS_XSTRIP_MAX] compact (x-strip number, weight bits); used when x_on
     int32_t* xcnt = nullptr;           // [B]
     bool x_on = false;                 // the batch's x-strip terms are in xpair (and NOT in the tail lists)
-    int32_t* tail_term = nullptr;      // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]
-    uint32_t* tail_w = nullptr;        // [nnz] accumulator-typed
+    uint4* tail_desc = nullptr;        // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]: per tail term
+                                       // (accumulator-typed weight bits, segment-table offset, shift, list start / 32)
     int32_t* tail_cnt = nullptr;       // [B]
-    uint2* tail32 = nullptr;           // [B][32] the first 32 tail terms as (term id or -1, weight bits): a fixed-stride
-                                       // copy the batch kernel can prefetch without reading indptr first
+    uint4* tail32 = nullptr;           // [B][32] the first 32 tail terms, same entries (shift = 0xFFFFFFFF: no term): a
+                                       // fixed-stride copy the batch kernel can prefetch without reading indptr first
     int32_t* status = nullptr;         // device status word: first validation error (gs_status_t) or 0
 };
 

@@ -100,41 +100,32 @@ __device__ __forceinline__ int32_t term_of_slot(const int64_t* __restrict__ inv_
     return lo;
 }
 
-// Per padded slot: duplicate detection (equal neighbours inside a list) + the tile segment table.
+// Per padded slot: duplicate detection (equal neighbours inside a list) + the compact tile-segment table: entry g of term t
+// = number of postings of t whose doc tile is < (g << shift_t).  The posting at list position i with group
+// grp = (doc / Ts) >> shift writes i into the entries (group of its predecessor, grp]; the last posting fills the rest.
 __global__ void k_segments(const int64_t* __restrict__ inv_off, const int32_t* __restrict__ inv_len,
                            const int32_t* __restrict__ inv_doc, int32_t V, int64_t P_pad, int32_t Ts, int32_t ntiles,
-                           uint32_t* __restrict__ seg, int* err) {
+                           const gs_term_meta* __restrict__ meta, uint32_t* __restrict__ tab, int* err) {
     int64_t pos = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (pos >= P_pad) return;
     int32_t t = term_of_slot(inv_off, V, pos);
     int32_t i = (int32_t)(pos - inv_off[t]);
     int32_t len = inv_len[t];
     if (i >= len) return;                       // padding slot
+    const gs_term_meta m = meta[t];
     int32_t doc = inv_doc[pos];
-    int32_t tile_cur = doc / Ts;
-    int32_t tile_prev = -1;
+    int32_t grp_cur = (doc / Ts) >> m.shift;
+    int32_t grp_prev = -1;
     if (i > 0) {
         int32_t prev = inv_doc[pos - 1];
         if (prev == doc) atomicCAS(err, 0, (int)GS_ERR_DUPLICATE_TERM);
-        tile_prev = prev / Ts;
+        grp_prev = (prev / Ts) >> m.shift;
     }
-    uint32_t* row = seg + (size_t)t * (ntiles + 1);
-    for (int32_t j = tile_prev + 1; j <= tile_cur; ++j) row[j] = (uint32_t)i;
+    uint32_t* row = tab + m.tab_off;
+    const int32_t n_ent = (ntiles >> m.shift) + 2;
+    for (int32_t j = grp_prev + 1; j <= grp_cur; ++j) row[j] = (uint32_t)i;
     if (i == len - 1)
-        for (int32_t j = tile_cur + 1; j <= ntiles; ++j) row[j] = (uint32_t)len;
-}
-
-// Pair form of the segment table for the batch kernel: seg2[t][j] = (first slot, one past the last slot) of the postings
-// of term t inside doc tile j, as absolute posting slots (needs P_pad < 2^32): one aligned 64-bit load per probe
-// instead of two table loads and a list-offset load.
-__global__ void k_segment_pairs(const int64_t* __restrict__ inv_off, const uint32_t* __restrict__ seg, int32_t V,
-                                int32_t ntiles, uint2* __restrict__ seg2) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (i >= (int64_t)V * ntiles) return;
-    const int32_t t = (int32_t)(i / ntiles), j = (int32_t)(i - (int64_t)t * ntiles);
-    const uint32_t off = (uint32_t)inv_off[t];
-    const uint32_t* row = seg + (size_t)t * (ntiles + 1);
-    seg2[i] = make_uint2(off + row[j], off + row[j + 1]);
+        for (int32_t j = grp_cur + 1; j < n_ent; ++j) row[j] = (uint32_t)len;
 }
 
 template <typename W>
@@ -388,13 +379,31 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     }
     ix->bytes_inverted = (int64_t)((sizeof(int32_t) + sizeof(W)) * (size_t)ix->P_pad);
 
-    // ---- segment table
-    const size_t seg_elems = (size_t)V * (size_t)(ix->ntiles + 1);
-    ix->seg = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * seg_elems, s);
-    if (!ix->seg) return GS_ERR_OOM;
-    GS_CUDA(cudaMemsetAsync(ix->seg, 0, sizeof(uint32_t) * seg_elems, s));
-    ix->bytes_meta = (int64_t)(sizeof(uint32_t) * seg_elems + sizeof(int64_t) * (size_t)(V + 1) +
-                               sizeof(int32_t) * (size_t)V + sizeof(int16_t) * (size_t)V);
+    // ---- compact tile-segment table: a group of 2^shift doc tiles per entry, ~kSegTarget postings per group on average
+    {
+        constexpr double kSegTarget = 4.0;
+        std::vector<gs_term_meta> h_meta((size_t)V);
+        int64_t n_ent = 0;
+        for (int32_t t = 0; t < V; ++t) {
+            uint32_t shift = 0;
+            while (shift < 15 && (double)h_len[t] * (double)(2u << shift) <= kSegTarget * (double)std::max(ix->ntiles, 1)) ++shift;
+            h_meta[t].tab_off = (uint32_t)n_ent;
+            h_meta[t].shift = shift;
+            h_meta[t].list_blk = (uint32_t)(h_off[t] / GS_WARP_BLOCK);
+            h_meta[t].len = (uint32_t)h_len[t];
+            n_ent += (ix->ntiles >> shift) + 2;
+            if (n_ent >= 0xFFFFFFF0LL || h_off[t] / GS_WARP_BLOCK > 0xFFFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+        }
+        ix->seg_entries = n_ent;
+        ix->term_meta = (gs_term_meta*)gs_dev_alloc(ix, sizeof(gs_term_meta) * (size_t)V, s);
+        ix->seg_tab = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)n_ent, s);
+        if (!ix->term_meta || !ix->seg_tab) return GS_ERR_OOM;
+        GS_CUDA(cudaMemcpyAsync(ix->term_meta, h_meta.data(), sizeof(gs_term_meta) * (size_t)V, cudaMemcpyHostToDevice, s));
+        GS_CUDA(cudaMemsetAsync(ix->seg_tab, 0, sizeof(uint32_t) * (size_t)n_ent, s));
+        GS_CUDA(cudaStreamSynchronize(s));            // h_meta is a local
+        ix->bytes_meta = (int64_t)(sizeof(uint32_t) * (size_t)n_ent + sizeof(gs_term_meta) * (size_t)V +
+                                   sizeof(int64_t) * (size_t)(V + 1) + sizeof(int32_t) * (size_t)V + 2 * sizeof(int16_t) * (size_t)V);
+    }
 
     if (P > 0) {
         // ---- stable sort of (term, source position) by term
@@ -420,21 +429,12 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         k_scatter_padded<W><<<grid_for(P), kThreads, 0, s>>>(d_sorted_terms, d_src_out, d_rowid, (const W*)docs->weights,
                                                             d_scan, ix->inv_off, P, ix->inv_doc, (W*)ix->inv_w);
         k_segments<<<grid_for(ix->P_pad), kThreads, 0, s>>>(ix->inv_off, ix->inv_len, ix->inv_doc, V, ix->P_pad, ix->Ts,
-                                                            ix->ntiles, ix->seg, d_err);
+                                                            ix->ntiles, ix->term_meta, ix->seg_tab, d_err);
         GS_CUDA(cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
         GS_CUDA(cudaStreamSynchronize(s));
         GS_CUDA(cudaGetLastError());
         if (h_err && o.validate) return (gs_status_t)h_err;
     }
-    if (ix->P_pad < (int64_t)0xFFFFFFFFLL && ix->ntiles > 0) {
-        const size_t pair_elems = (size_t)V * (size_t)ix->ntiles;
-        ix->seg2 = (uint2*)gs_dev_alloc(ix, sizeof(uint2) * pair_elems, s);
-        if (!ix->seg2) return GS_ERR_OOM;
-        k_segment_pairs<<<grid_for((int64_t)pair_elems), kThreads, 0, s>>>(ix->inv_off, ix->seg, V, ix->ntiles, ix->seg2);
-        GS_CUDA(cudaGetLastError());
-        ix->bytes_meta += (int64_t)(sizeof(uint2) * pair_elems);
-    }
-
     // ---- dense strips of the head lists
     if (ix->H > 0) {
         size_t strip_bytes = sizeof(W) * (size_t)ix->H * (size_t)ix->N_pad;

@@ -133,8 +133,9 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                                                       const void* __restrict__ weights, const int16_t* __restrict__ head_slot,
                                                       int H, int64_t q0, int64_t nq, int QT, int32_t V, int Wd,
                                                       const uint64_t* __restrict__ thr, unsigned char* __restrict__ scratch,
-                                                      int64_t n_passes, int64_t nnz_cap) {
+                                                      int64_t n_passes, int64_t nnz_cap, const int32_t* __restrict__ status) {
     extern __shared__ uint32_t sm[];                  // bitmap[Wd], prefix[Wd]
+    if (*status != 0) return;                         // ingest found a malformed batch (e.g. a non-monotone indptr): nothing is read
     __shared__ uint32_t warp_tot[32];
     __shared__ uint32_t s_hmask[2];
     __shared__ uint32_t s_total;
@@ -269,6 +270,7 @@ struct DocParams {
     int32_t sparse_cap_bytes;                   // shared memory left for a pass's row table + pairs
     int64_t qa; int32_t nqt;                    // queries [qa, qa+nqt) of the batch; q_rel = qa - q0 of the launch
     int64_t q_rel;
+    const int32_t* status;                      // ingest status word: non-zero = malformed batch, the pass does nothing
     gs_tileset ts;
     gs_sink sink;
 };
@@ -367,6 +369,7 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     using G = Geo<QT>;
     constexpr int AST = G::AST, NW = G::NW, QCAP = G::QCAP;
     extern __shared__ __align__(16) unsigned char smem[];
+    if (*p.status != 0) return;
     const int Wd = p.Wd;
     const uint32_t R = c_tile.R, np = c_tile.np;
     const int nh = (int)c_tile.nh;
@@ -589,7 +592,7 @@ gs_status_t launch_passes(DocParams p, const unsigned char* scratch, int Wd, int
     const size_t smem = (size_t)smem_max;
     p.sparse_cap_bytes = (int32_t)(smem - fixed);
     const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(sms, (n_subs + G::NW - 1) / G::NW));
-    GS_CUDA(cudaFuncSetAttribute(k_score_doc<WT, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GS_CUDA(gs_optin_smem(k_score_doc<WT, QT>));
     int dev = 0;
     cudaGetDevice(&dev);
     std::lock_guard<std::mutex> lock(g_tile_mu);
@@ -641,7 +644,6 @@ size_t gs_score_doc_scratch_bytes_ex(const gs_index* ix, int qtile, int64_t nq, 
 
 gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_qbatch& qb, int64_t q0, int64_t nq,
                                 int qtile, const gs_tileset& ts, const gs_sink& sink, void* scratch, cudaStream_t s) {
-    (void)qb;
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     const int QT = norm_qt(qtile);
     const int n_passes = (int)((nq + QT - 1) / QT);
@@ -658,13 +660,13 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
         if (bsm > (size_t)smem_max) return GS_ERR_OUT_OF_RANGE;
         GsProfScope ps(GS_K_QTILE, s);
         if (ix->wtype == GS_W_F32) {
-            GS_CUDA(cudaFuncSetAttribute(k_build_qtile<GS_W_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
+            GS_CUDA(gs_optin_smem(k_build_qtile<GS_W_F32>));
             k_build_qtile<GS_W_F32><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                              QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz);
+                                                              QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status);
         } else {
-            GS_CUDA(cudaFuncSetAttribute(k_build_qtile<GS_W_U8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bsm));
+            GS_CUDA(gs_optin_smem(k_build_qtile<GS_W_U8>));
             k_build_qtile<GS_W_U8><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                             QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz);
+                                                             QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status);
         }
         ++gs_tls_launches;
         GS_CUDA(cudaGetLastError());
@@ -675,7 +677,7 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
     p.strips = ix->head_strip; p.N_pad = ix->N_pad;
     p.N = ix->N; p.V = ix->V; p.Ts = ix->Ts; p.Wd = Wd;
     p.rows = ss.rows; p.pairs = ss.pairs;
-    p.ts = ts; p.sink = sink;
+    p.ts = ts; p.sink = sink; p.status = qb.status;
     const int64_t n_subs = (int64_t)ts.count * (ix->Ts / 32);
     return ix->wtype == GS_W_F32
                ? launch_doc_qt<GS_W_F32>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s)

@@ -820,11 +820,11 @@ int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); 
 template <int WT, bool XS>
 gs_status_t launch_x(const TermParams& p, unsigned grid, size_t smem, bool staged, cudaStream_t s) {
     if (staged) {
-        GS_CUDA(cudaFuncSetAttribute(k_score_term_staged<WT, XS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GS_CUDA(gs_optin_smem(k_score_term_staged<WT, XS>));
         GsProfScope ps(GS_K_SCORE_TERM, s);
         k_score_term_staged<WT, XS><<<grid, kWarpsStaged * 32, smem, s>>>(p);
     } else {
-        GS_CUDA(cudaFuncSetAttribute(k_score_term<WT, XS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GS_CUDA(gs_optin_smem(k_score_term<WT, XS>));
         GsProfScope ps(GS_K_SCORE_TERM, s);
         k_score_term<WT, XS><<<grid, p.warps * 32, smem, s>>>(p);
     }
@@ -906,7 +906,7 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
         const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 16;
         if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max && nq <= 65535) {
             auto go = [&](auto kern) -> gs_status_t {
-                GS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch));
+                GS_CUDA(gs_optin_smem(kern));
                 GsProfScope ps(GS_K_SCORE_TERM, s);
                 // persistent: one CTA per SM walks the (doc tile, query chunk) items
                 kern<<<(unsigned)std::min<int64_t>(grid, sms), kBWarps * 32, smem_batch, s>>>(p);

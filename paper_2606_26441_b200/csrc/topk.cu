@@ -414,7 +414,7 @@ gs_status_t run_select(const gs_sel_src& src, int64_t rows, int32_t k, int32_t* 
         int kp2 = 32;
         while (kp2 < k) kp2 <<= 1;
         const size_t smem = (size_t)kp2 * 8 + GS_SEL_BINS * 4;
-        GS_CUDA(cudaFuncSetAttribute(k_sel_row<WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GS_CUDA(gs_optin_smem(k_sel_row<WT>));
         // CTAs per row: enough to spread a few rows over the chip, one when there are rows to spare
         int C = 1;
         while (C < 8 && rows * C < GS_SEL_TARGET && max_items > (int64_t)C * 8192) C <<= 1;

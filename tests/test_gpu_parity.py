@@ -557,3 +557,126 @@ def _take_rows(csr, rows):
         terms.append(t); weights.append(w)
         indptr.append(indptr[-1] + len(t))
     return np.array(indptr, np.int64), np.concatenate(terms), np.concatenate(weights)
+
+
+# ----------------------------------------------------------------------------------------------------
+# the boundary: asynchronous gs_search (CUDA-graph capture), gs_search_finish, allocator callbacks, indptr checks
+# ----------------------------------------------------------------------------------------------------
+def test_search_is_asynchronous_and_replays_from_a_cuda_graph(gs, tiny):
+    """gs_search only enqueues work: captured once into a CUDA graph, the search is replayed for new query data written
+    into the same buffers, and every replay matches the oracle (asynchronous on the stream, never allocates)."""
+    import torch
+    docs = wl.make_docs("mid", n_docs=60_011)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    k, B = 10, 4
+    all_q = wl.make_queries("mid", n_queries=3 * B)
+    cap_nnz = int(max(all_q.slice_rows(i * B, (i + 1) * B).nnz for i in range(3)))
+    d = torch.device("cuda:0")
+    q_ip = torch.zeros(B + 1, dtype=torch.int64, device=d)
+    q_t = torch.zeros(cap_nnz, dtype=torch.int32, device=d)
+    q_w = torch.zeros(cap_nnz, dtype=torch.float32, device=d)
+    ws = torch.empty(ix.workspace_bytes(B, cap_nnz, k, algo="term"), dtype=torch.uint8, device=d)
+    out_ids = torch.empty((B, k), dtype=torch.int32, device=d)
+    out_sc = torch.empty((B, k), dtype=torch.float32, device=d)
+
+    def put(q):
+        q_ip.copy_(torch.from_numpy(q.indptr))
+        q_t[:q.nnz].copy_(torch.from_numpy(q.terms))
+        q_w[:q.nnz].copy_(torch.from_numpy(q.weights))
+
+    put(all_q.slice_rows(0, B))
+    ix.search(q_ip, q_t, q_w, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo="term")     # warm-up (module load, attributes)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        ix.search(q_ip, q_t, q_w, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo="term", finish=False)
+    n_launch = gs.last_launch_count()
+    assert n_launch > 0
+    for i in range(3):
+        q = all_q.slice_rows(i * B, (i + 1) * B)
+        put(q)
+        out_ids.fill_(-7)
+        g.replay()
+        torch.cuda.synchronize()
+        assert ix.stats(ws)["overflow_queries"] == 0
+        # the CSR arrays keep their captured length: entries past indptr[B] are never read
+        compare(gs, docs, q, wl.VOCAB, k, out_ids.cpu().numpy(), out_sc.cpu().numpy())
+    ix.close()
+
+
+def test_finish_resolves_overflow_after_an_asynchronous_search(gs):
+    """finish=False leaves the overflowed rows inexact and flagged; gs_search_finish re-runs exactly those queries."""
+    n = 200_000
+    d = np.arange(n)
+    has1, has2 = (d % 5 == 3) & ((d // 512) % 64 != 0), d % 50 == 7
+    nnz = 1 + has1.astype(np.int64) + has2.astype(np.int64)
+    indptr = np.concatenate([[0], np.cumsum(nnz)]).astype(np.int64)
+    terms = np.zeros(indptr[-1], np.int32)
+    terms[indptr[:-1][has1] + 1] = 1
+    terms[indptr[1:][has2] - 1] = 2
+    docs = wl.Csr(indptr, terms, np.ones(indptr[-1], np.float32))
+    # the queries that use term 1 (which the sampled tiles never hold) overflow; query 1 does not
+    queries = csr_from_dicts([{0: 1, 1: 1, 2: 2}, {0: 1}, {0: 1, 1: 1, 2: 1}, {0: 2, 1: 1}], np.float32)
+    ix = gs.Index.from_numpy(docs, 8)
+    qd = dev(queries)
+    ids, sc = ix.search(*qd, 50, algo="term", finish=False)
+    st = ix.stats()
+    n_ov = st["overflow_queries"]
+    assert 2 <= n_ov <= 3
+    resolved = ix.finish(*qd, 50, ids, sc, ix._last_ws, algo="term")
+    assert resolved == n_ov
+    compare(gs, docs, queries, 8, 50, ids.cpu().numpy(), sc.cpu().numpy())
+    ix.close()
+
+
+def test_index_build_through_allocator_callbacks(gs, tiny):
+    """gs_alloc_t: everything the handle owns comes from the caller's allocator (here torch's caching allocator through
+    ctypes callbacks) and goes back to it on gs_index_free."""
+    import ctypes
+    import torch
+    live = {}
+
+    @ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p)
+    def c_alloc(nbytes, stream, user):
+        p = torch.cuda.caching_allocator_alloc(int(nbytes), device=0)
+        live[p] = int(nbytes)
+        return p
+
+    @ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
+    def c_free(ptr, stream, user):
+        live.pop(ptr)
+        torch.cuda.caching_allocator_delete(ptr)
+
+    ix = gs.Index.from_numpy(tiny.docs, tiny.vocab, allocator=(c_alloc, c_free))
+    assert len(live) >= 8 and sum(live.values()) >= ix.info()["bytes_total"]
+    ids, sc = gpu_search(gs, ix, tiny.queries, 10, algo="term")
+    compare(gs, tiny.docs, tiny.queries, tiny.vocab, 10, ids, sc)
+    ids, sc = ix.search_host(tiny.queries.indptr, tiny.queries.terms, tiny.queries.weights, 10, algo="doc")
+    compare(gs, tiny.docs, tiny.queries, tiny.vocab, 10, ids, sc)
+    ix.close()
+    assert not live, "gs_index_free must return every block to the allocator"
+
+
+def test_malformed_query_indptr_is_rejected_not_dereferenced(gs, tiny):
+    """A non-monotone / out-of-range query indptr must never index past the nnz-sized arrays: the rows are treated as
+    empty, and with validation on the call returns GS_ERR_OUT_OF_RANGE."""
+    ix = gs.Index.from_numpy(tiny.docs, tiny.vocab)
+    q = tiny.queries
+    for bad in ("decreasing", "past_end", "first_not_zero"):
+        ip = q.indptr.copy()
+        if bad == "decreasing":
+            ip[3] = ip[2] - 1
+        elif bad == "past_end":
+            ip[-1] = q.nnz + 1000
+        else:
+            ip[0] = 2
+        bq = wl.Csr(ip, q.terms, q.weights)
+        for algo in ("term", "doc"):
+            with pytest.raises(gs.GsError) as e:
+                gpu_search(gs, ix, bq, 5, algo=algo, flags=gs.GS_FLAG_VALIDATE_QUERIES)
+            assert e.value.code == 2
+            ids, sc = gpu_search(gs, ix, bq, 5, algo=algo)       # validation off: memory-safe, result unspecified
+            assert ids.shape == (q.rows, 5)
+    ids, sc = gpu_search(gs, ix, q, 5)                           # the handle is still healthy
+    compare(gs, tiny.docs, q, tiny.vocab, 5, ids, sc)
+    ix.close()
