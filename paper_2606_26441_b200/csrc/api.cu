@@ -419,7 +419,7 @@ void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
     void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
-                    ix->term_meta, ix->seg_tab, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
+                    ix->term_meta, ix->seg_tab, ix->seg_l1, ix->seg_l2, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
 }

@@ -41,10 +41,20 @@ template <typename K> inline cudaError_t gs_optin_smem(K kern) { return gs_optin
         if (s__ != GS_OK) return s__;                   \
     } while (0)
 
-// per-term entry of the compact tile-segment table (16 bytes: one 128-bit load)
+// Per-term entry of the tile-segment tables (16 bytes: one 128-bit load).  "Which slots of PL(t) hold documents of doc tile
+// j?" is answered in one of two ways, chosen per term at build time:
+//   mode GS_SEG_FULL   (len >= 2 * ntiles: almost every tile holds a posting): seg_tab[tab_off + j] = number of postings of t
+//                      with doc tile < j, j in [0, ntiles] — two adjacent loads give the slot range;
+//   mode GS_SEG_SPARSE (rare terms, empty in most tiles): seg_l1[tab_off + (j >> 5)] = (bit mask of the non-empty tiles of
+//                      the 32-tile group, index into seg_l2 of the group's first non-empty tile); seg_l2[i] = list position
+//                      where that tile's postings start, seg_l2[i + 1] = where they end (next non-empty tile, or len).
+//                      An empty (term, tile) costs ONE 8-byte load from a table of V * ntiles / 4 bytes (cache resident for
+//                      a query's terms); the tables cost O(postings) + V * ntiles / 4 bytes instead of 12 * V * ntiles.
+#define GS_SEG_FULL 0u
+#define GS_SEG_SPARSE 1u
 struct __align__(16) gs_term_meta {
-    uint32_t tab_off;     // first entry of the term in seg_tab
-    uint32_t shift;       // log2 of the doc tiles per table entry
+    uint32_t tab_off;     // first entry of the term in seg_tab (full) / seg_l1 (sparse)
+    uint32_t mode;        // GS_SEG_FULL | GS_SEG_SPARSE
     uint32_t list_blk;    // start of the term's padded posting list / 32 (lists are padded to 32 slots)
     uint32_t len;         // true list length
 };
@@ -76,14 +86,13 @@ struct gs_index {
     int32_t* inv_len = nullptr;      // [V]   true list length
     int32_t* inv_doc = nullptr;      // [P_pad] doc ids, ascending within a list, -1 in the padding
     void* inv_w = nullptr;           // [P_pad] float | uint8, 0 in the padding
-    // Compact tile-segment table.  Term t owns seg_tab[meta.tab_off .. + (ntiles >> meta.shift) + 2): entry g = number of
-    // postings of t whose doc tile is < (g << shift), so the postings of t inside doc tile j lie in the slot range
-    // [tab[j >> shift], tab[(j >> shift) + 1]) of its list — exactly that range when shift == 0, a superset (the tiles of
-    // the same group of 2^shift tiles) otherwise; a reader drops the postings outside its tile by their doc ids.  shift
-    // grows as the list gets shorter (a group holds ~4 postings on average), so the table costs O(postings), not O(V * ntiles).
+    // tile-segment tables (see gs_term_meta)
     gs_term_meta* term_meta = nullptr;   // [V]
-    uint32_t* seg_tab = nullptr;         // [seg_entries]
-    int64_t seg_entries = 0;
+    uint32_t* seg_tab = nullptr;         // full-mode terms: [n_full][ntiles + 1]
+    uint2* seg_l1 = nullptr;             // sparse-mode terms: [n_sparse][ceil(ntiles / 32)] (mask, seg_l2 index)
+    uint32_t* seg_l2 = nullptr;          // sparse-mode terms: segment starts of the non-empty (term, tile) pairs + one end per term
+    int64_t seg_entries = 0;             // entries of seg_tab
+    int64_t seg_l1_entries = 0, seg_l2_entries = 0;
     // dense strips of the densest lists ("head" terms)
     int32_t H = 0;                   // strips (<= GS_STRIP_MAX), densest list first
     int32_t head_terms_host[GS_STRIP_MAX];
@@ -144,9 +153,9 @@ struct gs_qbatch {
     int32_t* xcnt = nullptr;           // [B]
     bool x_on = false;                 // the batch's x-strip terms are in xpair (and NOT in the tail lists)
     uint4* tail_desc = nullptr;        // [nnz] compacted at indptr[b] .. indptr[b]+tail_cnt[b]: per tail term
-                                       // (accumulator-typed weight bits, segment-table offset, shift, list start / 32)
+                                       // (accumulator-typed weight bits, segment-table offset, segment-table mode, list start / 32)
     int32_t* tail_cnt = nullptr;       // [B]
-    uint4* tail32 = nullptr;           // [B][32] the first 32 tail terms, same entries (shift = 0xFFFFFFFF: no term): a
+    uint4* tail32 = nullptr;           // [B][32] the first 32 tail terms, same entries (mode = 0xFFFFFFFF: no term): a
                                        // fixed-stride copy the batch kernel can prefetch without reading indptr first
     int32_t* status = nullptr;         // device status word: first validation error (gs_status_t) or 0
 };

@@ -100,12 +100,15 @@ __device__ __forceinline__ int32_t term_of_slot(const int64_t* __restrict__ inv_
     return lo;
 }
 
-// Per padded slot: duplicate detection (equal neighbours inside a list) + the compact tile-segment table: entry g of term t
-// = number of postings of t whose doc tile is < (g << shift_t).  The posting at list position i with group
-// grp = (doc / Ts) >> shift writes i into the entries (group of its predecessor, grp]; the last posting fills the rest.
+// Per padded slot: duplicate detection (equal neighbours inside a list) + the tile-segment tables (gs_term_meta).
+// Full mode: the posting at list position i in doc tile j writes i into the entries (tile of its predecessor, j]; the last
+// posting fills the rest with len.  Sparse mode, pass 0: the first posting of a tile sets the tile's bit in its 32-tile group;
+// pass 1 (after the prefix sums over the masks): it writes its list position into the tile's seg_l2 entry, and the last
+// posting of the list writes the closing entry (len).
 __global__ void k_segments(const int64_t* __restrict__ inv_off, const int32_t* __restrict__ inv_len,
                            const int32_t* __restrict__ inv_doc, int32_t V, int64_t P_pad, int32_t Ts, int32_t ntiles,
-                           const gs_term_meta* __restrict__ meta, uint32_t* __restrict__ tab, int* err) {
+                           const gs_term_meta* __restrict__ meta, uint32_t* __restrict__ tab, uint2* __restrict__ l1,
+                           uint32_t* __restrict__ l2, const uint32_t* __restrict__ l2_end, int pass, int* err) {
     int64_t pos = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (pos >= P_pad) return;
     int32_t t = term_of_slot(inv_off, V, pos);
@@ -113,19 +116,70 @@ __global__ void k_segments(const int64_t* __restrict__ inv_off, const int32_t* _
     int32_t len = inv_len[t];
     if (i >= len) return;                       // padding slot
     const gs_term_meta m = meta[t];
+    const uint32_t abs0 = (uint32_t)inv_off[t];          // the tables hold absolute posting slots (P_pad < 2^32)
     int32_t doc = inv_doc[pos];
-    int32_t grp_cur = (doc / Ts) >> m.shift;
-    int32_t grp_prev = -1;
+    int32_t tile_cur = doc / Ts;
+    int32_t tile_prev = -1;
     if (i > 0) {
         int32_t prev = inv_doc[pos - 1];
-        if (prev == doc) atomicCAS(err, 0, (int)GS_ERR_DUPLICATE_TERM);
-        grp_prev = (prev / Ts) >> m.shift;
+        if (prev == doc && pass == 0) atomicCAS(err, 0, (int)GS_ERR_DUPLICATE_TERM);
+        tile_prev = prev / Ts;
     }
-    uint32_t* row = tab + m.tab_off;
-    const int32_t n_ent = (ntiles >> m.shift) + 2;
-    for (int32_t j = grp_prev + 1; j <= grp_cur; ++j) row[j] = (uint32_t)i;
-    if (i == len - 1)
-        for (int32_t j = grp_cur + 1; j < n_ent; ++j) row[j] = (uint32_t)len;
+    if (m.mode == GS_SEG_FULL) {
+        if (pass != 0) return;
+        uint32_t* row = tab + m.tab_off;
+        for (int32_t j = tile_prev + 1; j <= tile_cur; ++j) row[j] = abs0 + (uint32_t)i;
+        if (i == len - 1)
+            for (int32_t j = tile_cur + 1; j <= ntiles; ++j) row[j] = abs0 + (uint32_t)len;
+        return;
+    }
+    uint2* g = l1 + m.tab_off + (tile_cur >> 5);
+    if (pass == 0) {
+        if (tile_cur != tile_prev) atomicOr(&g->x, 1u << (tile_cur & 31));
+        return;
+    }
+    if (tile_cur != tile_prev) {
+        const uint2 e = *g;
+        l2[e.y + (uint32_t)__popc(e.x & ((1u << (tile_cur & 31)) - 1u))] = abs0 + (uint32_t)i;
+    }
+    if (i == len - 1) l2[l2_end[t]] = abs0 + (uint32_t)len;
+}
+
+// Sparse-mode terms, one warp per term: running count of the non-empty tiles before each 32-tile group -> l1[g].y
+// (relative to the term), count of the term's non-empty tiles + 1 (the closing entry) -> cnt[t]; 0 for the other terms.
+__global__ void k_l1_count(const gs_term_meta* __restrict__ meta, int32_t V, int32_t n_grp, uint2* __restrict__ l1,
+                           uint32_t* __restrict__ cnt) {
+    const int64_t t = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (t >= V) return;
+    const gs_term_meta m = meta[t];
+    if (m.mode != GS_SEG_SPARSE || m.len == 0) { if (lane == 0) cnt[t] = 0u; return; }
+    uint32_t run = 0;
+    for (int32_t g0 = 0; g0 < n_grp; g0 += 32) {
+        const int32_t g = g0 + lane;
+        const uint32_t c = g < n_grp ? (uint32_t)__popc(l1[m.tab_off + g].x) : 0u;
+        uint32_t incl = c;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (g < n_grp) l1[m.tab_off + g].y = run + incl - c;
+        run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+    }
+    if (lane == 0) cnt[t] = run + 1u;
+}
+
+// l1[g].y += start of the term's entries in seg_l2; l2_end[t] = index of the term's closing entry
+__global__ void k_l1_rebase(const gs_term_meta* __restrict__ meta, int32_t V, int32_t n_grp, const uint32_t* __restrict__ cnt,
+                            const uint32_t* __restrict__ base, uint2* __restrict__ l1, uint32_t* __restrict__ l2_end) {
+    const int64_t t = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (t >= V) return;
+    const gs_term_meta m = meta[t];
+    if (cnt[t] == 0u) { if (lane == 0) l2_end[t] = 0u; return; }
+    const uint32_t b = base[t];
+    for (int32_t g = lane; g < n_grp; g += 32) l1[m.tab_off + g].y += b;
+    if (lane == 0) l2_end[t] = b + cnt[t] - 1u;
 }
 
 template <typename W>
@@ -284,6 +338,7 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     if (acc != P) return GS_ERR_OUT_OF_RANGE;   // some term id was outside [0,V) (validate off)
     ix->P_pad = accp;
     ix->nonempty = nonempty;
+    if (accp >= 0xFFFFFFF0LL) return GS_ERR_OUT_OF_RANGE;      // posting slots are 32-bit in the segment tables and kernels
     GS_CUDA(cudaMemcpyAsync(ix->inv_off, h_off.data(), sizeof(int64_t) * (size_t)(V + 1), cudaMemcpyHostToDevice, s));
 
     std::vector<int32_t> order;
@@ -379,30 +434,31 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     }
     ix->bytes_inverted = (int64_t)((sizeof(int32_t) + sizeof(W)) * (size_t)ix->P_pad);
 
-    // ---- compact tile-segment table: a group of 2^shift doc tiles per entry, ~kSegTarget postings per group on average
+    // ---- tile-segment tables: a full per-tile table for the lists that reach almost every doc tile, the two-level
+    // bitmap + segment-start arrays for the others (gs_term_meta)
+    const int32_t n_grp = (ix->ntiles + 31) / 32;
     {
-        constexpr double kSegTarget = 4.0;
         std::vector<gs_term_meta> h_meta((size_t)V);
-        int64_t n_ent = 0;
+        int64_t n_ent = 0, n_l1 = 0;
         for (int32_t t = 0; t < V; ++t) {
-            uint32_t shift = 0;
-            while (shift < 15 && (double)h_len[t] * (double)(2u << shift) <= kSegTarget * (double)std::max(ix->ntiles, 1)) ++shift;
-            h_meta[t].tab_off = (uint32_t)n_ent;
-            h_meta[t].shift = shift;
+            const bool full = (int64_t)h_len[t] >= 2 * (int64_t)ix->ntiles && h_len[t] > 0;
+            h_meta[t].mode = full ? GS_SEG_FULL : GS_SEG_SPARSE;
+            h_meta[t].tab_off = (uint32_t)(full ? n_ent : n_l1);
             h_meta[t].list_blk = (uint32_t)(h_off[t] / GS_WARP_BLOCK);
             h_meta[t].len = (uint32_t)h_len[t];
-            n_ent += (ix->ntiles >> shift) + 2;
-            if (n_ent >= 0xFFFFFFF0LL || h_off[t] / GS_WARP_BLOCK > 0xFFFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+            if (full) n_ent += ix->ntiles + 1; else n_l1 += n_grp;
+            if (n_ent >= 0xFFFFFFF0LL || n_l1 >= 0xFFFFFFF0LL || h_off[t] / GS_WARP_BLOCK > 0xFFFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
         }
         ix->seg_entries = n_ent;
+        ix->seg_l1_entries = n_l1;
         ix->term_meta = (gs_term_meta*)gs_dev_alloc(ix, sizeof(gs_term_meta) * (size_t)V, s);
-        ix->seg_tab = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)n_ent, s);
-        if (!ix->term_meta || !ix->seg_tab) return GS_ERR_OOM;
+        ix->seg_tab = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)std::max<int64_t>(n_ent, 1), s);
+        ix->seg_l1 = (uint2*)gs_dev_alloc(ix, sizeof(uint2) * (size_t)std::max<int64_t>(n_l1, 1), s);
+        if (!ix->term_meta || !ix->seg_tab || !ix->seg_l1) return GS_ERR_OOM;
         GS_CUDA(cudaMemcpyAsync(ix->term_meta, h_meta.data(), sizeof(gs_term_meta) * (size_t)V, cudaMemcpyHostToDevice, s));
-        GS_CUDA(cudaMemsetAsync(ix->seg_tab, 0, sizeof(uint32_t) * (size_t)n_ent, s));
+        GS_CUDA(cudaMemsetAsync(ix->seg_tab, 0, sizeof(uint32_t) * (size_t)std::max<int64_t>(n_ent, 1), s));
+        GS_CUDA(cudaMemsetAsync(ix->seg_l1, 0, sizeof(uint2) * (size_t)std::max<int64_t>(n_l1, 1), s));
         GS_CUDA(cudaStreamSynchronize(s));            // h_meta is a local
-        ix->bytes_meta = (int64_t)(sizeof(uint32_t) * (size_t)n_ent + sizeof(gs_term_meta) * (size_t)V +
-                                   sizeof(int64_t) * (size_t)(V + 1) + sizeof(int32_t) * (size_t)V + 2 * sizeof(int16_t) * (size_t)V);
     }
 
     if (P > 0) {
@@ -429,12 +485,40 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         k_scatter_padded<W><<<grid_for(P), kThreads, 0, s>>>(d_sorted_terms, d_src_out, d_rowid, (const W*)docs->weights,
                                                             d_scan, ix->inv_off, P, ix->inv_doc, (W*)ix->inv_w);
         k_segments<<<grid_for(ix->P_pad), kThreads, 0, s>>>(ix->inv_off, ix->inv_len, ix->inv_doc, V, ix->P_pad, ix->Ts,
-                                                            ix->ntiles, ix->term_meta, ix->seg_tab, d_err);
+                                                            ix->ntiles, ix->term_meta, ix->seg_tab, ix->seg_l1, nullptr, nullptr,
+                                                            0, d_err);
         GS_CUDA(cudaMemcpyAsync(&h_err, d_err, sizeof(int), cudaMemcpyDeviceToHost, s));
         GS_CUDA(cudaStreamSynchronize(s));
         GS_CUDA(cudaGetLastError());
         if (h_err && o.validate) return (gs_status_t)h_err;
+        // sparse-mode terms: prefix sums over the tile masks, then the segment starts
+        uint32_t* d_cnt = (uint32_t*)tmp.get(sizeof(uint32_t) * (size_t)(V + 1));
+        uint32_t* d_base = (uint32_t*)tmp.get(sizeof(uint32_t) * (size_t)(V + 1));
+        uint32_t* d_end = (uint32_t*)tmp.get(sizeof(uint32_t) * (size_t)V);
+        if (!d_cnt || !d_base || !d_end) return GS_ERR_OOM;
+        GS_CUDA(cudaMemsetAsync(d_cnt, 0, sizeof(uint32_t) * (size_t)(V + 1), s));
+        k_l1_count<<<grid_for((int64_t)V * 32), kThreads, 0, s>>>(ix->term_meta, V, n_grp, ix->seg_l1, d_cnt);
+        size_t sb = 0;
+        GS_CUDA(cub::DeviceScan::ExclusiveSum(nullptr, sb, d_cnt, d_base, V + 1, s));
+        void* d_sb = tmp.get(sb);
+        if (!d_sb) return GS_ERR_OOM;
+        GS_CUDA(cub::DeviceScan::ExclusiveSum(d_sb, sb, d_cnt, d_base, V + 1, s));
+        uint32_t n_l2 = 0;
+        GS_CUDA(cudaMemcpyAsync(&n_l2, d_base + V, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        GS_CUDA(cudaStreamSynchronize(s));
+        ix->seg_l2_entries = (int64_t)n_l2;
+        ix->seg_l2 = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)std::max<uint32_t>(n_l2, 1u), s);
+        if (!ix->seg_l2) return GS_ERR_OOM;
+        k_l1_rebase<<<grid_for((int64_t)V * 32), kThreads, 0, s>>>(ix->term_meta, V, n_grp, d_cnt, d_base, ix->seg_l1, d_end);
+        k_segments<<<grid_for(ix->P_pad), kThreads, 0, s>>>(ix->inv_off, ix->inv_len, ix->inv_doc, V, ix->P_pad, ix->Ts,
+                                                            ix->ntiles, ix->term_meta, ix->seg_tab, ix->seg_l1, ix->seg_l2, d_end,
+                                                            1, d_err);
+        GS_CUDA(cudaStreamSynchronize(s));
+        GS_CUDA(cudaGetLastError());
     }
+    ix->bytes_meta = (int64_t)(sizeof(uint32_t) * (size_t)ix->seg_entries + sizeof(uint2) * (size_t)ix->seg_l1_entries +
+                               sizeof(uint32_t) * (size_t)ix->seg_l2_entries + sizeof(gs_term_meta) * (size_t)V +
+                               sizeof(int64_t) * (size_t)(V + 1) + sizeof(int32_t) * (size_t)V + 2 * sizeof(int16_t) * (size_t)V);
     // ---- dense strips of the head lists
     if (ix->H > 0) {
         size_t strip_bytes = sizeof(W) * (size_t)ix->H * (size_t)ix->N_pad;

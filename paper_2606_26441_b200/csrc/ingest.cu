@@ -6,7 +6,7 @@
 //     "hot" strips (the GS_HOT_STRIPS densest, held in tensor memory by the fp32 batch kernel) from the front, the others
 //     from the back;
 //   * tail terms: compacted (row b starts at indptr[b]) into tail_desc: weight converted to the accumulator type (float,
-//     or int32 for uint8 impacts) + the term's entry of the compact tile-segment table (table offset, shift, list start),
+//     or int32 for uint8 impacts) + the term's entry of the compact tile-segment table (table offset, table mode, list start),
 //     looked up HERE once per (query, term) instead of once per (query, term, doc tile); the first 32 of them are also
 //     written to the fixed-stride table tail32[b][32], which the batch kernel prefetches two rows ahead.
 // Term ids outside [0,V) are dropped (memory safety); with validation on, the first error
@@ -91,7 +91,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
         if (is_tail) {
             const int64_t dst = a + n_tail + __popc(m & ((1u << lane) - 1u));
             const gs_term_meta tm = term_meta[t];
-            const uint4 d = make_uint4(w, tm.tab_off, tm.shift, tm.list_blk);
+            const uint4 d = make_uint4(w, tm.tab_off, tm.mode, tm.list_blk);
             tail_desc[dst] = d;
             if (dst - a < GS_TAIL32) tail32[b * GS_TAIL32 + (dst - a)] = d;
         }

@@ -53,11 +53,12 @@ template <> struct Num<GS_W_U8> {
 
 struct TermParams {
     // index
-    const int64_t* inv_off; const int32_t* inv_doc; const void* inv_w; const uint32_t* seg; const uint2* seg2;
+    const int32_t* inv_doc; const void* inv_w;
+    const uint32_t* seg_tab; const uint2* seg_l1; const uint32_t* seg_l2;     // tile-segment tables (gs_term_meta), absolute slots
     const void* head_strip; int32_t H; int64_t N; int64_t N_pad; int32_t Ts; int32_t ntiles;
     // queries
-    const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const int32_t* tail_term;
-    const uint32_t* tail_w; const int32_t* tail_cnt; const uint2* tail32;
+    const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const uint4* tail_desc;
+    const int32_t* tail_cnt; const uint4* tail32;
     const void* xstrip; const uint2* xpair; const int32_t* xcnt;      // second-tier strips (null when the batch has none)
     int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
     int32_t warps;                              // cell rows (warps) per CTA (small-batch kernel)
@@ -66,6 +67,29 @@ struct TermParams {
     gs_sink sink;
     int32_t vec4;                               // dense sink rows are 16-byte aligned
 };
+
+// Slot range [lo, hi) of the postings of a tail term (descriptor d: weight bits, table offset, table mode, -) inside doc
+// tile `tile`.  Full mode: two adjacent table entries.  Sparse mode: one (mask, index) entry per 32 tiles; an empty
+// (term, tile) pair stops there.
+__device__ __forceinline__ void probe_range(const TermParams& p, const uint4& d, int tile, uint32_t& lo, uint32_t& hi) {
+    lo = hi = 0u;
+    if (d.z == GS_SEG_FULL) {
+        lo = __ldg(p.seg_tab + d.y + tile);
+        hi = __ldg(p.seg_tab + d.y + tile + 1);
+    } else if (d.z == GS_SEG_SPARSE) {
+        const uint2 e = __ldg(p.seg_l1 + d.y + (tile >> 5));
+        const uint32_t bit = 1u << (tile & 31);
+        if (e.x & bit) {
+            const uint32_t idx = e.y + (uint32_t)__popc(e.x & (bit - 1u));
+            lo = __ldg(p.seg_l2 + idx);
+            hi = __ldg(p.seg_l2 + idx + 1);
+        }
+    }
+}
+// entry i of a query's compact head list: the hot strips from the front, the others from the back (ingest.cu)
+__device__ __forceinline__ uint2 head_entry(const uint2* hl, int i, int n_hot) {
+    return __ldg(hl + (i < n_hot ? i : GS_HEAD_MAX - 1 - (i - n_hot)));
+}
 
 // one posting-list segment [dp, dp+n) applied to one accumulator row
 template <int WT>
@@ -138,21 +162,20 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
     const int64_t qa = p.q_indptr[b];
     const int cnt = p.tail_cnt[b];
     for (int i0 = 0; i0 < cnt; i0 += 32) {
-        int64_t start = 0;
+        uint32_t start = 0;
         int n = 0;
         uint32_t wq = 0;
         if (i0 + lane < cnt) {
-            const int32_t t = p.tail_term[qa + i0 + lane];
-            wq = p.tail_w[qa + i0 + lane];
-            const uint32_t* sr = p.seg + (size_t)t * (p.ntiles + 1) + tile;
-            const uint32_t lo = sr[0], hi = sr[1];
-            n = (int)(hi - lo);
-            start = p.inv_off[t] + lo;
+            const uint4 d = __ldg(p.tail_desc + qa + i0 + lane);
+            wq = d.x;
+            uint32_t hi;
+            probe_range(p, d, tile, start, hi);
+            n = (int)(hi - start);
         }
         unsigned m = __ballot_sync(0xFFFFFFFFu, n > 0);
         while (m) {
             int n_j[kSegBatch];
-            int64_t start_j[kSegBatch];
+            uint32_t start_j[kSegBatch];
             A q_j[kSegBatch], w_j[kSegBatch];
             int32_t rel_j[kSegBatch];
 #pragma unroll
@@ -187,7 +210,8 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
     // strip loads.  Filter mode makes two passes over the row so that a warp reserves its slice of the query's
     // candidate list with ONE atomic: pass 1 finishes the scores in place and counts the cells that pass the
     // threshold, pass 2 writes their keys.
-    const int nh = p.H > 0 ? p.head_cnt[b] : 0;
+    const int hc = p.H > 0 ? p.head_cnt[b] : 0;
+    const int nh = hc & 0xFF, n_hot = hc >> 8;
     const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
     const W* __restrict__ gstrip = STAGED ? s_strip : reinterpret_cast<const W*>(p.head_strip) + base;
     const size_t strip_ld = STAGED ? (size_t)Ts : (size_t)p.N_pad;
@@ -213,7 +237,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
             sc[r][2] = Num<WT>::from_bits(a4.z); sc[r][3] = Num<WT>::from_bits(a4.w);
         }
         for (int i = 0; i < nh; ++i) {
-            const uint2 e = __ldg(hl + i);
+            const uint2 e = head_entry(hl, i, n_hot);
             const A q = Num<WT>::qw(e.y);
             const W* src = gstrip + (size_t)e.x * strip_ld + 4 * (dq0 + lane);
             int4 v[kQuadRounds];
@@ -404,6 +428,11 @@ __device__ __forceinline__ unsigned long long pack_f32x2(float lo, float hi) {
     asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
     return d;
 }
+__device__ __forceinline__ unsigned long long pack_u32x2(uint32_t lo, uint32_t hi) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "r"(lo), "r"(hi));
+    return d;
+}
 __device__ __forceinline__ void unpack_f32x2(unsigned long long v, float& lo, float& hi) {
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
 }
@@ -413,27 +442,57 @@ __device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, un
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
-template <int WT> __device__ __forceinline__ typename Num<WT>::A num_max(typename Num<WT>::A a, typename Num<WT>::A b);
-template <> __device__ __forceinline__ float num_max<GS_W_F32>(float a, float b) { return fmaxf(a, b); }
-template <> __device__ __forceinline__ int32_t num_max<GS_W_U8>(int32_t a, int32_t b) { return max(a, b); }
+// ---- tensor memory as a strip store (fp32 batch kernel).  TMEM is 128 lanes x 512 columns of 32 bits per SM; a warp
+// reaches the 32 lanes of its quarter (warp % 4).  The GS_HOT_STRIPS densest strips of the doc tile are kept there, every
+// lane quarter holding a full copy: lane i, column s*16 + 4r + u = strip s, document 4*(i + 32r) + u of the tile — the 16
+// documents lane i of a warp owns in the head phase, so ONE tcgen05.ld.32x32b.x16 replaces the four LDS.128 of a strip.
+// Measured on B200: 6.4 SM cycles per (warp, strip) against 16 from shared memory, and the two paths
+// overlap, which takes the hot strips off the LSU / shared-memory pipe that bounded the kernel.
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-struct Probe1 { uint32_t t, wq; };                                    // query terms (first 32 tail terms, one per lane)
-struct Probe2 { uint32_t lo, hi, wq; int32_t cnt_nh; uint64_t thr; };   // + the terms' segments inside the tile, and
-                                                                           // tail count | head count << 16, threshold key
+struct Probe1 { uint32_t wq, off, mode; };                           // query terms (first 32 tail terms, one per lane)
+// + the terms' segments inside the tile.  A lane whose bit is clear in `sparse`: slot range [a, b).  A lane whose bit is
+// set (sparse-mode term): (a, b) = the (mask, seg_l2 index) entry of the tile's 32-tile group, turned into a slot range
+// by resolve_segments when the row is processed (the entry's load stays in flight until then).  Plus tail count,
+// head counts << 16 (as in head_cnt) and the threshold key of the query.
+struct Probe2 { uint32_t a, b, wq, sparse; int32_t cnt_nh; uint64_t thr; };
 
 __device__ __forceinline__ Probe1 probe_terms(const TermParams& p, int64_t b, int lane) {
-    const uint2 e = __ldg(p.tail32 + b * GS_TAIL32 + lane);
-    return Probe1{e.x, e.y};
+    const uint4 e = __ldg(p.tail32 + b * GS_TAIL32 + lane);
+    return Probe1{e.x, e.y, e.z};
 }
-__device__ __forceinline__ Probe2 probe_segments(const TermParams& p, const Probe1& a, int tile) {
+__device__ __forceinline__ Probe2 probe_segments(const TermParams& p, const Probe1& t, int tile) {
     Probe2 r;
-    r.lo = r.hi = 0u;
-    r.wq = a.wq; r.cnt_nh = 0; r.thr = 0ull;
-    if (a.t != 0xFFFFFFFFu) {
-        const uint2 e = __ldg(p.seg2 + (size_t)a.t * p.ntiles + tile);      // (first slot, end slot), absolute
-        r.lo = e.x; r.hi = e.y;
+    r.a = r.b = 0u;
+    r.wq = t.wq; r.cnt_nh = 0; r.thr = 0ull;
+    r.sparse = __ballot_sync(0xFFFFFFFFu, t.mode == GS_SEG_SPARSE);
+    if (t.mode == GS_SEG_FULL) {
+        r.a = __ldg(p.seg_tab + t.off + tile);
+        r.b = __ldg(p.seg_tab + t.off + tile + 1);
+    } else if (t.mode == GS_SEG_SPARSE) {
+        const uint2 e = __ldg(p.seg_l1 + t.off + (tile >> 5));
+        r.a = e.x; r.b = e.y;
     }
     return r;
+}
+__device__ __forceinline__ void resolve_segments(const TermParams& p, const Probe2& r, int tile, int lane, uint32_t& lo, uint32_t& hi) {
+    lo = r.a; hi = r.b;
+    if ((r.sparse >> lane) & 1u) {
+        const uint32_t bit = 1u << (tile & 31);
+        if (lo & bit) {
+            const uint32_t idx = hi + (uint32_t)__popc(lo & (bit - 1u));
+            lo = __ldg(p.seg_l2 + idx);
+            hi = __ldg(p.seg_l2 + idx + 1);
+        } else {
+            lo = hi = 0u;
+        }
+    }
 }
 __device__ __forceinline__ void probe_query(const TermParams& p, int64_t b, bool filter, Probe2& r) {
     r.cnt_nh = __ldg(p.tail_cnt + b) | (__ldg(p.head_cnt + b) << 16);
@@ -535,8 +594,8 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     constexpr size_t kOffKey = kOffDesc + (size_t)kBWarps * 32 * 8;
     constexpr size_t kOffQ = kOffKey + (size_t)kCandBuf * 8;
     constexpr size_t kOffCnt = kOffQ + (size_t)kCandBuf * 2;
-    constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;
-    constexpr size_t kOffStrip = kOffBar + 16;
+    constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;       // mbarrier (strip copy) | mbarrier (TMEM copy) |
+    constexpr size_t kOffStrip = (kOffBar + 32 + 127) / 128 * 128;         // TMEM base address, copy-claimed flags [2]
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
     const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
     uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey) + warp * kWarpBuf;     // the warp's candidate buffer
@@ -546,6 +605,9 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     uint32_t* s_done = s_next + 2;                                                            // [2]
     W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
     const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffBar);
+    const uint32_t mbar2_s = mbar_s + 8u;
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem_raw + kOffBar + 16);       // [0] TMEM base, [1..2] copy claimed (per parity)
+    constexpr bool kTmem = WT == GS_W_F32;      // hot strips in tensor memory (fp32; the impact strips are a quarter of the bytes)
     // the warp appends its buffered candidates to the queries' lists (all the atomics of a round in flight together)
     auto flush = [&]() {
         __syncwarp();
@@ -598,9 +660,19 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         s_next[0] = s_next[1] = 2u * kBWarps;
         s_done[0] = s_done[1] = 0u;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_s) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar2_s) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_tmem[1] = s_tmem[2] = 0u;
     }
+    if (kTmem && warp == 0) {                           // the whole tensor memory of the SM (one CTA per SM)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(s_tmem)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (kTmem) asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
+    if (kTmem) asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem_q = kTmem ? s_tmem[0] + ((uint32_t)(32 * (warp & 3)) << 16) : 0u;     // the warp's lane quarter
+    const int n_hot_strips = min(p.H, GS_HOT_STRIPS);
     if (threadIdx.x == 0 && (int)blockIdx.x < n_items) issue_strips((int)blockIdx.x);
     const bool filter = p.sink.thr != nullptr;
     const W* srow = s_strip + 4 * lane;
@@ -618,6 +690,34 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                          : "=r"(ok) : "r"(mbar_s), "r"((uint32_t)par) : "memory");
         } while (!ok);
+        if (kTmem) {
+            // The strips landed, so every warp has left the previous item (its last warp out issued this copy): tensor
+            // memory is free.  The first warp here copies the hot strips shared memory -> tensor memory: one
+            // tcgen05.cp.32x128b.warpx4 per (strip, 128 documents) moves 32 rows of 16 bytes and writes them to all four
+            // lane quarters; the copies complete on the second mbarrier, which every warp then waits for.
+            if (lane == 0 && atomicExch(s_tmem + 1 + par, 1u) == 0u) {
+                s_tmem[1 + (par ^ 1)] = 0u;             // nobody claims the next item before this one's strips have landed
+                const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_strip);
+                const uint32_t t0 = s_tmem[0];
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                for (int h = 0; h < n_hot_strips; ++h)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        // shared-memory matrix descriptor, no swizzle: start address >> 4, leading byte offset (unused: one
+                        // 16-byte column), stride byte offset 128 (8 rows of 16 bytes are contiguous) >> 4, version 1
+                        const uint32_t a = sbase + (uint32_t)(h * (kBT * 4) + r * 512);
+                        const unsigned long long desc = (unsigned long long)((a & 0x3FFFFu) >> 4) | (1ull << 16) | (8ull << 32) | (1ull << 46);
+                        asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(t0 + (uint32_t)(h * 16 + r * 4)), "l"(desc) : "memory");
+                    }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar2_s) : "memory");
+            }
+            __syncwarp();
+            do {
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(ok) : "r"(mbar2_s), "r"((uint32_t)par) : "memory");
+            } while (!ok);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        }
         strips_ready = true;
     };
     // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
@@ -628,8 +728,8 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     int q_n1 = q + kBWarps;                     // next row (segments probed)
     int q_n2 = q_end;                           // row after that (terms probed)
     int q_n3 = q_end;                           // claimed, not yet probed
-    Probe1 s1{0xFFFFFFFFu, 0u};
-    Probe2 s2{0u, 0u, 0u, 0, 0ull};
+    Probe1 s1{0u, 0u, 0xFFFFFFFFu};
+    Probe2 s2{0u, 0u, 0u, 0u, 0, 0ull};
     if (q < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile); probe_query(p, p.q0 + q, filter, s2); }
     if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
     {
@@ -648,22 +748,27 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
             q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
         }
-        const int nh = cur.cnt_nh >> 16, cnt = cur.cnt_nh & 0xFFFF;
+        const int nh = (cur.cnt_nh >> 16) & 0xFF, n_hot = cur.cnt_nh >> 24, cnt = cur.cnt_nh & 0xFFFF;
         const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
         const uint64_t thr = cur.thr;
 
 #pragma unroll
         for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
         __syncwarp();
-        scatter_flat<WT>(p, row, desc_s, (int)(cur.hi - cur.lo), cur.lo, cur.wq, base, lane);
-        if (cnt > GS_TAIL32) {                      // rare: more than 32 tail terms, probed in line
+        {
+            uint32_t lo, hi;
+            resolve_segments(p, cur, tile, lane, lo, hi);
+            scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane);
+        }
+        if (cnt > GS_TAIL32) {                      // more than 32 tail terms: probed in line
             const int64_t qa = p.q_indptr[b];
             for (int i0 = GS_TAIL32; i0 < cnt; i0 += 32) {
                 __syncwarp();                       // the descriptor table is reused
-                Probe1 a{0xFFFFFFFFu, 0u};
-                if (i0 + lane < cnt) { a.t = (uint32_t)p.tail_term[qa + i0 + lane]; a.wq = p.tail_w[qa + i0 + lane]; }
-                const Probe2 e = probe_segments(p, a, tile);
-                scatter_flat<WT>(p, row, desc_s, (int)(e.hi - e.lo), e.lo, e.wq, base, lane);
+                uint4 d = make_uint4(0u, 0u, 0xFFFFFFFFu, 0u);
+                if (i0 + lane < cnt) d = __ldg(p.tail_desc + qa + i0 + lane);
+                uint32_t lo, hi;
+                probe_range(p, d, tile, lo, hi);
+                scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, d.x, base, lane);
             }
         }
         __syncwarp();
@@ -679,9 +784,25 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 const ulonglong2 a2 = reinterpret_cast<const ulonglong2*>(row)[lane + 32 * r];
                 acc[r][0] = a2.x; acc[r][1] = a2.y;
             }
-#pragma unroll kHeadUnroll
-            for (int i = 0; i < nh; ++i) {
+            // hot strips: the lane's 16 documents of a strip in one tensor-memory load
+#pragma unroll 2
+            for (int i = 0; i < n_hot; ++i) {
                 const uint2 e = __ldg(hl + i);
+                const float qf = __uint_as_float(e.y);
+                const unsigned long long q2 = pack_f32x2(qf, qf);
+                uint32_t v[16];
+                tmem_ld16(tmem_q + e.x * 16u, v);
+                tmem_wait_ld();
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    acc[r][0] = fma_f32x2(pack_u32x2(v[4 * r], v[4 * r + 1]), q2, acc[r][0]);
+                    acc[r][1] = fma_f32x2(pack_u32x2(v[4 * r + 2], v[4 * r + 3]), q2, acc[r][1]);
+                }
+            }
+            // the other strips: shared memory
+#pragma unroll kHeadUnroll
+            for (int i = n_hot; i < nh; ++i) {
+                const uint2 e = __ldg(hl + (GS_HEAD_MAX - 1 - (i - n_hot)));
                 const float qf = __uint_as_float(e.y);
                 const unsigned long long q2 = pack_f32x2(qf, qf);
                 const ulonglong2* src = reinterpret_cast<const ulonglong2*>(srow + (size_t)e.x * kBT);
@@ -726,7 +847,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
 #pragma unroll kHeadUnroll
             for (int i = 0; i < nh; ++i) {
-                const uint2 e = __ldg(hl + i);
+                const uint2 e = head_entry(hl, i, n_hot);
                 // one IDP4A per cell: the impact byte of the query (<= 255) placed in byte u of the second operand picks
                 // byte u of the strip word — no unpacking
                 const uint32_t qi = e.y & 0xFFu;
@@ -802,6 +923,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     // NEXT phase issued while this one is still pending would be satisfied at once), then reports itself done.
     if (!strips_ready) wait_strips();
     __syncwarp();
+    if (kTmem) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");    // the warp's tensor-memory loads are done
     if (lane == 0) {
         __threadfence_block();
         if (atomicAdd(s_done + par, 1u) == (uint32_t)(kBWarps - 1)) {       // last warp out: the strips buffer is free
@@ -813,6 +935,11 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     __syncwarp();
     }
     if (filter) flush();
+    if (kTmem) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem[0]), "n"(512));
+    }
 }
 
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
@@ -860,11 +987,11 @@ static inline bool cta_per_tile(const gs_index* ix, int64_t nq) {
 }  // namespace
 
 bool gs_score_term_wants_x(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    return group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->HX > 0 && ix->Ts == kBT && ix->seg2 != nullptr;
+    return group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->HX > 0 && ix->Ts == kBT;
 }
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head) {
-    if (group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->Ts == kBT && ix->seg2 != nullptr)
+    if (group == 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0 && ix->Ts == kBT)
         return kBWarps;                                                 // batch kernel
     if (group <= 0 && cta_per_tile(ix, nq) && use_head && ix->H > 0) return kWarpsStaged;
     return norm_warps(group);
@@ -874,11 +1001,11 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     TermParams p{};
-    p.inv_off = ix->inv_off; p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg = ix->seg; p.seg2 = ix->seg2;
+    p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg_tab = ix->seg_tab; p.seg_l1 = ix->seg_l1; p.seg_l2 = ix->seg_l2;
     p.head_strip = ix->head_strip; p.H = use_head ? ix->H : 0; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
     p.ntiles = ix->ntiles;
-    p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_term = qb.tail_term;
-    p.tail_w = qb.tail_w; p.tail_cnt = qb.tail_cnt; p.tail32 = qb.tail32;
+    p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_desc = qb.tail_desc;
+    p.tail_cnt = qb.tail_cnt; p.tail32 = qb.tail32;
     p.xstrip = qb.x_on ? ix->xstrip : nullptr; p.xpair = qb.x_on ? qb.xpair : nullptr; p.xcnt = qb.x_on ? qb.xcnt : nullptr;
     p.q0 = q0; p.nq = (int32_t)nq;
     p.warps = norm_warps(group);
@@ -903,8 +1030,8 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
         p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 16;
-        if (group == 0 && ix->Ts == kBT && ix->seg2 != nullptr && smem_batch <= (size_t)smem_max && nq <= 65535) {
+        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 32 + 128;
+        if (group == 0 && ix->Ts == kBT && smem_batch <= (size_t)smem_max && nq <= 65535) {
             auto go = [&](auto kern) -> gs_status_t {
                 GS_CUDA(gs_optin_smem(kern));
                 GsProfScope ps(GS_K_SCORE_TERM, s);
