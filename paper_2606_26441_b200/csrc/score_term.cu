@@ -401,9 +401,14 @@ __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(cons
 //     order of the additions into a cell is the query's term order: deterministic, no atomics;
 //   * the probes (query terms -> segment table -> list offsets) of the NEXT TWO queries of the warp are prefetched
 //     (two-stage software pipeline) from the fixed-stride tail32 table;
-//   * head: a lane keeps its 16 documents in registers, one 128-bit shared-memory load feeds two FFMA2;
-//   * filter: one max over the lane's 16 scores and one ballot reject a row chunk that holds no candidate (the common
-//     case) before any per-cell test or write-back.
+//   * head: a lane keeps its 16 documents in registers.  The query's compact strip lists are loaded once, one entry per
+//     lane, and broadcast by shuffle.  fp32: the GS_HOT_STRIPS densest strips of the tile live in TENSOR MEMORY (one
+//     tcgen05.ld.32x32b.x16 per strip feeds eight FFMA2, see tmem_ld16_wait), the other strips in shared memory (one
+//     LDS.128 feeds two FFMA2), the second-tier strips come from global memory.  Integer mode: one IDP4A per cell;
+//   * filter: a cell that reaches the threshold score goes to the warp's candidate buffer in shared memory.
+// Things measured and dropped in round 2 (profiles/r02_kernels.md): a 16-warp x 128-register variant that worked on two
+// rows per warp (one per half-warp in the tail phase, strip loads double-buffered) — 20.2 ms against 16.4 ms; an L2
+// prefetch of the next row's posting segments — 16.9 ms.
 // ------------------------------------------------------------------------------------------------
 constexpr int kBT = 512;          // documents per tile
 #ifndef GS_BWARPS
@@ -448,13 +453,19 @@ __device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, un
 // documents lane i of a warp owns in the head phase, so ONE tcgen05.ld.32x32b.x16 replaces the four LDS.128 of a strip.
 // Measured on B200: 6.4 SM cycles per (warp, strip) against 16 from shared memory, and the two paths
 // overlap, which takes the hot strips off the LSU / shared-memory pipe that bounded the kernel.
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                 : "r"(taddr));
+// Loads the lane's 16 documents of one strip and waits for them (tcgen05.wait::ld waits for every tensor-memory load of
+// the thread).  Load, wait and the packing into eight f32x2 operands are ONE asm block, so the compiler cannot move a use
+// of the values above the wait, and ptxas allocates the 16 destination registers as aligned pairs (FFMA2 operands).
+__device__ __forceinline__ void tmem_ld16_wait(uint32_t taddr, unsigned long long (&d)[8]) {
+    asm volatile(
+        "{\n\t.reg .b32 t<16>;\n\t"
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {t0,t1,t2,t3,t4,t5,t6,t7,t8,t9,t10,t11,t12,t13,t14,t15}, [%8];\n\t"
+        "tcgen05.wait::ld.sync.aligned;\n\t"
+        "mov.b64 %0, {t0,t1};\n\tmov.b64 %1, {t2,t3};\n\tmov.b64 %2, {t4,t5};\n\tmov.b64 %3, {t6,t7};\n\t"
+        "mov.b64 %4, {t8,t9};\n\tmov.b64 %5, {t10,t11};\n\tmov.b64 %6, {t12,t13};\n\tmov.b64 %7, {t14,t15};\n\t}"
+        : "=l"(d[0]), "=l"(d[1]), "=l"(d[2]), "=l"(d[3]), "=l"(d[4]), "=l"(d[5]), "=l"(d[6]), "=l"(d[7])
+        : "r"(taddr) : "memory");
 }
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 struct Probe1 { uint32_t wq, off, mode; };                           // query terms (first 32 tail terms, one per lane)
 // + the terms' segments inside the tile.  A lane whose bit is clear in `sparse`: slot range [a, b).  A lane whose bit is
@@ -574,12 +585,103 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
     }
 }
 
+
+
 constexpr int kWarpBuf = 80;                  // candidate keys a warp collects in shared memory before it appends them
 #ifndef GS_FLUSH_AT
 #define GS_FLUSH_AT 40
 #endif
 constexpr int kFlushAt = GS_FLUSH_AT;                  // ... which it does at the end of a row once it holds more than this many
 constexpr int kCandBuf = kBWarps * kWarpBuf;
+
+// ---- cold paths of the batch kernel, kept out of line: the kernel's warps sit in different phases of the row loop, so
+// the loop body has to fit the instruction cache (a 116 KB variant of this kernel ran at half the speed of a 45 KB one).
+
+// The warp appends its buffered candidates to the queries' lists (all the atomics of a round in flight together).  The
+// buffer holds one run of entries per row the warp has finished: the first lane of a run reserves the whole run in its
+// query's list with ONE atomic (same-address atomics of one warp instruction are served one after the other, each a round
+// trip: 32 lanes on two or three counters cost tens of microseconds per flush).
+__device__ __noinline__ void batch_flush(uint32_t* cand_cnt, uint64_t* cand, int64_t cand_cap, int64_t q0, const uint64_t* w_key,
+                                         const uint16_t* w_q, uint32_t* w_cnt, int lane) {
+    __syncwarp();
+    const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)kWarpBuf);
+    const unsigned le_ = 0xFFFFFFFFu >> (31 - lane);
+#pragma unroll 1
+    for (uint32_t i0 = 0; i0 < n_buf; i0 += 32) {
+        const uint32_t i = i0 + lane;
+        const bool valid = i < n_buf;
+        const uint32_t qi = valid ? (uint32_t)w_q[i] : 0xFFFFFFFFu;
+        const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, qi, 1);
+        const bool head = valid && (lane == 0 || qi != prev);
+        const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
+        const int n_valid = __popc(__ballot_sync(0xFFFFFFFFu, valid));
+        const int start = 31 - __clz((int)(heads & le_));                 // first lane of this lane's run
+        const unsigned later = heads & ~le_;
+        const int end = later ? __ffs((int)later) - 1 : n_valid;          // one past the run's last lane
+        const int64_t bb = q0 + (valid ? (int64_t)qi : 0);
+        uint32_t pos = 0;
+        if (head) pos = atomicAdd(&cand_cnt[bb], (uint32_t)(end - lane));
+        pos = __shfl_sync(0xFFFFFFFFu, pos, start & 31) + (uint32_t)(lane - start);
+        if (valid && (int64_t)pos < cand_cap) cand[bb * cand_cap + pos] = w_key[i];
+    }
+    __syncwarp();
+    if (lane == 0) *w_cnt = 0u;
+    __syncwarp();
+}
+
+// One thread: the TMA bulk copies of a work item's strips (one 1-D copy per strip: kBT weights, contiguous in the strip)
+// into shared memory, completing on the mbarrier at mbar_s.
+// g = the first strip at the item's doc tile, ld = elements between strips
+template <typename W>
+__device__ __noinline__ void batch_issue_strips(const W* g, int64_t ld, int H, uint32_t strip_s, uint32_t mbar_s) {
+    const uint32_t row_bytes = (uint32_t)(kBT * sizeof(W));
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_s), "r"(row_bytes * (uint32_t)H) : "memory");
+#pragma unroll 1
+    for (int h = 0; h < H; ++h)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(strip_s + (uint32_t)h * row_bytes), "l"(g + (size_t)h * ld), "r"(row_bytes), "r"(mbar_s) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t mbar_s, uint32_t parity) {
+    uint32_t ok = 0;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(mbar_s), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+// Every warp, once per work item, before its first head phase: waits for the item's strips (TMA, first mbarrier).  With
+// TMEM: the strips landed, so every warp has left the previous item (its last warp out issued this copy) and tensor memory
+// is free.  The first warp here copies the hot strips shared memory -> tensor memory: one tcgen05.cp.32x128b.warpx4 per
+// (strip, 128 documents) moves 32 rows of 16 bytes and writes them to all four lane quarters; the copies complete on the
+// second mbarrier, which every warp then waits for.  s_tmem: [0] TMEM base, [1..2] copy claimed (per parity).
+template <bool TMEM>
+__device__ __noinline__ void batch_wait_strips(uint32_t mbar_s, uint32_t strip_s, uint32_t* s_tmem, int n_hot_strips, int par, int lane) {
+    mbar_wait(mbar_s, (uint32_t)par);
+    if (TMEM) {
+        const uint32_t mbar2_s = mbar_s + 8u;
+        if (lane == 0 && atomicExch(s_tmem + 1 + par, 1u) == 0u) {
+            s_tmem[1 + (par ^ 1)] = 0u;             // nobody claims the next item before this one's strips have landed
+            const uint32_t t0 = s_tmem[0];
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+            for (int h = 0; h < n_hot_strips; ++h)
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    // shared-memory matrix descriptor, no swizzle: start address >> 4, leading byte offset (unused: one
+                    // 16-byte column), stride byte offset 128 (8 rows of 16 bytes are contiguous) >> 4, version 1
+                    const uint32_t a = strip_s + (uint32_t)(h * (kBT * 4) + r * 512);
+                    const unsigned long long d = (unsigned long long)((a & 0x3FFFFu) >> 4) | (1ull << 16) | (8ull << 32) | (1ull << 46);
+                    asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(t0 + (uint32_t)(h * 16 + r * 4)), "l"(d) : "memory");
+                }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar2_s) : "memory");
+        }
+        __syncwarp();
+        mbar_wait(mbar2_s, (uint32_t)par);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    }
+}
 
 template <int WT>
 __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const TermParams p) {
@@ -608,35 +710,6 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     const uint32_t mbar2_s = mbar_s + 8u;
     uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem_raw + kOffBar + 16);       // [0] TMEM base, [1..2] copy claimed (per parity)
     constexpr bool kTmem = WT == GS_W_F32;      // hot strips in tensor memory (fp32; the impact strips are a quarter of the bytes)
-    // the warp appends its buffered candidates to the queries' lists (all the atomics of a round in flight together)
-    auto flush = [&]() {
-        __syncwarp();
-        const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)kWarpBuf);
-        // The buffer holds one run of entries per row the warp has finished: the first lane of a run reserves the whole
-        // run in its query's list with ONE atomic (same-address atomics of one warp instruction are served one after the
-        // other, each a round trip: 32 lanes on two or three counters cost tens of microseconds per flush).
-        const unsigned le_ = 0xFFFFFFFFu >> (31 - lane);
-        for (uint32_t i0 = 0; i0 < n_buf; i0 += 32) {
-            const uint32_t i = i0 + lane;
-            const bool valid = i < n_buf;
-            const uint32_t qi = valid ? (uint32_t)w_q[i] : 0xFFFFFFFFu;
-            const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, qi, 1);
-            const bool head = valid && (lane == 0 || qi != prev);
-            const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
-            const int n_valid = __popc(__ballot_sync(0xFFFFFFFFu, valid));
-            const int start = 31 - __clz((int)(heads & le_));                 // first lane of this lane's run
-            const unsigned later = heads & ~le_;
-            const int end = later ? __ffs((int)later) - 1 : n_valid;          // one past the run's last lane
-            const int64_t bb = p.q0 + (valid ? (int64_t)qi : 0);
-            uint32_t pos = 0;
-            if (head) pos = atomicAdd(&p.sink.cand_cnt[bb], (uint32_t)(end - lane));
-            pos = __shfl_sync(0xFFFFFFFFu, pos, start & 31) + (uint32_t)(lane - start);
-            if (valid && (int64_t)pos < p.sink.cand_cap) p.sink.cand[bb * p.sink.cand_cap + pos] = w_key[i];
-        }
-        __syncwarp();
-        if (lane == 0) *w_cnt = 0u;
-        __syncwarp();
-    };
     // A work item = (doc tile, chunk of queries).  The CTA is persistent: it takes items blockIdx.x, blockIdx.x + gridDim.x, ...
     // The item's strips come in by TMA: one thread issues a 1-D bulk copy per strip (kBT weights, contiguous in the
     // strip) that completes on an mbarrier (one phase per item); a warp waits for it only before its first head phase.
@@ -644,16 +717,9 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     // warp out of an item (shared-memory counter) starts the copy of the next item's strips — nobody reads the old ones
     // any more — so the copy, the item prologue and the slow warps' last rows overlap with the other warps' work.
     const int n_items = p.ts.count * p.n_chunks;
-    auto issue_strips = [&](int item) {                 // one thread
-        const int tile_ = p.ts.first + (item / p.n_chunks) * p.ts.stride;
-        const uint32_t row_bytes = (uint32_t)(kBT * sizeof(W));
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar_s), "r"(row_bytes * (uint32_t)p.H) : "memory");
-        const W* g = reinterpret_cast<const W*>(p.head_strip) + (size_t)tile_ * kBT;
-        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s_strip);
-        for (int h = 0; h < p.H; ++h)
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                         ::"r"(dst + (uint32_t)h * row_bytes), "l"(g + (size_t)h * p.N_pad), "r"(row_bytes), "r"(mbar_s) : "memory");
+    const uint32_t strip_s = (uint32_t)__cvta_generic_to_shared(s_strip);
+    auto item_strips = [&](int item) {
+        return reinterpret_cast<const W*>(p.head_strip) + (size_t)(p.ts.first + (item / p.n_chunks) * p.ts.stride) * kBT;
     };
     if (lane == 0) *w_cnt = 0u;
     if (threadIdx.x == 0) {
@@ -673,7 +739,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     if (kTmem) asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem_q = kTmem ? s_tmem[0] + ((uint32_t)(32 * (warp & 3)) << 16) : 0u;     // the warp's lane quarter
     const int n_hot_strips = min(p.H, GS_HOT_STRIPS);
-    if (threadIdx.x == 0 && (int)blockIdx.x < n_items) issue_strips((int)blockIdx.x);
+    if (threadIdx.x == 0 && (int)blockIdx.x < n_items) batch_issue_strips<W>(item_strips((int)blockIdx.x), p.N_pad, p.H, strip_s, mbar_s);
     const bool filter = p.sink.thr != nullptr;
     const W* srow = s_strip + 4 * lane;
     int it = 0;
@@ -684,42 +750,6 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     const int tile = p.ts.first + j * p.ts.stride;
     const int32_t base = tile * kBT;
     bool strips_ready = false;
-    auto wait_strips = [&]() {                          // the bulk copies of this item's strips have landed
-        uint32_t ok = 0;
-        do {
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                         : "=r"(ok) : "r"(mbar_s), "r"((uint32_t)par) : "memory");
-        } while (!ok);
-        if (kTmem) {
-            // The strips landed, so every warp has left the previous item (its last warp out issued this copy): tensor
-            // memory is free.  The first warp here copies the hot strips shared memory -> tensor memory: one
-            // tcgen05.cp.32x128b.warpx4 per (strip, 128 documents) moves 32 rows of 16 bytes and writes them to all four
-            // lane quarters; the copies complete on the second mbarrier, which every warp then waits for.
-            if (lane == 0 && atomicExch(s_tmem + 1 + par, 1u) == 0u) {
-                s_tmem[1 + (par ^ 1)] = 0u;             // nobody claims the next item before this one's strips have landed
-                const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_strip);
-                const uint32_t t0 = s_tmem[0];
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                for (int h = 0; h < n_hot_strips; ++h)
-#pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        // shared-memory matrix descriptor, no swizzle: start address >> 4, leading byte offset (unused: one
-                        // 16-byte column), stride byte offset 128 (8 rows of 16 bytes are contiguous) >> 4, version 1
-                        const uint32_t a = sbase + (uint32_t)(h * (kBT * 4) + r * 512);
-                        const unsigned long long desc = (unsigned long long)((a & 0x3FFFFu) >> 4) | (1ull << 16) | (8ull << 32) | (1ull << 46);
-                        asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(t0 + (uint32_t)(h * 16 + r * 4)), "l"(desc) : "memory");
-                    }
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar2_s) : "memory");
-            }
-            __syncwarp();
-            do {
-                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                             : "=r"(ok) : "r"(mbar2_s), "r"((uint32_t)par) : "memory");
-            } while (!ok);
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        }
-        strips_ready = true;
-    };
     // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
     // warp and warp + kBWarps of the chunk and claims further ones from a shared-memory counter, two rows ahead of the
     // row it works on (the probes of the next two rows are in flight).
@@ -773,7 +803,10 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         }
         __syncwarp();
 
-        if (!strips_ready) wait_strips();           // once per warp and item
+        if (!strips_ready) {                        // once per warp and item
+            batch_wait_strips<kTmem>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
+            strips_ready = true;
+        }
         // head strips: the lane's 16 documents (quads lane, lane+32, lane+64, lane+96) stay in registers
         const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
         A sc[4][4];
@@ -784,28 +817,29 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 const ulonglong2 a2 = reinterpret_cast<const ulonglong2*>(row)[lane + 32 * r];
                 acc[r][0] = a2.x; acc[r][1] = a2.y;
             }
+            // The query's compact strip lists are loaded once, one entry per lane, and broadcast by shuffle: a load per
+            // strip put an L1 round trip in front of every strip (profiles/r02_kernels.md).
+            const uint2 e_hot = lane < n_hot ? __ldg(hl + lane) : make_uint2(0u, 0u);
+            const uint2 e_cold = lane < nh - n_hot ? __ldg(hl + (GS_HEAD_MAX - 1 - lane)) : make_uint2(0u, 0u);
             // hot strips: the lane's 16 documents of a strip in one tensor-memory load
 #pragma unroll 2
             for (int i = 0; i < n_hot; ++i) {
-                const uint2 e = __ldg(hl + i);
-                const float qf = __uint_as_float(e.y);
+                const float qf = __uint_as_float(__shfl_sync(0xFFFFFFFFu, e_hot.y, i));
                 const unsigned long long q2 = pack_f32x2(qf, qf);
-                uint32_t v[16];
-                tmem_ld16(tmem_q + e.x * 16u, v);
-                tmem_wait_ld();
+                unsigned long long t[8];
+                tmem_ld16_wait(tmem_q + __shfl_sync(0xFFFFFFFFu, e_hot.x, i) * 16u, t);
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
-                    acc[r][0] = fma_f32x2(pack_u32x2(v[4 * r], v[4 * r + 1]), q2, acc[r][0]);
-                    acc[r][1] = fma_f32x2(pack_u32x2(v[4 * r + 2], v[4 * r + 3]), q2, acc[r][1]);
+                    acc[r][0] = fma_f32x2(t[2 * r], q2, acc[r][0]);
+                    acc[r][1] = fma_f32x2(t[2 * r + 1], q2, acc[r][1]);
                 }
             }
             // the other strips: shared memory
-#pragma unroll kHeadUnroll
-            for (int i = n_hot; i < nh; ++i) {
-                const uint2 e = __ldg(hl + (GS_HEAD_MAX - 1 - (i - n_hot)));
-                const float qf = __uint_as_float(e.y);
+#pragma unroll 2
+            for (int i = 0; i < nh - n_hot; ++i) {
+                const float qf = __uint_as_float(__shfl_sync(0xFFFFFFFFu, e_cold.y, i));
                 const unsigned long long q2 = pack_f32x2(qf, qf);
-                const ulonglong2* src = reinterpret_cast<const ulonglong2*>(srow + (size_t)e.x * kBT);
+                const ulonglong2* src = reinterpret_cast<const ulonglong2*>(srow + (size_t)__shfl_sync(0xFFFFFFFFu, e_cold.x, i) * kBT);
                 ulonglong2 v[4];
 #pragma unroll
                 for (int r = 0; r < 4; ++r) v[r] = src[32 * r];
@@ -818,9 +852,12 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (nx > 0) {                          // second-tier strips: same contraction, the strip read from global memory
                 const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
                 const float* gx = reinterpret_cast<const float*>(p.xstrip) + (size_t)base + 4 * lane;
-#pragma unroll kXUnroll
+                const uint2 e_x = lane < nx ? __ldg(xl + lane) : make_uint2(0u, 0u);
+#pragma unroll 1
                 for (int i = 0; i < nx; ++i) {
-                    const uint2 e = __ldg(xl + i);
+                    uint2 e;
+                    if (i < 32) { e.x = __shfl_sync(0xFFFFFFFFu, e_x.x, i); e.y = __shfl_sync(0xFFFFFFFFu, e_x.y, i); }
+                    else e = __ldg(xl + i);
                     const float qf = __uint_as_float(e.y);
                     const unsigned long long q2 = pack_f32x2(qf, qf);
                     const ulonglong2* src = reinterpret_cast<const ulonglong2*>(gx + (size_t)e.x * (size_t)p.N_pad);
@@ -917,11 +954,12 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
         }
         __syncwarp();
-        if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt) flush();
+        if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt)
+            batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
     }
     // out of rows in this item.  Every warp observes every phase of the mbarrier (a warp without rows too: a wait for the
     // NEXT phase issued while this one is still pending would be satisfied at once), then reports itself done.
-    if (!strips_ready) wait_strips();
+    if (!strips_ready) batch_wait_strips<kTmem>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
     __syncwarp();
     if (kTmem) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");    // the warp's tensor-memory loads are done
     if (lane == 0) {
@@ -929,12 +967,12 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         if (atomicAdd(s_done + par, 1u) == (uint32_t)(kBWarps - 1)) {       // last warp out: the strips buffer is free
             s_done[par] = 0u;
             s_next[par] = 2u * kBWarps;                                    // for the item after the next
-            if (item + (int)gridDim.x < n_items) issue_strips(item + (int)gridDim.x);
+            if (item + (int)gridDim.x < n_items) batch_issue_strips<W>(item_strips(item + (int)gridDim.x), p.N_pad, p.H, strip_s, mbar_s);
         }
     }
     __syncwarp();
     }
-    if (filter) flush();
+    if (filter) batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
     if (kTmem) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
