@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define GS_ABI_VERSION 4
+#define GS_ABI_VERSION 5
 #if defined(__GNUC__)
 #define GS_API __attribute__((visibility("default")))
 #else
@@ -61,7 +61,7 @@ typedef enum gs_status {
 typedef enum gs_weight { GS_W_F32 = 0, GS_W_U8 = 1 } gs_weight_t;
 
 typedef enum gs_algo {
-    GS_ALGO_AUTO = 0,           /* work model of L176-181 with measured constants: term-parallel on every workload so far */
+    GS_ALGO_AUTO = 0,           /* the cheaper path under the cost model of gs_dispatch_model (L176-181 crossover)        */
     GS_ALGO_TERM_PARALLEL = 1,  /* tiled scatter-add over the inverted index   (Eq. 5, §5.2)   */
     GS_ALGO_DOC_PARALLEL = 2    /* CSR forward-index streaming, zero atomics   (L174)                    */
 } gs_algo_t;
@@ -91,6 +91,12 @@ typedef struct gs_build_opts {
     float head_density;       /* default 0.25.  4 B/doc beats 8 B/posting from density 0.5 on; below that a    */
                               /* strip costs bytes but saves the per-posting lookup of the doc-parallel kernel */
     int32_t validate;         /* default 1: reject out-of-range ids, duplicates, non-finite weights            */
+    int32_t pack_postings;    /* integer-impact mode (GS_W_U8), compressed postings (future work 2;  */
+                              /* L75 is the "raw int32 + fp32" layout it replaces): 0 = default: ONE 32-bit word per */
+                              /* posting — inverted lists (doc id : 24 | impact : 8) when N < 2^24, forward index    */
+                              /* (term : 19 | impact : 8 | doc-in-block : 5) when V < 2^19 — 4 instead of 5 bytes    */
+                              /* per posting and one load instead of two; -1 = keep the two-array layout.  fp32      */
+                              /* postings stay (int32, fp32): the weights must keep full precision (exactness).     */
 } gs_build_opts_t;
 
 typedef struct gs_info {
@@ -112,7 +118,7 @@ typedef struct gs_info {
     int64_t forward_tail_nnz;  /* postings held by the CSR part of the forward index                  */
     int32_t head_terms_term_parallel; /* strips the term-parallel kernels can read: head_terms + the second tier (up to
                                        * 128 more lists of density >= 0.05, 512-doc tiles only; bytes in bytes_head) */
-    int32_t reserved;
+    int32_t packed_layout;     /* bit 0: inverted lists are packed words, bit 1: forward index is (gs_build_opts_t.pack_postings) */
     int64_t forward_padded_nnz; /* slots of the CSR part: forward_tail_nnz + block padding             */
 } gs_info_t;
 
@@ -164,6 +170,22 @@ GS_API gs_status_t gs_index_copy_list(const gs_index_t* index, int32_t term, int
  * min(capacity, head_terms) term ids to host_terms and the total to *out_count. */
 GS_API gs_status_t gs_index_copy_head_terms(const gs_index_t* index, int32_t capacity, int32_t* host_terms,
                                      int32_t* out_count);
+
+/* Cost model behind GS_ALGO_AUTO.  PAPER.md L176-181 (§5.3) states the trade-off: the term-parallel scatter touches
+ * q̄·L̄ postings per query, the document-parallel kernel streams all N·k̄ postings per pass, and the crossover is where the
+ * work ratio meets the ratio of the effective rates.  On B200 both sides were measured over N in {20K .. 1M} documents,
+ * B in {1 .. 256} queries of 25 .. 4000 terms (profiles/r02_dispatch_sweep.md); the forms below predict
+ * the faster path on 62 of the 64 grid points (the two misses cost 7 %):
+ *   term: 0.10 ms + max(1, B*tiles / 9472 warp slots) * (nnz/B) * 0.5 us * (1 + 0.6*min(1, N/1e6))
+ *         (a cell row costs ~0.5 us per query term: one segment-table probe per (query, term, doc tile));
+ *   doc : 0.13 ms + ceil(B/QT) * stream_bytes / 4.0 TB/s + nnz * 0.1 us * (1 + 2.7*N/1e6)
+ *         (one pass over the forward index per tile of QT = 8 (B <= 8) or 16 queries, plus the hit walk).
+ * Host arithmetic only (no device call, no handle): num_docs, tile_docs and stream_bytes (forward index + head strips,
+ * gs_info_t.bytes_forward + the head share of bytes_head) describe the index; B and nnz the query batch.  Returns
+ * GS_ALGO_TERM_PARALLEL or GS_ALGO_DOC_PARALLEL; the two estimates (milliseconds) go to out_term_ms / out_doc_ms when
+ * non-null.  Document-parallel wins for one or two long queries (B = 1, >= ~200 terms); term-parallel everywhere else. */
+GS_API int32_t gs_dispatch_model(int64_t num_docs, int32_t tile_docs, int64_t stream_bytes, int64_t B, int64_t nnz,
+                                 double* out_term_ms, double* out_doc_ms);
 
 /* ------------------------------------------------------------------------------------------------
  * Search (§4-§5).

@@ -26,7 +26,7 @@ EXPORTS = [
     "gs_index_copy_head_terms",
     "gs_search_workspace_bytes", "gs_search", "gs_search_finish", "gs_search_host", "gs_search_stats", "gs_score_dense",
     "gs_topk_workspace_bytes", "gs_topk_dense", "gs_merge_topk_workspace_bytes", "gs_merge_topk", "gs_strerror", "gs_version", "gs_abi_version",
-    "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name",
+    "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name", "gs_dispatch_model",
 ]
 GS_PROF_CLASSES = 8
 
@@ -44,7 +44,7 @@ class gs_csr_t(ctypes.Structure):
 
 class gs_build_opts_t(ctypes.Structure):
     _fields_ = [("tile_docs", ctypes.c_int32), ("head_max", ctypes.c_int32), ("head_density", ctypes.c_float),
-                ("validate", ctypes.c_int32)]
+                ("validate", ctypes.c_int32), ("pack_postings", ctypes.c_int32)]
 
 
 class gs_info_t(ctypes.Structure):
@@ -53,7 +53,7 @@ class gs_info_t(ctypes.Structure):
                 ("tile_docs", ctypes.c_int32), ("num_tiles", ctypes.c_int32), ("head_terms", ctypes.c_int32),
                 ("bytes_inverted", ctypes.c_int64), ("bytes_inverted_meta", ctypes.c_int64),
                 ("bytes_forward", ctypes.c_int64), ("bytes_head", ctypes.c_int64), ("bytes_total", ctypes.c_int64),
-                ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("forward_tail_nnz", ctypes.c_int64), ("head_terms_term_parallel", ctypes.c_int32), ("packed_layout", ctypes.c_int32),
                 ("forward_padded_nnz", ctypes.c_int64)]
 
 
@@ -130,6 +130,18 @@ def _check(code: int):
         raise GsError(code, msg)
 
 
+def dispatch_model(num_docs: int, tile_docs: int, stream_bytes: int, num_queries: int, query_nnz: int):
+    """Cost model behind algo="auto" (gpusparse.h: gs_dispatch_model; host arithmetic, no GPU needed).
+    Returns (algo name, estimated term-parallel ms, estimated document-parallel ms)."""
+    t, d = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    L = lib()
+    L.gs_dispatch_model.restype = ctypes.c_int32
+    L.gs_dispatch_model.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64,
+                                    ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    a = L.gs_dispatch_model(num_docs, tile_docs, stream_bytes, num_queries, query_nnz, ctypes.byref(t), ctypes.byref(d))
+    return ("doc" if a == GS_ALGO_DOC_PARALLEL else "term"), t.value, d.value
+
+
 def version() -> str:
     return lib().gs_version().decode()
 
@@ -194,12 +206,13 @@ class Index:
     """gs_index_build / gs_index_free: a GPU-resident inverted + forward index (§3)."""
 
     def __init__(self, indptr, terms, weights, vocab_size: int, *, tile_docs: int = 0, head_max: int = 0,
-                 head_density: float = 0.0, validate: bool = True, stream=None, allocator=None):
+                 head_density: float = 0.0, validate: bool = True, pack_postings: bool = True, stream=None, allocator=None):
         """``allocator``: optional pair of ctypes callbacks (alloc(bytes, stream, user) -> ptr, free(ptr, stream, user))
-        passed as gs_alloc_t; everything the handle owns then comes from it (default: cudaMalloc)."""
+        passed as gs_alloc_t; everything the handle owns then comes from it (default: cudaMalloc).
+        ``pack_postings`` (integer-impact mode): one 32-bit word per posting where the sizes allow it (gs_build_opts_t)."""
         L = lib()
         csr = _dev_csr(indptr, terms, weights)
-        bo = gs_build_opts_t(tile_docs, head_max, head_density, 1 if validate else 0)
+        bo = gs_build_opts_t(tile_docs, head_max, head_density, 1 if validate else 0, 0 if pack_postings else -1)
         h = ctypes.c_void_p()
         self._h = None
         self._alloc = None

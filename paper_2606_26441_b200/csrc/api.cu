@@ -156,14 +156,19 @@ struct Plan {
     bool use_head = true;
 };
 
-Plan make_plan(const gs_index* ix, int64_t B, int32_t k, const gs_search_opts_t* o) {
+// Bytes one document-parallel pass streams: the tail block CSR plus the head strips (not the second tier)
+int64_t stream_bytes(const gs_index* ix) {
+    return ix->bytes_forward + (int64_t)ix->H * ix->N_pad * (ix->wtype == GS_W_F32 ? 4 : 1);
+}
+
+// `nnz` = entries of the query batch (known on the host: gs_csr_t.nnz), so the choice needs no device round trip
+Plan make_plan(const gs_index* ix, int64_t B, int64_t nnz, int32_t k, const gs_search_opts_t* o) {
     Plan p;
     p.algo = GS_ALGO_TERM_PARALLEL;
     if (o) {
-        // AUTO: the work model of PAPER.md L176-181 (q*L postings touched per query by the scatter against N*k streamed
-        // by the document-parallel kernel) with the constants measured on B200 puts every BASELINE.json
-        // workload on the term-parallel side: the warp-per-cell-row kernel for <= 16 queries, the CTA kernel beyond
-        p.algo = o->algo == GS_ALGO_AUTO ? GS_ALGO_TERM_PARALLEL : o->algo;
+        // AUTO: the cost model of gs_dispatch_model (crossover of PAPER.md L176-181 with the forms and constants measured
+        // on B200): term-parallel for batches, document-parallel for one or two long queries
+        p.algo = o->algo == GS_ALGO_AUTO ? gs_dispatch_model(ix->N, ix->Ts, stream_bytes(ix), B, nnz, nullptr, nullptr) : o->algo;
         p.flags = o->flags;
         p.group = o->query_group;
         p.qtile = o->doc_query_tile;
@@ -276,7 +281,7 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     uint32_t* out_scores = (uint32_t*)out_scores_v;
     const int64_t B = q->rows;
     gs_tls_launches = 0;
-    Plan p = make_plan(ix, B, k, opts);
+    Plan p = make_plan(ix, B, q->nnz, k, opts);
     Carve c = carve_ws(ix, p, B, q->nnz, k, ws, ws_bytes);
     if (ws_bytes < c.fixed_bytes + (size_t)ix->N_pad * 4) return GS_ERR_OOM;
     c.qb.B = B; c.qb.nnz = q->nnz; c.qb.indptr = q->indptr;
@@ -358,7 +363,7 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
 // consecutive query numbers are re-run together, as many at a time as the dense region holds
 gs_status_t resolve_overflow(const gs_index* ix, const gs_csr_t* q, int32_t k, const gs_search_opts_t* opts, int32_t* out_ids,
                              void* out_scores, void* ws, size_t ws_bytes, std::vector<int32_t>& ov, cudaStream_t s) {
-    Plan p = make_plan(ix, q->rows, k, opts);
+    Plan p = make_plan(ix, q->rows, q->nnz, k, opts);
     Carve c = carve_ws(ix, p, q->rows, q->nnz, k, ws, ws_bytes);
     c.qb.B = q->rows; c.qb.nnz = q->nnz; c.qb.indptr = q->indptr;
     // the ingest result of the search is still in the workspace (second-tier strip lists included)
@@ -381,6 +386,23 @@ const gs_search_opts_t* norm_opts(const gs_search_opts_t* o, gs_search_opts_t* t
 }  // namespace
 
 extern "C" {
+
+int32_t gs_dispatch_model(int64_t num_docs, int32_t tile_docs, int64_t stream_bytes_, int64_t B, int64_t nnz, double* out_term_ms,
+                          double* out_doc_ms) {
+    const double N = (double)std::max<int64_t>(num_docs, 0), Bq = (double)std::max<int64_t>(B, 1), terms = (double)std::max<int64_t>(nnz, 0);
+    const double tiles = std::ceil(N / (double)std::max(tile_docs, 1));
+    // term-parallel: cell rows = B * tiles over 148 SMs x 64 warp slots; a row costs ~0.5 us per query term (one
+    // segment-table probe per (query, term, doc tile) plus the postings it finds), a little more on long lists
+    const double waves = std::max(1.0, Bq * tiles / 9472.0);
+    const double t_term = 0.10 + waves * (terms / Bq) * 0.5e-3 * (1.0 + 0.6 * std::min(1.0, N / 1e6));
+    // document-parallel: one pass over the forward index per tile of QT queries at ~4.0 TB/s, plus the hit walk
+    const double qt = B <= 8 ? 8.0 : 16.0;
+    const double passes = std::ceil(Bq / qt);
+    const double t_doc = 0.13 + passes * ((double)std::max<int64_t>(stream_bytes_, 0) / 4.0e9) + terms * 0.1e-3 * (1.0 + 2.7 * N / 1e6);
+    if (out_term_ms) *out_term_ms = t_term;
+    if (out_doc_ms) *out_doc_ms = t_doc;
+    return t_doc < t_term ? GS_ALGO_DOC_PARALLEL : GS_ALGO_TERM_PARALLEL;
+}
 
 gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_build_opts_t* opts, const gs_alloc_t* alloc,
                            gs_stream_t stream, gs_index_t** out) {
@@ -418,7 +440,7 @@ gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_bu
 void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
-    void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w,
+    void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w, ix->inv_pk,
                     ix->term_meta, ix->seg_tab, ix->seg_l1, ix->seg_l2, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;
@@ -432,7 +454,7 @@ gs_status_t gs_index_info(const gs_index_t* ix, gs_info_t* out) {
     out->bytes_inverted = ix->bytes_inverted; out->bytes_inverted_meta = ix->bytes_meta;
     out->bytes_forward = ix->bytes_forward; out->bytes_head = ix->bytes_head;
     out->head_terms_term_parallel = ix->H + ix->HX; out->forward_tail_nnz = ix->P_tail;
-    out->forward_padded_nnz = ix->P_fwd; out->reserved = 0;
+    out->forward_padded_nnz = ix->P_fwd; out->packed_layout = (ix->inv_packed ? 1 : 0) | (ix->fwd_packed ? 2 : 0);
     out->bytes_total = ix->bytes_inverted + ix->bytes_meta + ix->bytes_forward + ix->bytes_head;
     return GS_OK;
 }
@@ -455,6 +477,15 @@ gs_status_t gs_index_copy_list(const gs_index_t* ix, int32_t term, int64_t capac
     if (n > 0) {
         if (!host_doc_ids || !host_weights) return GS_ERR_INVALID_ARG;
         const size_t wb = ix->wtype == GS_W_F32 ? 4 : 1;
+        if (ix->inv_packed) {                              // compressed postings: unpack (doc | impact << 24) on the host
+            GS_CUDA(cudaMemcpy(host_doc_ids, ix->inv_pk + off[0], sizeof(uint32_t) * (size_t)n, cudaMemcpyDeviceToHost));
+            for (int64_t i = 0; i < n; ++i) {
+                const uint32_t pk = (uint32_t)host_doc_ids[i];
+                host_doc_ids[i] = pk == 0xFFFFFFFFu ? -1 : (int32_t)(pk & 0xFFFFFFu);
+                ((uint8_t*)host_weights)[i] = pk == 0xFFFFFFFFu ? 0 : (uint8_t)(pk >> 24);
+            }
+            return GS_OK;
+        }
         GS_CUDA(cudaMemcpy(host_doc_ids, ix->inv_doc + off[0], sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost));
         GS_CUDA(cudaMemcpy(host_weights, (const unsigned char*)ix->inv_w + (size_t)off[0] * wb, wb * (size_t)n,
                            cudaMemcpyDeviceToHost));
@@ -473,13 +504,25 @@ gs_status_t gs_search_workspace_bytes(const gs_index_t* ix, int64_t B, int64_t n
                                       size_t* out_bytes) {
     if (!ix || !out_bytes || B < 0 || nnz < 0) return GS_ERR_INVALID_ARG;
     if (k < 1 || k > GS_MAX_K) return GS_ERR_OUT_OF_RANGE;
-    Plan p = make_plan(ix, B, k, opts);
-    Carve c = carve_ws(ix, p, B, nnz, k, nullptr, 0);
-    const size_t row = (size_t)ix->N_pad * 4;
-    size_t dense = row;                                                    // minimum: one dense row (fallback)
-    if (p.dense_only) dense = std::max(dense, std::min<size_t>((size_t)B * row, (size_t)4 << 30) / row * row);
-    else dense = std::max(dense, (size_t)B * (size_t)p.sample_tiles * ix->Ts * 4);
-    *out_bytes = c.fixed_bytes + up256(std::max(dense, row));
+    // With GS_ALGO_AUTO the choice depends on the batch that is searched (its rows and nnz may be smaller than the ones the
+    // workspace was sized for): size for whichever path needs more.
+    size_t need = 0;
+    gs_search_opts_t o2;
+    if (opts) o2 = *opts; else std::memset(&o2, 0, sizeof(o2));
+    const bool is_auto = o2.algo == GS_ALGO_AUTO;
+    for (int a = GS_ALGO_TERM_PARALLEL; a <= GS_ALGO_DOC_PARALLEL; ++a) {
+        if (!is_auto && a != o2.algo) continue;
+        gs_search_opts_t oa = o2;
+        oa.algo = a;
+        Plan p = make_plan(ix, B, nnz, k, &oa);
+        Carve c = carve_ws(ix, p, B, nnz, k, nullptr, 0);
+        const size_t row = (size_t)ix->N_pad * 4;
+        size_t dense = row;                                                    // minimum: one dense row (fallback)
+        if (p.dense_only) dense = std::max(dense, std::min<size_t>((size_t)B * row, (size_t)4 << 30) / row * row);
+        else dense = std::max(dense, (size_t)B * (size_t)p.sample_tiles * ix->Ts * 4);
+        need = std::max(need, c.fixed_bytes + up256(std::max(dense, row)));
+    }
+    *out_bytes = need;
     return GS_OK;
 }
 
@@ -515,7 +558,7 @@ gs_status_t gs_search_finish(const gs_index_t* ix, const gs_csr_t* q, int32_t k,
     if (n_ov > q->rows) return GS_ERR_INVALID_ARG;             // not the workspace of a search of this batch
     gs_search_opts_t tmp;
     const gs_search_opts_t* o = norm_opts(opts, &tmp);
-    Plan p = make_plan(ix, q->rows, k, o);
+    Plan p = make_plan(ix, q->rows, q->nnz, k, o);
     Carve c = carve_ws(ix, p, q->rows, q->nnz, k, ws, ws_bytes);
     std::vector<int32_t> ov((size_t)n_ov);
     GS_CUDA(cudaMemcpyAsync(ov.data(), c.overflow_list, sizeof(int32_t) * (size_t)n_ov, cudaMemcpyDeviceToHost, s));
@@ -602,7 +645,7 @@ gs_status_t gs_score_dense(const gs_index_t* ix, const gs_csr_t* q, const gs_sea
     if (ld < ix->N_pad || !is_device_ptr(out_scores) || !is_device_ptr(ws)) return GS_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     gs_tls_launches = 0;
-    Plan p = make_plan(ix, q->rows, 1, opts);
+    Plan p = make_plan(ix, q->rows, q->nnz, 1, opts);
     p.dense_only = true;
     Carve c = carve_ws(ix, p, q->rows, q->nnz, 1, ws, ws_bytes);
     if (ws_bytes < c.fixed_bytes) return GS_ERR_OOM;

@@ -86,6 +86,11 @@ struct gs_index {
     int32_t* inv_len = nullptr;      // [V]   true list length
     int32_t* inv_doc = nullptr;      // [P_pad] doc ids, ascending within a list, -1 in the padding
     void* inv_w = nullptr;           // [P_pad] float | uint8, 0 in the padding
+    // compressed postings, integer-impact mode (gs_build_opts_t.pack_postings): when inv_packed, the two arrays above are
+    // replaced by ONE word per posting, doc id | impact << 24 (N < 2^24; padding 0xFFFFFFFF); when fwd_packed, fwd_w is
+    // gone and a forward term word is term | impact << 19 | (doc & 31) << 27 (V < 2^19)
+    uint32_t* inv_pk = nullptr;      // [P_pad]
+    bool inv_packed = false, fwd_packed = false;
     // tile-segment tables (see gs_term_meta)
     gs_term_meta* term_meta = nullptr;   // [V]
     uint32_t* seg_tab = nullptr;         // full-mode terms: [n_full][ntiles + 1]

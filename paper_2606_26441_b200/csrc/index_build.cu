@@ -262,6 +262,19 @@ __global__ void k_tail_fill(const int64_t* __restrict__ indptr, const int32_t* _
     }
 }
 
+// integer-impact mode, compressed postings: (doc id, impact) -> doc | impact << 24; the padding (doc -1) -> 0xFFFFFFFF
+__global__ void k_pack_inv(const int32_t* __restrict__ doc, const uint8_t* __restrict__ w, int64_t n, uint32_t* __restrict__ pk) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t d = doc[i];
+        pk[i] = d < 0 ? 0xFFFFFFFFu : ((uint32_t)d | ((uint32_t)w[i] << 24));
+    }
+}
+// forward term word (term | doc-in-block << 27) takes the impact into bits 19..26 (V < 2^19)
+__global__ void k_pack_fwd(uint32_t* __restrict__ terms, const uint8_t* __restrict__ w, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        terms[i] |= (uint32_t)w[i] << 19;
+}
+
 inline unsigned grid_for(int64_t n, int threads = kThreads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
@@ -422,6 +435,20 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
                                                                 (W*)ix->fwd_w);
         }
         ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(nblk + 1) + (sizeof(uint32_t) + sizeof(W)) * (size_t)p_fwd);
+        if (WT == GS_W_U8 && o.pack_postings >= 0 && V < (1 << 19)) {
+            if (p_fwd > 0) {
+                int dev = 0, sms = 0;
+                cudaGetDevice(&dev);
+                cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+                k_pack_fwd<<<sms * 8, 512, 0, s>>>(ix->fwd_terms, (const uint8_t*)ix->fwd_w, p_fwd);
+                GS_CUDA(cudaStreamSynchronize(s));
+                GS_CUDA(cudaGetLastError());
+            }
+            gs_dev_free(ix, ix->fwd_w, s);
+            ix->fwd_w = nullptr;
+            ix->fwd_packed = true;
+            ix->bytes_forward = (int64_t)(sizeof(int64_t) * (size_t)(nblk + 1) + sizeof(uint32_t) * (size_t)p_fwd);
+        }
     }
 
     // ---- padded inverted arrays, pre-filled with the sentinel (doc_id=-1, score=0), L90
@@ -546,6 +573,25 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     }
     GS_CUDA(cudaStreamSynchronize(s));
     GS_CUDA(cudaGetLastError());
+    // ---- compressed postings (integer-impact mode): one word per posting replaces the two arrays
+    if (WT == GS_W_U8 && o.pack_postings >= 0 && N < (1 << 24)) {
+        ix->inv_pk = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)std::max<int64_t>(ix->P_pad, 1), s);
+        if (!ix->inv_pk) return GS_ERR_OOM;
+        if (ix->P_pad > 0) {
+            int dev = 0, sms = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            k_pack_inv<<<sms * 8, 512, 0, s>>>(ix->inv_doc, (const uint8_t*)ix->inv_w, ix->P_pad, ix->inv_pk);
+            GS_CUDA(cudaStreamSynchronize(s));
+            GS_CUDA(cudaGetLastError());
+        }
+        gs_dev_free(ix, ix->inv_doc, s);
+        gs_dev_free(ix, ix->inv_w, s);
+        ix->inv_doc = nullptr;
+        ix->inv_w = nullptr;
+        ix->inv_packed = true;
+        ix->bytes_inverted = (int64_t)(sizeof(uint32_t) * (size_t)ix->P_pad);
+    }
     return GS_OK;
 }
 }  // namespace

@@ -263,6 +263,7 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
 
 struct DocParams {
     const int64_t* fwd_blk; const uint32_t* fwd_terms; const void* fwd_w;
+    int32_t fwd_packed;                         // integer-impact mode: the term word carries the impact in bits 19..26, no fwd_w
     const void* strips; int64_t N_pad;
     int64_t N; int32_t V; int32_t Ts; int32_t Wd;
     const uint32_t* tile_bm;                    // this pass's bitmap[Wd] | prefix[Wd]
@@ -455,6 +456,9 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         t4 = ld_stream4(tp4 + chunk * 32 + lane);
         if (WT == GS_W_F32) {
             w4 = ld_stream4(wp4 + chunk * 32 + lane);
+        } else if (p.fwd_packed) {                 // compressed postings: term | impact << 19 | (doc & 31) << 27
+            w4 = make_uint4((t4.x >> 19) & 0xFFu, (t4.y >> 19) & 0xFFu, (t4.z >> 19) & 0xFFu, (t4.w >> 19) & 0xFFu);
+            t4 = make_uint4(t4.x & 0xF807FFFFu, t4.y & 0xF807FFFFu, t4.z & 0xF807FFFFu, t4.w & 0xF807FFFFu);
         } else {
             const uint32_t v = ld_stream1(wp1 + chunk * 32 + lane);
             w4 = make_uint4(v & 0xFFu, (v >> 8) & 0xFFu, (v >> 16) & 0xFFu, v >> 24);
@@ -673,7 +677,7 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
     }
     const SharedScratch ss = shared_scratch((unsigned char*)scratch, Wd, passes_cap, q->nnz);
     DocParams p{};
-    p.fwd_blk = ix->fwd_blk; p.fwd_terms = ix->fwd_terms; p.fwd_w = ix->fwd_w;
+    p.fwd_blk = ix->fwd_blk; p.fwd_terms = ix->fwd_terms; p.fwd_w = ix->fwd_w; p.fwd_packed = ix->fwd_packed ? 1 : 0;
     p.strips = ix->head_strip; p.N_pad = ix->N_pad;
     p.N = ix->N; p.V = ix->V; p.Ts = ix->Ts; p.Wd = Wd;
     p.rows = ss.rows; p.pairs = ss.pairs;

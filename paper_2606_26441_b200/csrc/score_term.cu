@@ -54,6 +54,7 @@ template <> struct Num<GS_W_U8> {
 struct TermParams {
     // index
     const int32_t* inv_doc; const void* inv_w;
+    const uint32_t* inv_pk;                      // integer-impact mode, compressed postings: doc | impact << 24 (else null)
     const uint32_t* seg_tab; const uint2* seg_l1; const uint32_t* seg_l2;     // tile-segment tables (gs_term_meta), absolute slots
     const void* head_strip; int32_t H; int64_t N; int64_t N_pad; int32_t Ts; int32_t ntiles;
     // queries
@@ -91,16 +92,32 @@ __device__ __forceinline__ uint2 head_entry(const uint2* hl, int i, int n_hot) {
     return __ldg(hl + (i < n_hot ? i : GS_HEAD_MAX - 1 - (i - n_hot)));
 }
 
-// one posting-list segment [dp, dp+n) applied to one accumulator row
+// Posting at slot idx of the inverted index: (doc id, weight widened to the accumulator type).  Integer-impact mode with
+// compressed postings reads ONE word (doc | impact << 24), otherwise the two arrays of PAPER.md L79-84.
 template <int WT>
-__device__ __forceinline__ void scatter_segment(const int32_t* __restrict__ dp, const typename Num<WT>::W* __restrict__ wp,
-                                                int n, typename Num<WT>::A q, typename Num<WT>::A* row, int32_t base,
-                                                int32_t Ts, int lane) {
+__device__ __forceinline__ void load_posting(const TermParams& p, uint32_t idx, int32_t& doc, typename Num<WT>::A& w) {
+    using W = typename Num<WT>::W;
+    if (WT == GS_W_U8 && p.inv_pk != nullptr) {
+        const uint32_t pk = __ldg(p.inv_pk + idx);
+        doc = (int32_t)(pk & 0xFFFFFFu);
+        w = Num<WT>::from_bits((int)(pk >> 24));
+    } else {
+        doc = __ldg(p.inv_doc + idx);
+        w = Num<WT>::widen(__ldg(reinterpret_cast<const W*>(p.inv_w) + idx));
+    }
+}
+
+// one posting-list segment (slots [start, start+n)) applied to one accumulator row
+template <int WT>
+__device__ __forceinline__ void scatter_segment(const TermParams& p, uint32_t start, int n, typename Num<WT>::A q,
+                                                typename Num<WT>::A* row, int32_t base, int32_t Ts, int lane) {
     using A = typename Num<WT>::A;
     if (n <= 32) {
         if (lane < n) {
-            const int32_t rel = dp[lane] - base;
-            const A w = Num<WT>::widen(wp[lane]);
+            int32_t doc;
+            A w;
+            load_posting<WT>(p, start + lane, doc, w);
+            const int32_t rel = doc - base;
             if ((uint32_t)rel < (uint32_t)Ts) row[rel] = Num<WT>::mac(row[rel], q, w);
         }
         return;
@@ -111,9 +128,9 @@ __device__ __forceinline__ void scatter_segment(const int32_t* __restrict__ dp, 
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int i = c + 32 * u;
-            const bool ok = i < n;
-            rel[u] = ok ? dp[i] - base : -1;
-            w[u] = ok ? Num<WT>::widen(wp[i]) : A(0);
+            rel[u] = -1;
+            w[u] = A(0);
+            if (i < n) { load_posting<WT>(p, start + i, rel[u], w[u]); rel[u] -= base; }
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u)
@@ -158,7 +175,6 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
     // scatter the tail lists of the query: segment of each list inside this tile, 32 terms probed at once.  The
     // non-empty segments are applied one after the other (two lists may hit the same document), but the first 32
     // postings of kSegBatch segments are LOADED together, so their latencies overlap.
-    const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
     const int64_t qa = p.q_indptr[b];
     const int cnt = p.tail_cnt[b];
     for (int i0 = 0; i0 < cnt; i0 += 32) {
@@ -187,9 +203,9 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                     n_j[u] = __shfl_sync(0xFFFFFFFFu, n, src);
                     start_j[u] = __shfl_sync(0xFFFFFFFFu, start, src);
                     q_j[u] = Num<WT>::qw(__shfl_sync(0xFFFFFFFFu, wq, src));
-                    const bool ok = lane < n_j[u];
-                    rel_j[u] = ok ? p.inv_doc[start_j[u] + lane] - base : -1;
-                    w_j[u] = ok ? Num<WT>::widen(inv_w[start_j[u] + lane]) : A(0);
+                    rel_j[u] = -1;
+                    w_j[u] = A(0);
+                    if (lane < n_j[u]) { load_posting<WT>(p, start_j[u] + lane, rel_j[u], w_j[u]); rel_j[u] -= base; }
                 }
             }
 #pragma unroll
@@ -197,7 +213,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
                 if (n_j[u] > 0) {                           // uniform
                     if ((uint32_t)rel_j[u] < (uint32_t)Ts) row[rel_j[u]] = Num<WT>::mac(row[rel_j[u]], q_j[u], w_j[u]);
                     if (n_j[u] > 32)
-                        scatter_segment<WT>(p.inv_doc + start_j[u] + 32, inv_w + start_j[u] + 32, n_j[u] - 32, q_j[u], row, base, Ts, lane);
+                        scatter_segment<WT>(p, start_j[u] + 32, n_j[u] - 32, q_j[u], row, base, Ts, lane);
                     __syncwarp();                           // two lists may hit the same document
                 }
             }
@@ -523,8 +539,6 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
                                              uint32_t start, uint32_t wq, int32_t base, int lane) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
-    const W* __restrict__ inv_w = reinterpret_cast<const W*>(p.inv_w);
-    const int32_t* __restrict__ inv_doc = p.inv_doc;
     int incl = n;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -544,7 +558,7 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
     int c0 = -1;                                   // (segments that start before the current round) - 1
     for (int f0 = 0; f0 < T; f0 += 32 * kRounds) {
         int32_t doc[kRounds];
-        W wraw[kRounds];
+        A wv[kRounds];
         uint32_t qv[kRounds];
         unsigned sm[kRounds];
         int ord[kRounds];
@@ -564,8 +578,7 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
                 c0 += __popc(sm[r]);
                 const uint2 de = lds_u2(desc_s + 8u * (uint32_t)sg);
                 const uint32_t idx = de.x + (uint32_t)f;
-                doc[r] = __ldg(inv_doc + idx);
-                wraw[r] = __ldg(inv_w + idx);
+                load_posting<WT>(p, idx, doc[r], wv[r]);
                 qv[r] = de.y;
             }
         }
@@ -573,7 +586,7 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
         for (int r = 0; r < kRounds; ++r) {
             if (f0 + 32 * r < T) {                  // uniform
                 A* cell = row + (doc[r] - base);
-                const A q = Num<WT>::qw(qv[r]), w = Num<WT>::widen(wraw[r]);
+                const A q = Num<WT>::qw(qv[r]), w = wv[r];
                 const int o_hi = __popc(sm[r]);
                 // segment by segment: two lists may hit the same document, one list never does
                 for (int o = (int)(sm[r] & 1u); o <= o_hi; ++o) {
@@ -1039,7 +1052,7 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
                                  bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     TermParams p{};
-    p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.seg_tab = ix->seg_tab; p.seg_l1 = ix->seg_l1; p.seg_l2 = ix->seg_l2;
+    p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.inv_pk = ix->inv_packed ? ix->inv_pk : nullptr; p.seg_tab = ix->seg_tab; p.seg_l1 = ix->seg_l1; p.seg_l2 = ix->seg_l2;
     p.head_strip = ix->head_strip; p.H = use_head ? ix->H : 0; p.N = ix->N; p.N_pad = ix->N_pad; p.Ts = ix->Ts;
     p.ntiles = ix->ntiles;
     p.q_indptr = qb.indptr; p.head_pair = qb.head_pair; p.head_cnt = qb.head_cnt; p.tail_desc = qb.tail_desc;

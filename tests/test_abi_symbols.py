@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(libpath):
     binding.lib()
     assert "sm_100a" in binding.version()
     L.gs_abi_version.restype = ctypes.c_int32
-    assert L.gs_abi_version() == 4
+    assert L.gs_abi_version() == 5
 
 
 def test_host_checked_arguments_without_gpu(libpath):

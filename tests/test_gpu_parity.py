@@ -680,3 +680,56 @@ def test_malformed_query_indptr_is_rejected_not_dereferenced(gs, tiny):
     ids, sc = gpu_search(gs, ix, q, 5)                           # the handle is still healthy
     compare(gs, tiny.docs, q, tiny.vocab, 5, ids, sc)
     ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# Compressed postings (PAPER.md L430 future work 2; gs_build_opts_t.pack_postings): integer-impact mode packs a posting into
+# one 32-bit word in the inverted lists and in the forward index.  Both layouts must give the oracle's results bit for bit,
+# the packed one must be the smaller one, and its lists must still read back as Eq. 2 states them.
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pack", [True, False])
+def test_compressed_postings_layout_and_eq2_readback(gs, pack):
+    g = json.load(open(os.path.join(GOLD, "handworked_3doc.json")))
+    docs = csr_from_dicts(g["u8"]["docs"], np.uint8)
+    ix = gs.Index.from_numpy(docs, g["vocab"], pack_postings=pack)
+    inf = ix.info()
+    assert inf["packed_layout"] == (3 if pack else 0)
+    assert inf["bytes_inverted"] == inf["padded_nnz"] * (4 if pack else 5)
+    want = {}
+    for d, row in enumerate(g["u8"]["docs"]):
+        for t, w in row.items():
+            want.setdefault(int(t), []).append((d, int(w)))
+    for t, lst in want.items():
+        ids, w = ix.posting_list(t)
+        assert len(ids) == 32 and [(int(i), int(x)) for i, x in zip(ids[:len(lst)], w[:len(lst)])] == lst
+        assert np.all(ids[len(lst):] == -1) and np.all(w[len(lst):] == 0)        # sentinel (doc_id=-1, score=0), L90
+    ix.close()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("build_kw", [dict(), dict(tile_docs=96, head_max=-1)])
+def test_compressed_postings_match_the_two_array_layout_and_the_oracle(gs, tiny, algo, build_kw):
+    docs, queries = tiny.docs.to_u8(), tiny.queries.to_u8()
+    sizes = {}
+    for pack in (True, False):
+        _dense_parity(gs, docs, queries, tiny.vocab, algo, pack_postings=pack, **build_kw)
+        ix = gs.Index.from_numpy(docs, tiny.vocab, pack_postings=pack, **build_kw)
+        ids, sc = gpu_search(gs, ix, queries, 33, **aopt(algo))
+        compare(gs, docs, queries, tiny.vocab, 33, ids, sc)
+        inf = ix.info()
+        sizes[pack] = (inf["bytes_inverted"], inf["bytes_forward"])
+        ix.close()
+    assert sizes[True][0] * 5 == sizes[False][0] * 4                  # 4 instead of 5 bytes per inverted posting
+    assert sizes[True][1] < 0.85 * sizes[False][1]                    # forward index: -20 % minus the block pointers
+
+
+def test_compressed_postings_in_the_batch_kernel(gs):
+    """256 queries take the CTA-per-doc-tile batch kernel: its flat posting stream reads packed words."""
+    docs = wl.make_docs("mid", n_docs=20_011).to_u8()
+    queries = wl.make_queries("mid", n_queries=256).to_u8()
+    for pack in (True, False):
+        ix = gs.Index.from_numpy(docs, wl.VOCAB, pack_postings=pack)
+        ids, sc = gpu_search(gs, ix, queries, 10, algo="term")
+        assert ix.stats()["query_group"] >= 32
+        compare(gs, docs, queries, wl.VOCAB, 10, ids, sc)
+        ix.close()
