@@ -9,12 +9,8 @@
 #define GS_STRIP_MAX 64         // dense strips kept by the index
 #define GS_HEAD_MAX GS_STRIP_MAX // entries of a query's compact head list (one per strip at most)
 #define GS_HOT_STRIPS 32        // the densest strips: kept in tensor memory by the fp32 batch kernel
-#ifndef GS_XSTRIP_MAX
-#define GS_XSTRIP_MAX 128
-#endif
-#ifndef GS_XDENS
-#define GS_XDENS 0.05f
-#endif
+#define GS_XSTRIP_MAX 128      // second tier of strips: the next 128 lists ...
+#define GS_XDENS 0.05f         // ... of density >= 0.05 (sweep: 64 lists 16.3 ms, 128 15.4, 192 15.3, 384 15.9 per batch)
 // GS_XSTRIP_MAX: second tier of dense strips, read from global memory by the term-parallel kernels only
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
 #define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings

@@ -427,22 +427,11 @@ __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(cons
 // prefetch of the next row's posting segments — 16.9 ms.
 // ------------------------------------------------------------------------------------------------
 constexpr int kBT = 512;          // documents per tile
-#ifndef GS_BWARPS
-#define GS_BWARPS 32
-#endif
-#ifndef GS_ROUNDS
-#define GS_ROUNDS 1
-#endif
-#ifndef GS_HEAD_UNROLL
-#define GS_HEAD_UNROLL 4
-#endif
-constexpr int kBWarps = GS_BWARPS;   // warps (cell rows in flight) per CTA
-constexpr int kRounds = GS_ROUNDS;   // flat posting rounds whose loads are issued together
-constexpr int kHeadUnroll = GS_HEAD_UNROLL;
-#ifndef GS_X_UNROLL
-#define GS_X_UNROLL 1
-#endif
-constexpr int kXUnroll = GS_X_UNROLL;     // second-tier strip terms whose loads are issued together
+// Values kept after the sweeps of rounds 1 and 2 (profiles/r01d_kernels.md, profiles/r02_kernels.md): 24 warps x 80 registers
+// 23.5-25.9 ms, two posting rounds in flight 17.6 vs 16.7 ms (spills), head loop unrolled by 4 16.7 -> 16.3 ms.
+constexpr int kBWarps = 32;       // warps (cell rows in flight) per CTA
+constexpr int kRounds = 1;        // flat posting rounds whose loads are issued together
+constexpr int kHeadUnroll = 4;    // strips of the integer head loop whose loads are issued together
 
 __device__ __forceinline__ unsigned long long pack_f32x2(float lo, float hi) {
     unsigned long long d;
@@ -601,10 +590,7 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
 
 
 constexpr int kWarpBuf = 80;                  // candidate keys a warp collects in shared memory before it appends them
-#ifndef GS_FLUSH_AT
-#define GS_FLUSH_AT 40
-#endif
-constexpr int kFlushAt = GS_FLUSH_AT;                  // ... which it does at the end of a row once it holds more than this many
+constexpr int kFlushAt = 40;                  // ... which it does at the end of a row once it holds more than this many
 constexpr int kCandBuf = kBWarps * kWarpBuf;
 
 // ---- cold paths of the batch kernel, kept out of line: the kernel's warps sit in different phases of the row loop, so
@@ -1020,17 +1006,11 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged,
 // batch kernel): 8.8M docs 48: 3.03 / 3.19, 64: 3.89 / 3.37, 128: 7.25 / 5.51, 256: 13.7 / 9.49, 500: 25.9 / 16.6;
 // 1M docs 64: 0.61 / 0.62, 96: 0.84 / 0.88, 128: 1.04 / 0.98, 256: 1.87 / 1.53, 500: 3.41 / 2.59 — the fixed cost of a CTA
 // (staging, first-row probes) is amortised over fewer rows when the collection has few doc tiles.
-#ifndef GS_STAGED_MIN
-#define GS_STAGED_MIN 128
-#endif
-constexpr int kStagedMinQueries = GS_STAGED_MIN;
-constexpr int kStagedMinQueriesLarge = GS_STAGED_MIN < 64 ? GS_STAGED_MIN : 64;     // collections of >= kLargeTiles doc tiles
+constexpr int kStagedMinQueries = 128;
+constexpr int kStagedMinQueriesLarge = 64;     // collections of >= kLargeTiles doc tiles
 constexpr int kLargeTiles = 8192;
 constexpr int kStagedChunk = 512;         // most queries per CTA of the staged / batch kernels
-#ifndef GS_CHUNK_WAVES
-#define GS_CHUNK_WAVES 16
-#endif
-constexpr int kChunkWaves = GS_CHUNK_WAVES;   // CTAs per SM a launch aims for before it stops splitting the queries
+constexpr int kChunkWaves = 16;   // CTAs per SM a launch aims for before it stops splitting the queries
 static inline bool cta_per_tile(const gs_index* ix, int64_t nq) {
     return nq >= (ix->ntiles >= kLargeTiles ? kStagedMinQueriesLarge : kStagedMinQueries);
 }

@@ -13,9 +13,7 @@
 
 #include "gs_internal.cuh"
 
-#ifndef GS_SEL_TARGET
 #define GS_SEL_TARGET 128     // CTAs a select launch aims for before it stops splitting rows over clusters
-#endif
 
 namespace {
 
