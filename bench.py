@@ -523,6 +523,15 @@ def suite_entry(torch, gs, wl, name, args, peaks, docs, ix):
             r["latency"] = {kk: lat[kk] for kk in ("calls", "p50_ms", "p99_ms", "p50_ms_per_query", "graph_p50_ms", "graph_p99_ms") if kk in lat}
         res["algos"][algo] = r
         del ws
+    if c["wtype"] == "u8" and B >= 64:
+        # the same term-parallel search with the head contraction on the tensor cores (tcgen05.mma kind::i8, opt-in flag):
+        # bit-identical results (tests/test_gpu_parity.py::test_tensor_core_head_contraction_is_bit_exact)
+        ws = torch.empty(ix.workspace_bytes(B, batch.nnz, k, algo="term", flags=gs.GS_FLAG_TENSOR_CORE_HEAD), dtype=torch.uint8, device=dev)
+        ms = timed_steps(torch, None, lambda: ix.search(*q_dev, k, out_ids=out_ids, out_scores=out_sc, workspace=ws, algo="term",
+                                                        flags=gs.GS_FLAG_TENSOR_CORE_HEAD, finish=False), steps, max(args.warmup, 3), 1)
+        res["algos"]["term_tensor_core_head"] = {"ms_per_step": ms / steps, "qps": B * steps / (ms * 1e-3),
+                                                 "kernel": "k_score_term_mma (tcgen05.mma kind::i8, uint8 x uint8 -> int32, exact)"}
+        del ws
     return res
 
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgpusparse.so")
 
 GS_W_F32, GS_W_U8 = 0, 1
 GS_ALGO_AUTO, GS_ALGO_TERM_PARALLEL, GS_ALGO_DOC_PARALLEL = 0, 1, 2
-GS_FLAG_VALIDATE_QUERIES, GS_FLAG_FORCE_DENSE_TOPK, GS_FLAG_NO_HEAD_STRIPS = 1, 2, 4
+GS_FLAG_VALIDATE_QUERIES, GS_FLAG_FORCE_DENSE_TOPK, GS_FLAG_NO_HEAD_STRIPS, GS_FLAG_TENSOR_CORE_HEAD = 1, 2, 4, 8
 GS_MAX_K = 4096
 ALGOS = {"auto": GS_ALGO_AUTO, "term": GS_ALGO_TERM_PARALLEL, "doc": GS_ALGO_DOC_PARALLEL}
 

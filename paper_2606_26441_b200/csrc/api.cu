@@ -251,7 +251,7 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
 gs_status_t run_score(const gs_index* ix, const Plan& p, const gs_csr_t* q, const gs_qbatch& qb, int64_t q0, int64_t nq,
                       const gs_tileset& ts, const gs_sink& sink, void* doc_scratch, cudaStream_t s) {
     if (p.algo == GS_ALGO_DOC_PARALLEL) return gs_launch_score_doc(ix, q, qb, q0, nq, p.qtile, ts, sink, doc_scratch, s);
-    return gs_launch_score_term(ix, qb, q0, nq, p.group, p.use_head, ts, sink, s);
+    return gs_launch_score_term(ix, qb, q0, nq, p.group, p.use_head, (p.flags & GS_FLAG_TENSOR_CORE_HEAD) != 0, ts, sink, s);
 }
 
 // dense path for queries [q0, q0+nq): score every tile into the dense region, select, write results
@@ -440,7 +440,7 @@ gs_status_t gs_index_build(const gs_csr_t* docs, int32_t vocab_size, const gs_bu
 void gs_index_free(gs_index_t* ix) {
     if (!ix) return;
     cudaDeviceSynchronize();
-    void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w, ix->inv_pk,
+    void* ptrs[] = {ix->fwd_blk, ix->fwd_terms, ix->fwd_w, ix->inv_off, ix->inv_len, ix->inv_doc, ix->inv_w, ix->inv_pk, ix->mma_strips,
                     ix->term_meta, ix->seg_tab, ix->seg_l1, ix->seg_l2, ix->head_slot, ix->head_strip, ix->xslot, ix->xstrip, ix->host_ws, ix->host_stage};
     for (void* p : ptrs) gs_dev_free(ix, p, 0);
     delete ix;

@@ -12,6 +12,7 @@
 #define GS_XSTRIP_MAX 128      // second tier of strips: the next 128 lists ...
 #define GS_XDENS 0.05f         // ... of density >= 0.05 (sweep: 64 lists 16.3 ms, 128 15.4, 192 15.3, 384 15.9 per batch)
 // GS_XSTRIP_MAX: second tier of dense strips, read from global memory by the term-parallel kernels only
+#define GS_MMA_K 192            // strips (head + second tier) of the tensor-core head contraction = K of the integer MMA
 #define GS_FWD_DOC_SHIFT 27     // forward term word = term id | (doc id & 31) << 27   (V < 2^27)
 #define GS_FWD_CHUNK 128        // a 32-document block of the forward index is padded to a multiple of this many postings
 #define GS_TAIL32 32            // tail terms of a query kept in the fixed-stride prefetch table
@@ -105,6 +106,12 @@ struct gs_index {
     int32_t HX = 0;
     int16_t* xslot = nullptr;        // [V]: x-strip number of a term or -1
     void* xstrip = nullptr;          // [HX][N_pad]
+    // Integer-impact mode, 512-doc tiles: the strips once more, as the A operand of the tensor-core head contraction
+    // (k_score_term_mma).  Per doc tile 4 sub-tiles of 128 documents; a sub-tile is a 128 x GS_MMA_K matrix of
+    // uint8 (row = document, column = strip: head strips in columns 0..63, second-tier strips in 64..191, 0 where there is no
+    // strip) in the K-major no-swizzle core-matrix layout tcgen05.mma reads from shared memory: [K/16][128/8][8 rows][16 B],
+    // so a sub-tile is ONE contiguous block of 24 KB and a doc tile one 1-D TMA bulk copy of 96 KB.
+    uint8_t* mma_strips = nullptr;   // [ntiles][4][GS_MMA_K/16][16][8][16]
     // allocator
     gs_alloc_t alloc{};
     bool has_alloc = false;
@@ -199,7 +206,7 @@ gs_status_t gs_launch_ingest(const gs_index* ix, const gs_csr_t* q, bool validat
 bool gs_score_term_wants_x(const gs_index* ix, int64_t nq, int group, bool use_head);   // the batch kernel will run
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
-                                 bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
+                                 bool use_head, bool use_mma, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s);
 
 int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head);   // cell rows (warps) per CTA actually used
 int gs_score_doc_qtile(int qtile);                                    // queries per pass actually used

@@ -275,6 +275,30 @@ __global__ void k_pack_fwd(uint32_t* __restrict__ terms, const uint8_t* __restri
         terms[i] |= (uint32_t)w[i] << 19;
 }
 
+// A operand of the tensor-core head contraction (gs_index::mma_strips): one thread per 16-byte unit = (doc, 16 strips)
+__global__ void k_build_mma_strips(const uint8_t* __restrict__ head, int H, const uint8_t* __restrict__ xs, int HX, int64_t N_pad,
+                                   int32_t ntiles, uint8_t* __restrict__ out) {
+    constexpr int KC = GS_MMA_K / 16;
+    const int64_t u = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;           // unit = ((tile*4 + s)*KC + kc)*128 + row
+    if (u >= (int64_t)ntiles * 4 * KC * 128) return;
+    const int row = (int)(u & 127);
+    const int kc = (int)((u >> 7) % KC);
+    const int64_t ts = (u >> 7) / KC;                                           // tile*4 + s
+    const int64_t doc = ts * 128 + row;
+    uint32_t w[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int kb = 0; kb < 16; ++kb) {
+        const int k = kc * 16 + kb;
+        uint32_t v = 0u;
+        if (k < GS_STRIP_MAX) { if (k < H) v = head[(size_t)k * N_pad + doc]; }
+        else if (k - GS_STRIP_MAX < HX) v = xs[(size_t)(k - GS_STRIP_MAX) * N_pad + doc];
+        w[kb >> 2] |= v << (8 * (kb & 3));
+    }
+    // core matrix (kc, rg = row/8): 8 rows of 16 bytes
+    uint4* dst = reinterpret_cast<uint4*>(out + (size_t)ts * (KC * 2048) + (size_t)(kc * 16 + (row >> 3)) * 128 + (row & 7) * 16);
+    *dst = make_uint4(w[0], w[1], w[2], w[3]);
+}
+
 inline unsigned grid_for(int64_t n, int threads = kThreads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
@@ -573,6 +597,18 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
     }
     GS_CUDA(cudaStreamSynchronize(s));
     GS_CUDA(cudaGetLastError());
+    // ---- integer-impact mode: the strips as the A operand of the tensor-core head contraction
+    if (WT == GS_W_U8 && ix->Ts == 512 && ix->H > 0 && ix->ntiles > 0) {
+        const size_t bytes = (size_t)ix->ntiles * 4 * (GS_MMA_K / 16) * 2048;
+        ix->mma_strips = (uint8_t*)gs_dev_alloc(ix, bytes, s);
+        if (!ix->mma_strips) return GS_ERR_OOM;
+        const int64_t units = (int64_t)ix->ntiles * 4 * (GS_MMA_K / 16) * 128;
+        k_build_mma_strips<<<grid_for(units), kThreads, 0, s>>>((const uint8_t*)ix->head_strip, ix->H, (const uint8_t*)ix->xstrip, ix->HX,
+                                                              ix->N_pad, ix->ntiles, ix->mma_strips);
+        GS_CUDA(cudaStreamSynchronize(s));
+        GS_CUDA(cudaGetLastError());
+        ix->bytes_head += (int64_t)bytes;
+    }
     // ---- compressed postings (integer-impact mode): one word per posting replaces the two arrays
     if (WT == GS_W_U8 && o.pack_postings >= 0 && N < (1 << 24)) {
         ix->inv_pk = (uint32_t*)gs_dev_alloc(ix, sizeof(uint32_t) * (size_t)std::max<int64_t>(ix->P_pad, 1), s);

@@ -61,6 +61,7 @@ struct TermParams {
     const int64_t* q_indptr; const uint2* head_pair; const int32_t* head_cnt; const uint4* tail_desc;
     const int32_t* tail_cnt; const uint4* tail32;
     const void* xstrip; const uint2* xpair; const int32_t* xcnt;      // second-tier strips (null when the batch has none)
+    const uint8_t* mma_strips;                  // integer mode: the strips as the A operand of k_score_term_mma (else null)
     int64_t q0; int32_t nq;                     // queries [q0, q0+nq)
     int32_t warps;                              // cell rows (warps) per CTA (small-batch kernel)
     int32_t chunk, n_chunks;                    // staged kernel: queries per CTA, CTAs per doc tile
@@ -979,6 +980,275 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Integer-impact mode, batches: the head contraction on the TENSOR CORES.  The strips of a doc tile are a
+// genuinely dense block: scores_head[512 docs x B queries] = S[512 x 192 strips] * Q[192 x B], uint8 x uint8 -> int32, which
+// tcgen05.mma kind::i8 computes exactly (integer addition is associative: bit-identical to the IDP4A path and to the
+// oracle).  The fp32 path does not use this: its products would have to be rounded (PAPER.md keeps fp32, L75/L165).
+//
+// One persistent CTA of 32 warps per SM walks (doc tile, query chunk) items; inside an item, groups of 32 queries:
+//   * A operand: the tile's strips in the K-major core-matrix layout (gs_index::mma_strips), 96 KB, one TMA bulk copy per
+//     128-document sub-tile, once per item; B operand: the group's query impacts as a dense 32 x 192 uint8 matrix, built
+//     in shared memory from the compact strip lists (double buffered); D: 4 sub-tiles x (128 docs x 32 queries) int32 =
+//     128 columns of tensor memory, four groups deep, so the 24 MMAs of group g+1 are issued (by one thread) while the
+//     warps still work on group g;
+//   * tail: warp w owns the row of query w of the group (shared memory, 2 KB) and scatters the query's tail lists into
+//     it with the flat posting stream of the batch kernel (scatter_flat) — no atomics, fixed order;
+//   * epilogue (replaces the head phase: ~60 instead of ~300 instructions per row): warp w reads, for its lane quarter
+//     (documents 32(w%4) .. +31 of every sub-tile) and its 4 queries (4(w/4) .. +3), the head scores from tensor memory
+//     (tcgen05.ld.32x32b.x4: lane = document, columns = queries), adds the tail rows (conflict-free: consecutive lanes are
+//     consecutive documents) and hands the cells to the sink (dense store or threshold filter).
+// Synchronisation is by TEAMS of four warps: the rows of queries 4t .. 4t+3 are written by warps 4t .. 4t+3 and read by the
+// same four warps (one lane quarter each), so two named barriers of 128 threads per group replace CTA barriers and the
+// teams drift apart freely (a CTA barrier made every group as slow as its slowest of 32 rows: 19.2 ms per batch against
+// 13.9 ms on the CUDA cores).  The B operand of a group is complete when all 32 warps have written their row: the last
+// one to arrive (shared-memory counter) issues the group's MMAs.
+// ------------------------------------------------------------------------------------------------
+constexpr int kMQ = 32;                                     // queries per group = N of the MMA = warps of the CTA
+constexpr size_t kMOffDesc = (size_t)kMQ * kBT * 4;         // rows [32][512] int32 | flat-stream descriptors [32][32] uint2
+constexpr size_t kMOffKey = kMOffDesc + (size_t)kMQ * 32 * 8;
+constexpr size_t kMOffQ = kMOffKey + (size_t)kCandBuf * 8;
+constexpr size_t kMOffCnt = kMOffQ + (size_t)kCandBuf * 2;
+constexpr size_t kMOffBar = kMOffCnt + (size_t)(kMQ + 4) * 4;   // mbarrier A | mbarrier MMA [4] | tensor-memory base
+constexpr size_t kMOffB = (kMOffBar + 64 + 127) / 128 * 128;    // B operand [4][GS_MMA_K/16][4][8][16]
+constexpr size_t kMBBytes = (size_t)(GS_MMA_K / 16) * 4 * 128;
+constexpr int kMLook = 3;                                       // groups whose B operand and MMAs run ahead of the rows
+constexpr size_t kMOffA = kMOffB + 4 * kMBBytes;                // A operand [4][GS_MMA_K/16][16][8][16]
+constexpr size_t kMABytes = (size_t)4 * (GS_MMA_K / 16) * 2048;
+constexpr size_t kMSmem = kMOffA + kMABytes;
+static_assert(kMOffBar % 8 == 0 && kMOffA % 128 == 0, "alignment");
+
+// shared-memory matrix descriptor, K-major, no swizzle: start address >> 4 | leading byte offset (between core matrices
+// along K) >> 4 << 16 | stride byte offset (between 8-row groups along M/N) >> 4 << 32 | version 1 << 46
+__device__ __forceinline__ unsigned long long umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+    return (unsigned long long)((saddr & 0x3FFFFu) >> 4) | ((unsigned long long)(lbo >> 4) << 16) |
+           ((unsigned long long)(sbo >> 4) << 32) | (1ull << 46);
+}
+
+// One thread: the 24 MMAs of a group, D[sub-tile s] (128 x 32, int32, tensor memory) = A_s (128 x 192) * B^T (32 x 192),
+// and the commit that makes their completion arrive on an mbarrier.
+__device__ __noinline__ void mma_issue_group(uint32_t a_s, uint32_t b_s, uint32_t d_tmem, uint32_t mbar) {
+    // instruction descriptor: D int32 (2 << 4), A and B unsigned 8 bit (0 << 7, 0 << 10), both K-major, N = 32 (>> 3 << 17),
+    // M = 128 (>> 4 << 24)
+    constexpr uint32_t idesc = (2u << 4) | ((uint32_t)(kMQ >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+#pragma unroll 1
+    for (int s = 0; s < 4; ++s)
+#pragma unroll 1
+        for (int j = 0; j < GS_MMA_K / 32; ++j) {
+            const unsigned long long ad = umma_desc(a_s + (uint32_t)(s * (GS_MMA_K / 16) * 2048 + j * 2 * 2048), 2048u, 128u);
+            const unsigned long long bd = umma_desc(b_s + (uint32_t)(j * 2 * 512), 512u, 128u);
+            const uint32_t acc = j > 0 ? 1u : 0u;
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                         "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+                         ::"r"(d_tmem + (uint32_t)(s * kMQ)), "l"(ad), "l"(bd), "r"(idesc), "r"(acc) : "memory");
+        }
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar) : "memory");
+}
+
+// One thread: the item's A operand, one bulk copy per sub-tile
+__device__ __noinline__ void mma_issue_a(const uint8_t* g, uint32_t a_s, uint32_t mbar) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"((uint32_t)kMABytes) : "memory");
+#pragma unroll 1
+    for (int s = 0; s < 4; ++s)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(a_s + (uint32_t)(s * (kMABytes / 4))), "l"(g + (size_t)s * (kMABytes / 4)), "r"((uint32_t)(kMABytes / 4)), "r"(mbar) : "memory");
+}
+
+__global__ void __launch_bounds__(kMQ * 32, 1) k_score_term_mma(const TermParams p) {
+    constexpr int WT = GS_W_U8;
+    using A = int32_t;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    A* rows = reinterpret_cast<A*>(smem_raw);
+    A* row = rows + (size_t)warp * kBT;
+    const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kMOffDesc) + (uint32_t)warp * 256u;
+    uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kMOffKey) + warp * kWarpBuf;
+    uint16_t* w_q = reinterpret_cast<uint16_t*>(smem_raw + kMOffQ) + warp * kWarpBuf;
+    uint32_t* w_cnt = reinterpret_cast<uint32_t*>(smem_raw + kMOffCnt) + warp;
+    uint32_t* s_bcnt = reinterpret_cast<uint32_t*>(smem_raw + kMOffCnt) + kMQ;       // [4] warps that have written their B row
+    const uint32_t mbar_a = (uint32_t)__cvta_generic_to_shared(smem_raw + kMOffBar);
+    const uint32_t mbar_m = mbar_a + 8u;                                            // [4]
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem_raw + kMOffBar + 40);
+    volatile uint32_t* s_issue = s_tmem + 1;                                         // next group whose MMAs are to be issued
+    uint8_t* s_b = smem_raw + kMOffB;
+    const uint32_t b_s = (uint32_t)__cvta_generic_to_shared(s_b);
+    const uint32_t a_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kMOffA);
+    const bool filter = p.sink.thr != nullptr;
+    const int n_items = p.ts.count * p.n_chunks;
+    auto item_a = [&](int item) {
+        return p.mma_strips + (size_t)(p.ts.first + (item / p.n_chunks) * p.ts.stride) * kMABytes;
+    };
+    if (lane == 0) *w_cnt = 0u;
+    if (threadIdx.x == 0) {
+        s_bcnt[0] = s_bcnt[1] = s_bcnt[2] = s_bcnt[3] = 0u;
+        *s_issue = 0u;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_a) : "memory");
+        for (int i = 0; i < 4; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_m + 8u * i) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {                                    // the whole tensor memory of the SM (one CTA per SM)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(s_tmem)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem0 = s_tmem[0];
+    if (threadIdx.x == 0 && (int)blockIdx.x < n_items) mma_issue_a(item_a((int)blockIdx.x), a_s, mbar_a);
+
+    // B operand of the group whose first query is qs: warp w writes row w (query qs + w): zeros, then the query's impacts at
+    // the columns of its strips (head strip h -> column h, second-tier strip x -> column 64 + x)
+    auto build_b = [&](int qs, int q_end, int buf) {
+        uint8_t* bb = s_b + (size_t)buf * kMBBytes + (size_t)(warp >> 3) * 128 + (size_t)(warp & 7) * 16;    // + (k >> 4) * 512 + (k & 15)
+        if (lane < GS_MMA_K / 16) *reinterpret_cast<uint4*>(bb + lane * 512) = make_uint4(0u, 0u, 0u, 0u);
+        __syncwarp();
+        const int q = qs + warp;
+        if (q < q_end) {
+            const int64_t b = p.q0 + q;
+            const int hc = __ldg(p.head_cnt + b);
+            const int nh = hc & 0xFF, n_hot = hc >> 8;
+            const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;
+            const uint2* hl = p.head_pair + b * GS_HEAD_MAX;
+            if (lane < n_hot) { const uint2 e = __ldg(hl + lane); bb[(e.x >> 4) * 512 + (e.x & 15)] = (uint8_t)e.y; }
+            if (lane < nh - n_hot) { const uint2 e = __ldg(hl + (GS_HEAD_MAX - 1 - lane)); bb[(e.x >> 4) * 512 + (e.x & 15)] = (uint8_t)e.y; }
+            for (int i = lane; i < nx; i += 32) {
+                const uint2 e = __ldg(p.xpair + b * GS_XSTRIP_MAX + i);
+                const uint32_t k = GS_STRIP_MAX + e.x;
+                bb[(k >> 4) * 512 + (k & 15)] = (uint8_t)e.y;
+            }
+        }
+    };
+
+    uint32_t G = 0;                                     // groups done by this CTA: tensor-memory buffer G & 3, phase (G >> 2) & 1
+    int it = 0;
+    for (int item = (int)blockIdx.x; item < n_items; item += (int)gridDim.x, ++it) {
+        const int j = item / p.n_chunks;
+        const int chunk = item - j * p.n_chunks;
+        const int tile = p.ts.first + j * p.ts.stride;
+        const int32_t base = tile * kBT;
+        const int q_beg = chunk * p.chunk;
+        const int q_end = min(p.nq, (chunk + 1) * p.chunk);
+        const int n_groups = (q_end - q_beg + kMQ - 1) / kMQ;
+        const int n_live = (int)min((int64_t)kBT, p.N - (int64_t)base);
+        // B row of the warp's query of group X (first query qs); the last warp to arrive issues the group's MMAs — after
+        // the item's strips have landed when X is the item's first group — and, when X is the item's last group, waits
+        // for them and starts the copy of the next item's strips (nobody reads the old ones any more)
+        auto b_ready = [&](uint32_t X, int qs, bool /*first*/, bool last) {
+            build_b(qs, q_end, (int)(X & 3u));
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence_block();
+                if (atomicAdd(s_bcnt + (X & 3u), 1u) == (uint32_t)(kMQ - 1)) {
+                    s_bcnt[X & 3u] = 0u;
+                    __threadfence_block();
+                    while (*s_issue != X) {}              // groups are issued in order (the strips of the next item follow the last one)
+                    mbar_wait(mbar_a, (uint32_t)(it & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    mma_issue_group(a_s, b_s + (X & 3u) * (uint32_t)kMBBytes, tmem0 + (X & 3u) * 128u, mbar_m + 8u * (X & 3u));
+                    if (last && item + (int)gridDim.x < n_items) {
+                        mbar_wait(mbar_m + 8u * (X & 3u), (X >> 2) & 1u);
+                        mma_issue_a(item_a(item + (int)gridDim.x), a_s, mbar_a);
+                    }
+                    __threadfence_block();
+                    *s_issue = X + 1u;
+                }
+            }
+            __syncwarp();
+        };
+        for (int x = 0; x < min(kMLook, n_groups); ++x) b_ready(G + (uint32_t)x, q_beg + x * kMQ, x == 0, x + 1 == n_groups);
+        // probes of the warp's query of the first group (terms -> segment tables), the next group's are asked for one group ahead
+        Probe2 s2{0u, 0u, 0u, 0u, 0, 0ull};
+        if (q_beg + warp < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q_beg + warp, lane), tile); probe_query(p, p.q0 + q_beg + warp, filter, s2); }
+#pragma unroll 1
+        for (int g = 0; g < n_groups; ++g, ++G) {
+            const int qg = q_beg + g * kMQ;
+            const int q = qg + warp;
+            const Probe2 cur = s2;
+            if (q + kMQ < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q + kMQ, lane), tile); probe_query(p, p.q0 + q + kMQ, filter, s2); }
+            // ---- tail: the row of query q
+#pragma unroll
+            for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
+            __syncwarp();
+            if (q < q_end) {
+                const int cnt = cur.cnt_nh & 0xFFFF;
+                uint32_t lo, hi;
+                resolve_segments(p, cur, tile, lane, lo, hi);
+                scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane);
+                if (cnt > GS_TAIL32) {                  // more than 32 tail terms: probed in line
+                    const int64_t qa = p.q_indptr[p.q0 + q];
+                    for (int i0 = GS_TAIL32; i0 < cnt; i0 += 32) {
+                        __syncwarp();                   // the descriptor table is reused
+                        uint4 d = make_uint4(0u, 0u, 0xFFFFFFFFu, 0u);
+                        if (i0 + lane < cnt) d = __ldg(p.tail_desc + qa + i0 + lane);
+                        probe_range(p, d, tile, lo, hi);
+                        scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, d.x, base, lane);
+                    }
+                }
+            }
+            // ---- B of the next group; then the team's four rows are complete
+            if (g + kMLook < n_groups) b_ready(G + (uint32_t)kMLook, qg + kMLook * kMQ, false, g + kMLook + 1 == n_groups);
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + (warp >> 2)) : "memory");
+            // ---- epilogue of group g: head scores from tensor memory + tail rows -> sink
+            mbar_wait(mbar_m + 8u * (G & 3u), (G >> 2) & 1u);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            {
+                const int k4 = warp & 3, gq = warp >> 2;
+                A thr_s[4];
+                int tie[4];
+                bool okq[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int qq = qg + 4 * gq + u;
+                    okq[u] = qq < q_end;
+                    const uint64_t thr = (filter && okq[u]) ? __ldg(p.sink.thr + p.q0 + qq) : 0ull;
+                    thr_s[u] = thr == 0ull ? Num<WT>::lowest() : (A)((uint32_t)(thr >> 32) ^ 0x80000000u);
+                    const int64_t thr_cell = (int64_t)(0xFFFFFFFFu - (uint32_t)thr) - (int64_t)base;
+                    tie[u] = (int)max((int64_t)-1, min((int64_t)kBT, thr_cell));
+                }
+#pragma unroll 1
+                for (int s = 0; s < 4; ++s) {
+                    uint32_t v[4];
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];\n\ttcgen05.wait::ld.sync.aligned;"
+                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+                                 : "r"(tmem0 + ((uint32_t)(32 * k4) << 16) + (G & 3u) * 128u + (uint32_t)(s * kMQ + 4 * gq)) : "memory");
+                    const int cell = 128 * s + 32 * k4 + lane;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (!okq[u]) continue;
+                        const int qq = qg + 4 * gq + u;
+                        const A sc = (A)v[u] + rows[(size_t)(4 * gq + u) * kBT + cell];
+                        const int64_t b = p.q0 + qq;
+                        if (!filter) {
+                            if ((int64_t)base + cell < p.N) p.sink.dense[(b - p.q0) * p.sink.ld + (int64_t)j * kBT + cell] = (uint32_t)sc;
+                        } else if (sc >= thr_s[u] && cell < n_live && (sc > thr_s[u] || cell <= tie[u])) {
+                            const uint64_t key = gs_make_key(gs_ord_bits<WT>((uint32_t)sc), (uint32_t)(base + cell));
+                            const uint32_t slot = atomicAdd(w_cnt, 1u);
+                            if (slot < (uint32_t)kWarpBuf) {
+                                w_key[slot] = key;
+                                w_q[slot] = (uint16_t)qq;
+                            } else {                                         // buffer full: append directly
+                                const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                                if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
+                            }
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (filter && *reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt)
+                batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + (warp >> 2)) : "memory");      // the team's rows are free
+        }
+    }
+    if (filter) batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem0), "n"(512));
+}
+
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
 template <int WT, bool XS>
@@ -1029,7 +1299,7 @@ int gs_score_term_group(const gs_index* ix, int64_t nq, int group, bool use_head
 }
 
 gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_t q0, int64_t nq, int group,
-                                 bool use_head, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
+                                 bool use_head, bool use_mma, const gs_tileset& ts, const gs_sink& sink, cudaStream_t s) {
     if (nq <= 0 || ts.count <= 0) return GS_OK;
     TermParams p{};
     p.inv_doc = ix->inv_doc; p.inv_w = ix->inv_w; p.inv_pk = ix->inv_packed ? ix->inv_pk : nullptr; p.seg_tab = ix->seg_tab; p.seg_l1 = ix->seg_l1; p.seg_l2 = ix->seg_l2;
@@ -1062,6 +1332,17 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
         const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 32 + 128;
+        if (group == 0 && ix->Ts == kBT && ix->wtype == GS_W_U8 && use_mma && ix->mma_strips != nullptr &&
+            (ix->HX == 0 || qb.x_on) && kMSmem <= (size_t)smem_max && nq <= 65535) {
+            // integer impacts: the head contraction on the tensor cores
+            p.mma_strips = ix->mma_strips;
+            GS_CUDA(gs_optin_smem(k_score_term_mma));
+            GsProfScope ps(GS_K_SCORE_TERM, s);
+            k_score_term_mma<<<(unsigned)std::min<int64_t>(grid, sms), kMQ * 32, kMSmem, s>>>(p);
+            ++gs_tls_launches;
+            GS_CUDA(cudaGetLastError());
+            return GS_OK;
+        }
         if (group == 0 && ix->Ts == kBT && smem_batch <= (size_t)smem_max && nq <= 65535) {
             auto go = [&](auto kern) -> gs_status_t {
                 GS_CUDA(gs_optin_smem(kern));

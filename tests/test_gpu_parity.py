@@ -733,3 +733,23 @@ def test_compressed_postings_in_the_batch_kernel(gs):
         assert ix.stats()["query_group"] >= 32
         compare(gs, docs, queries, wl.VOCAB, 10, ids, sc)
         ix.close()
+
+
+# ----------------------------------------------------------------------------------------------------
+# Integer-impact mode, batches: the head contraction on the tensor cores (tcgen05.mma kind::i8, k_score_term_mma,
+# GS_FLAG_TENSOR_CORE_HEAD) must be bit-identical to the CUDA-core path and to the oracle — every score, then the top-k.
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_docs,n_q", [(20_011, 256), (3_000, 130), (70_001, 500)])
+def test_tensor_core_head_contraction_is_bit_exact(gs, n_docs, n_q):
+    docs = wl.make_docs("mid", n_docs=n_docs).to_u8()
+    queries = wl.make_queries("mid", n_queries=n_q).to_u8()
+    R_d, R_q = oracle.as_rows(docs, wl.VOCAB), oracle.as_rows(queries, wl.VOCAB)
+    o_ids, o_sc, A = oracle.search(R_q, R_d, 100, all_scores=True)
+    ix = gs.Index.from_numpy(docs, wl.VOCAB)
+    for flags in (gs.GS_FLAG_TENSOR_CORE_HEAD, 0):
+        S = ix.score_dense(*dev(queries), algo="term", flags=flags).cpu().numpy()[:, :docs.rows]
+        assert np.array_equal(S.astype(np.int64), A.astype(np.int64)), f"flags={flags}"
+        ids, sc = gpu_search(gs, ix, queries, 100, algo="term", flags=flags)
+        assert ix.stats()["query_group"] >= 32
+        parity.check_int_exact(ids, sc, o_ids, o_sc)
+    ix.close()
