@@ -46,7 +46,7 @@ constexpr int kMaxQT = 64;
 // What a pass needs with warp-uniform access.  Built in the search workspace by k_build_qtile, copied to
 // c_tile before the pass's launch (stream ordered).  qh is last: a pass copies only its [GS_STRIP_MAX][QT] prefix.
 struct ConstTile {
-    uint32_t nh;                         // strips some query of the tile uses, rounded up to a multiple of 4 (zero rows)
+    uint32_t nh;                         // strips some query of the tile uses, rounded up to a multiple of 4 (fp32) / 8 (impacts): zero rows
     uint32_t R;                          // distinct tail terms of the tile (rows)
     uint32_t np;                         // (row, query) pairs
     uint32_t row_off;                    // this pass's slice of the shared row array
@@ -184,9 +184,9 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
         uint32_t n = 0;
         for (int h = 0; h < H; ++h)
             if ((s_hmask[h >> 5] >> (h & 31)) & 1u) ct->hl[n++] = (uint32_t)h;
-        const uint32_t n4 = (n + 3u) & ~3u;
+        const uint32_t n8 = WT == GS_W_F32 ? ((n + 3u) & ~3u) : ((n + 7u) & ~7u);      // strips per turn of strips_phase
         for (uint32_t i = n; i < GS_STRIP_MAX; ++i) ct->hl[i] = 0u;      // padding rows carry zero weights
-        ct->nh = n4;
+        ct->nh = n8;
         ct->R = R;
         ct->row_off = row_off;
         ct->pair_off = pair_off;
@@ -311,21 +311,24 @@ __device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ mya
 #pragma unroll
         for (int q = 0; q < QT / 2; ++q)
             asm("mov.b64 %0, {%1, %2};" : "=l"(acc[q]) : "f"(myacc[2 * q]), "f"(myacc[2 * q + 1]));
-        // the strip values of the next group of 4 are loaded before the multiply-adds of the current one
-        float xn[4];
+        // The strip values of the next kSG strips are loaded before the multiply-adds of the current ones: a strip value is
+        // one DRAM round trip per block of 32 documents, and with 4 in flight that wait is 20 % of the kernel's stall
+        // samples (profiles/r02_kernels.md).  c_tile.hl is padded with valid strip numbers up to a multiple of kSG.
+        constexpr int kSG = 4;
+        float xn[kSG];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) xn[u] = sp[(size_t)c_tile.hl[u] * N_pad];
+        for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[u] * N_pad];
 #pragma unroll 1
-        for (int i0 = 0; i0 < nh; i0 += 4) {
-            float x[4];
+        for (int i0 = 0; i0 < nh; i0 += kSG) {
+            float x[kSG];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) x[u] = xn[u];
-            if (i0 + 4 < nh) {
+            for (int u = 0; u < kSG; ++u) x[u] = xn[u];
+            if (i0 + kSG < nh) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) xn[u] = sp[(size_t)c_tile.hl[i0 + 4 + u] * N_pad];
+                for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[i0 + kSG + u] * N_pad];
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < kSG; ++u) {
 #pragma unroll
                 for (int q = 0; q < QT; q += 4) {
                     const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(&c_tile.qh[(i0 + u) * QT + q]);
@@ -347,14 +350,23 @@ __device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ mya
         for (int q = 0; q < QT; ++q) acc[q] = myacc[q];
         // integer impacts: the document's bytes of four strips packed into one word, the tile's weights of the same four
         // strips packed per query (k_build_qtile): one IDP4A per (four strips, query)
+        // the bytes of the next 8 strips are loaded before the IDP4As of the current ones (see the fp32 branch)
+        uint32_t xn[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[u] * N_pad];
 #pragma unroll 1
-        for (int i0 = 0; i0 < nh; i0 += 4) {
-            uint32_t x4 = 0;
+        for (int i0 = 0; i0 < nh; i0 += 8) {
+            const uint32_t xa = xn[0] | (xn[1] << 8) | (xn[2] << 16) | (xn[3] << 24);
+            const uint32_t xb = xn[4] | (xn[5] << 8) | (xn[6] << 16) | (xn[7] << 24);
+            if (i0 + 8 < nh) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) x4 |= (uint32_t)sp[(size_t)c_tile.hl[i0 + u] * N_pad] << (8 * u);
+                for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[i0 + 8 + u] * N_pad];
+            }
 #pragma unroll
-            for (int q = 0; q < QT; ++q)
-                acc[q] = (A)__dp4a(x4, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
+            for (int q = 0; q < QT; ++q) {
+                acc[q] = (A)__dp4a(xa, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
+                acc[q] = (A)__dp4a(xb, c_tile.qh[((i0 >> 2) + 1) * QT + q], (uint32_t)acc[q]);
+            }
         }
 #pragma unroll
         for (int q = 0; q < QT; ++q) myacc[q] = acc[q];
