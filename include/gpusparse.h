@@ -201,7 +201,8 @@ GS_API int32_t gs_dispatch_model(int64_t num_docs, int32_t tile_docs, int64_t st
  * out_doc_ids [B*k] int32, out_scores [B*k] float (GS_W_F32) or int32_t (GS_W_U8), row-major, each row sorted by
  * (score desc, doc id asc).  If k > N, slots >= N hold id -1 and score -inf / INT32_MIN.  Query term ids outside
  * [0,V) are ignored unless validation is on.  B == 0 is legal (nothing is written; the output pointers may then be
- * NULL).  Limits: B <= 65535 queries per call, k <= GS_MAX_K, a query row holds fewer than 2^24 terms.
+ * NULL).  Limits: B <= 65535 queries per call, k <= GS_MAX_K, a query row holds fewer than 2^19 terms (longer rows are
+ * treated as empty and reported as GS_ERR_OUT_OF_RANGE under GS_FLAG_VALIDATE_QUERIES).
  * workspace: >= gs_search_workspace_bytes(...) bytes, 256-byte aligned; it must stay untouched until the search (and
  * its gs_search_finish) is done.
  *

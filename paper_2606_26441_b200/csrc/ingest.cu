@@ -30,7 +30,7 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
     int64_t a = indptr[b], e = indptr[b + 1];
     // memory safety: the row's range must lie inside the nnz-sized arrays (always checked); a bad row is treated as empty
     // and reported as GS_ERR_OUT_OF_RANGE (returned to the caller when validation is on)
-    if (a < 0 || e < a || e > nnz || (b == 0 && a != 0)) {
+    if (a < 0 || e < a || e > nnz || (b == 0 && a != 0) || e - a >= (1 << 19)) {      // rows of >= 2^19 terms: not supported
         if (lane == 0) atomicCAS(status, 0, (int)GS_ERR_OUT_OF_RANGE);
         a = e = 0;
     }

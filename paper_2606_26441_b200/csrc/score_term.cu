@@ -512,7 +512,9 @@ __device__ __forceinline__ void resolve_segments(const TermParams& p, const Prob
     }
 }
 __device__ __forceinline__ void probe_query(const TermParams& p, int64_t b, bool filter, Probe2& r) {
-    r.cnt_nh = __ldg(p.tail_cnt + b) | (__ldg(p.head_cnt + b) << 16);
+    // tail count (19 bits: ingest rejects longer rows) | head terms << 19 (7 bits) | hot ones << 26 (6 bits)
+    const int hc = __ldg(p.head_cnt + b);
+    r.cnt_nh = __ldg(p.tail_cnt + b) | ((hc & 0xFF) << 19) | ((hc >> 8) << 26);
     r.thr = filter ? __ldg(p.sink.thr + b) : 0ull;
 }
 
@@ -778,7 +780,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
             q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
         }
-        const int nh = (cur.cnt_nh >> 16) & 0xFF, n_hot = cur.cnt_nh >> 24, cnt = cur.cnt_nh & 0xFFFF;
+        const int nh = (cur.cnt_nh >> 19) & 0x7F, n_hot = (int)((uint32_t)cur.cnt_nh >> 26), cnt = cur.cnt_nh & 0x7FFFF;
         const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
         const uint64_t thr = cur.thr;
 
@@ -1172,7 +1174,7 @@ __global__ void __launch_bounds__(kMQ * 32, 1) k_score_term_mma(const TermParams
             for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
             __syncwarp();
             if (q < q_end) {
-                const int cnt = cur.cnt_nh & 0xFFFF;
+                const int cnt = cur.cnt_nh & 0x7FFFF;
                 uint32_t lo, hi;
                 resolve_segments(p, cur, tile, lane, lo, hi);
                 scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane);

@@ -6,7 +6,9 @@ partial top-k lists on the HOST (0.6x of one GPU at 100K docs); its future work 
 merge over NVLink.  Contiguous doc-id ranges are independent: every rank indexes its own range and returns its own
 [B, k] (local id, score); ONE exchange — an all-gather of B*k*8 bytes per rank (4 MB at B=500, k=1000: latency bound
 over NVLink 5 / NVSwitch) — and a k-way merge under the same order (score desc, global doc id asc) give exactly the
-single-index result, ties included.  The merge is ``gs_merge_topk`` (CUDA, merge.cu); this module holds the host
+single-index result, ties included, in integer-impact mode; in fp32 the merge itself is exact, but a shard picks its own
+dense strips, so a score may differ from the single-index one by the rounding of another accumulation order (inside the
+1e-5 tolerance; the tests compare sharded fp32 results with the oracle, not with the single index).  The merge is ``gs_merge_topk`` (CUDA, merge.cu); this module holds the host
 logic only: the ranges, the exchange and the call.  No scoring arithmetic lives here.
 """
 from __future__ import annotations
