@@ -40,7 +40,7 @@ template <typename K> inline cudaError_t gs_optin_smem(K kern) { return gs_optin
 
 // Per-term entry of the tile-segment tables (16 bytes: one 128-bit load).  "Which slots of PL(t) hold documents of doc tile
 // j?" is answered in one of two ways, chosen per term at build time:
-//   mode GS_SEG_FULL   (len >= 2 * ntiles: almost every tile holds a posting): seg_tab[tab_off + j] = number of postings of t
+//   mode GS_SEG_FULL   (len >= ntiles / 2: a posting in every other doc tile or more): seg_tab[tab_off + j] = number of postings of t
 //                      with doc tile < j, j in [0, ntiles] — two adjacent loads give the slot range;
 //   mode GS_SEG_SPARSE (rare terms, empty in most tiles): seg_l1[tab_off + (j >> 5)] = (bit mask of the non-empty tiles of
 //                      the 32-tile group, index into seg_l2 of the group's first non-empty tile); seg_l2[i] = list position

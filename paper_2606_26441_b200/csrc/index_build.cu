@@ -492,7 +492,10 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         std::vector<gs_term_meta> h_meta((size_t)V);
         int64_t n_ent = 0, n_l1 = 0;
         for (int32_t t = 0; t < V; ++t) {
-            const bool full = (int64_t)h_len[t] >= 2 * (int64_t)ix->ntiles && h_len[t] > 0;
+            // full mode from one posting per two doc tiles on: the two-level lookup of the sparse mode costs a dependent load
+            // when the tile is not empty (B200, 8.8M docs, 500 queries: threshold 2 postings per tile 16.3 ms per batch and
+            // 1.00 GB of tables; 1/2: 15.6 ms, 1.21 GB; 1/8: 15.5 ms, 2.10 GB)
+            const bool full = (int64_t)h_len[t] * 2 >= (int64_t)ix->ntiles && h_len[t] > 0;
             h_meta[t].mode = full ? GS_SEG_FULL : GS_SEG_SPARSE;
             h_meta[t].tab_off = (uint32_t)(full ? n_ent : n_l1);
             h_meta[t].list_blk = (uint32_t)(h_off[t] / GS_WARP_BLOCK);
