@@ -5,7 +5,7 @@ statement of the trade-off (the scatter side wins whenever a batch amortises the
 sweep recorded in profiles/r02_dispatch_sweep.md (which path was faster at each grid point).
 GPU part: AUTO really takes both outcomes, and each outcome matches the oracle.
 """
-import json
+import csv
 import os
 
 import numpy as np
@@ -37,14 +37,16 @@ def test_model_picks_term_parallel_for_batches_and_doc_parallel_for_single_long_
 
 
 def test_model_agrees_with_the_recorded_b200_sweep():
-    """profiles/r02_dispatch_sweep.json: measured ms of both paths on a 4 x 4 x 4 grid (collection, batch, query length).
+    """profiles/r02_dispatch_sweep.csv: measured ms of both paths on a 4 x 4 x 4 grid (collection, batch, query length).
     The model must name the faster path wherever the two differ by more than 10 %."""
     from paper_2606_26441_b200 import binding as gs
-    grid = json.load(open(os.path.join(ROOT, "profiles", "r02_dispatch_sweep.json")))
+    with open(os.path.join(ROOT, "profiles", "r02_dispatch_sweep.csv"), newline="") as f:
+        grid = [{k: (v if k == "winner" else float(v)) for k, v in r.items()} for r in csv.DictReader(f)]
     assert len(grid) >= 64
     wrong = 0
     for r in grid:
-        algo, _, _ = gs.dispatch_model(r["n_docs"], 512, stream_bytes(r["n_docs"], r["doc_nnz"]), r["B"], r["B"] * r["q_nnz"])
+        algo, _, _ = gs.dispatch_model(int(r["n_docs"]), 512, stream_bytes(int(r["n_docs"]), int(r["doc_nnz"])), int(r["B"]),
+                                       int(r["B"] * r["q_nnz"]))
         fast, slow = sorted((r["term_ms"], r["doc_ms"]))
         if slow > 1.10 * fast:
             assert algo == r["winner"], r
