@@ -493,8 +493,9 @@ gs_status_t build_typed(gs_index* ix, const gs_csr_t* docs, const gs_build_opts_
         int64_t n_ent = 0, n_l1 = 0;
         for (int32_t t = 0; t < V; ++t) {
             // full mode from one posting per two doc tiles on: the two-level lookup of the sparse mode costs a dependent load
-            // when the tile is not empty (B200, 8.8M docs, 500 queries: threshold 2 postings per tile 16.3 ms per batch and
-            // 1.00 GB of tables; 1/2: 15.6 ms, 1.21 GB; 1/8: 15.5 ms, 2.10 GB)
+            // when the tile is not empty.  Tables: 1.00 GB at a threshold of 2 postings per tile, 1.21 GB at 1/2, 2.10 GB at
+            // 1/8 (8.8M docs); same-box A/B of 2 vs 1/2 on the 500-query batch: 16.75 vs 16.6 ms, i.e. within the run-to-run
+            // noise (B200 units of the pool differ by ~5 %, which an earlier cross-box comparison mistook for a gain)
             const bool full = (int64_t)h_len[t] * 2 >= (int64_t)ix->ntiles && h_len[t] > 0;
             h_meta[t].mode = full ? GS_SEG_FULL : GS_SEG_SPARSE;
             h_meta[t].tab_off = (uint32_t)(full ? n_ent : n_l1);
