@@ -645,12 +645,17 @@ __device__ __noinline__ void batch_issue_strips(const W* g, int64_t ld, int H, u
                      ::"r"(strip_s + (uint32_t)h * row_bytes), "l"(g + (size_t)h * ld), "r"(row_bytes), "r"(mbar_s) : "memory");
 }
 
+// Waits for a phase of an mbarrier.  The try_wait carries a suspend-time hint and a failed try is followed by a short sleep:
+// a bare try_wait loop returned so often that the waiting warps executed 16 % of the kernel's instructions
+// (profiles/r02_kernels.md), in issue slots the working warps of the SM need.
 __device__ __forceinline__ void mbar_wait(uint32_t mbar_s, uint32_t parity) {
     uint32_t ok = 0;
-    do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(mbar_s), "r"(parity) : "memory");
-    } while (!ok);
+    for (;;) {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(mbar_s), "r"(parity), "r"(2000u) : "memory");
+        if (ok) break;
+        __nanosleep(200);
+    }
 }
 
 // Every warp, once per work item, before its first head phase: waits for the item's strips (TMA, first mbarrier).  With
