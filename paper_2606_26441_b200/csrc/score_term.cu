@@ -940,22 +940,35 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                                                                               : ((uint32_t)(thr >> 32) ^ 0x80000000u)));
         const int64_t thr_cell = (int64_t)(0xFFFFFFFFu - (uint32_t)thr) - (int64_t)base;   // threshold doc as a cell of this tile
         const int tie_cells = (int)max((int64_t)-1, min((int64_t)kBT, thr_cell));           // cells <= this index win a score tie
+        // bit 4r+u of `hit`: the lane's cell (r, u) reaches the threshold score.  A row has a few such cells, spread over the
+        // lanes: testing them one unrolled cell at a time made the warp run the emission body once per distinct (r, u)
+        // position with a hit (3.7 times per row); with the mask it runs once per hit of the busiest lane (1-2 times).
+        uint32_t hit = 0u;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < 4; ++r)
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (sc[r][u] >= thr_s) {                                 // rare (a few cells per row)
-                    const int cell = 4 * (lane + 32 * r) + u;
-                    if (cell < n_live && (sc[r][u] > thr_s || cell <= tie_cells)) {
-                        const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(sc[r][u])), (uint32_t)(base + cell));
-                        const uint32_t slot = atomicAdd(w_cnt, 1u);
-                        if (slot < (uint32_t)kWarpBuf) {
-                            w_key[slot] = key;
-                            w_q[slot] = (uint16_t)q;
-                        } else {                                         // buffer full: append directly
-                            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
-                            if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
-                        }
+            for (int u = 0; u < 4; ++u) hit |= sc[r][u] >= thr_s ? 1u << (4 * r + u) : 0u;
+        if (hit) {
+            // the lane's scores go back to its own cells of the row (nobody else reads them) to be picked by index
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                reinterpret_cast<uint4*>(row)[lane + 32 * r] = make_uint4(Num<WT>::bits(sc[r][0]), Num<WT>::bits(sc[r][1]),
+                                                                         Num<WT>::bits(sc[r][2]), Num<WT>::bits(sc[r][3]));
+#pragma unroll 1
+            while (hit) {
+                const int i = __ffs((int)hit) - 1;
+                hit &= hit - 1u;
+                const int cell = 4 * (lane + 32 * (i >> 2)) + (i & 3);
+                const A v = row[cell];
+                if (cell < n_live && (v > thr_s || cell <= tie_cells)) {
+                    const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(v)), (uint32_t)(base + cell));
+                    const uint32_t slot = atomicAdd(w_cnt, 1u);
+                    if (slot < (uint32_t)kWarpBuf) {
+                        w_key[slot] = key;
+                        w_q[slot] = (uint16_t)q;
+                    } else {                                             // buffer full: append directly
+                        const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                        if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                     }
                 }
             }
