@@ -526,9 +526,10 @@ __device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
 
 // Applies up to 32 posting-list segments (lane s: n postings from slot `start`, query weight bits wq) to `row`.
 // `desc_s` = shared-window address of the warp's 32-entry descriptor table.
+// `tag` (may be null): 512 bytes of shared memory owned by the warp, one per cell of the row — see the conflict pass below.
 template <int WT>
 __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<WT>::A* row, uint32_t desc_s, int n,
-                                             uint32_t start, uint32_t wq, int32_t base, int lane) {
+                                             uint32_t start, uint32_t wq, int32_t base, int lane, uint8_t* tag = nullptr) {
     using W = typename Num<WT>::W;
     using A = typename Num<WT>::A;
     int incl = n;
@@ -579,11 +580,30 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
             if (f0 + 32 * r < T) {                  // uniform
                 A* cell = row + (doc[r] - base);
                 const A q = Num<WT>::qw(qv[r]), w = wv[r];
-                const int o_hi = __popc(sm[r]);
-                // segment by segment: two lists may hit the same document, one list never does
-                for (int o = (int)(sm[r] & 1u); o <= o_hi; ++o) {
-                    if (ord[r] == o) *cell = Num<WT>::mac(*cell, q, w);
-                    __syncwarp();
+                if (tag != nullptr) {
+                    // Two lists may hit the same document in one round (one list never does).  Every lane writes its lane
+                    // number to the cell's tag byte; the lane whose number stays there owns the cell in this pass and
+                    // does its read-modify-write, the others (rare) go round again.  One pass in the common case instead
+                    // of one pass per list of the round.  Which lane a same-address store leaves behind is fixed-function
+                    // arbitration: the same lane in every run, so the fp32 sums stay reproducible run to run.
+                    uint8_t* tg = tag + (doc[r] - base);
+                    bool todo = ord[r] >= 0;
+                    while (__any_sync(0xFFFFFFFFu, todo)) {
+                        if (todo) *reinterpret_cast<volatile uint8_t*>(tg) = (uint8_t)lane;
+                        __syncwarp();
+                        if (todo && *reinterpret_cast<volatile uint8_t*>(tg) == (uint8_t)lane) {
+                            *cell = Num<WT>::mac(*cell, q, w);
+                            todo = false;
+                        }
+                        __syncwarp();
+                    }
+                } else {
+                    const int o_hi = __popc(sm[r]);
+                    // segment by segment: two lists may hit the same document, one list never does
+                    for (int o = (int)(sm[r] & 1u); o <= o_hi; ++o) {
+                        if (ord[r] == o) *cell = Num<WT>::mac(*cell, q, w);
+                        __syncwarp();
+                    }
                 }
             }
         }
@@ -595,6 +615,16 @@ __device__ __forceinline__ void scatter_flat(const TermParams& p, typename Num<W
 constexpr int kWarpBuf = 80;                  // candidate keys a warp collects in shared memory before it appends them
 constexpr int kFlushAt = 40;                  // ... which it does at the end of a row once it holds more than this many
 constexpr int kCandBuf = kBWarps * kWarpBuf;
+// The fp32 batch kernel gives 16 KB of its shared memory to the cell tags of scatter_flat (227 KB per CTA, 192 KB of them rows
+// and strips) and keeps a smaller candidate buffer; the integer kernel has room (strips are a quarter of the bytes) but its
+// tail is faster with the per-list passes (same-box A/B: 12.44 vs 13.08 ms per batch), so it keeps them and the big buffer.
+template <int WT> struct BatchGeo {
+    static constexpr bool kTags = WT == GS_W_F32;
+    static constexpr int kBuf = kTags ? 32 : kWarpBuf;
+    static constexpr int kFlush = kBuf / 2;
+    static constexpr size_t kTagBytes = kTags ? (size_t)kBWarps * 512 : 0;
+    static constexpr size_t kFixed = (size_t)kBWarps * 32 * 8 + (size_t)kBWarps * kBuf * 10 + (size_t)(kBWarps + 4) * 4 + 32 + 128 + kTagBytes;
+};
 
 // ---- cold paths of the batch kernel, kept out of line: the kernel's warps sit in different phases of the row loop, so
 // the loop body has to fit the instruction cache (a 116 KB variant of this kernel ran at half the speed of a 45 KB one).
@@ -604,9 +634,9 @@ constexpr int kCandBuf = kBWarps * kWarpBuf;
 // query's list with ONE atomic (same-address atomics of one warp instruction are served one after the other, each a round
 // trip: 32 lanes on two or three counters cost tens of microseconds per flush).
 __device__ __noinline__ void batch_flush(uint32_t* cand_cnt, uint64_t* cand, int64_t cand_cap, int64_t q0, const uint64_t* w_key,
-                                         const uint16_t* w_q, uint32_t* w_cnt, int lane) {
+                                         const uint16_t* w_q, uint32_t* w_cnt, int lane, int wbuf = kWarpBuf) {
     __syncwarp();
-    const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)kWarpBuf);
+    const uint32_t n_buf = min(*reinterpret_cast<volatile uint32_t*>(w_cnt), (uint32_t)wbuf);
     const unsigned le_ = 0xFFFFFFFFu >> (31 - lane);
 #pragma unroll 1
     for (uint32_t i0 = 0; i0 < n_buf; i0 += 32) {
@@ -701,15 +731,18 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     // counters of the even / odd work items) | mbarrier | strips [H][kBT]
     constexpr size_t kOffDesc = (size_t)kBWarps * kBT * 4;
     constexpr size_t kOffKey = kOffDesc + (size_t)kBWarps * 32 * 8;
-    constexpr size_t kOffQ = kOffKey + (size_t)kCandBuf * 8;
-    constexpr size_t kOffCnt = kOffQ + (size_t)kCandBuf * 2;
+    constexpr int WB = BatchGeo<WT>::kBuf;                                   // candidate keys the warp buffers
+    constexpr size_t kOffQ = kOffKey + (size_t)kBWarps * WB * 8;
+    constexpr size_t kOffCnt = kOffQ + (size_t)kBWarps * WB * 2;
     constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;       // mbarrier (strip copy) | mbarrier (TMEM copy) |
-    constexpr size_t kOffStrip = (kOffBar + 32 + 127) / 128 * 128;         // TMEM base address, copy-claimed flags [2]
+    constexpr size_t kOffTag = kOffBar + 32;                                // TMEM base address, copy-claimed flags [2] | cell tags
+    constexpr size_t kOffStrip = (kOffTag + BatchGeo<WT>::kTagBytes + 127) / 128 * 128;   // [kBWarps][kBT] bytes (scatter_flat, fp32)
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
     const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
-    uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey) + warp * kWarpBuf;     // the warp's candidate buffer
-    uint16_t* w_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ) + warp * kWarpBuf;
+    uint64_t* w_key = reinterpret_cast<uint64_t*>(smem_raw + kOffKey) + warp * WB;          // the warp's candidate buffer
+    uint16_t* w_q = reinterpret_cast<uint16_t*>(smem_raw + kOffQ) + warp * WB;
     uint32_t* w_cnt = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + warp;
+    uint8_t* w_tag = BatchGeo<WT>::kTags ? smem_raw + kOffTag + (size_t)warp * kBT : nullptr;
     uint32_t* s_next = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + kBWarps;           // [2]
     uint32_t* s_done = s_next + 2;                                                            // [2]
     W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
@@ -795,7 +828,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         {
             uint32_t lo, hi;
             resolve_segments(p, cur, tile, lane, lo, hi);
-            scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane);
+            scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane, w_tag);
         }
         if (cnt > GS_TAIL32) {                      // more than 32 tail terms: probed in line
             const int64_t qa = p.q_indptr[b];
@@ -805,7 +838,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 if (i0 + lane < cnt) d = __ldg(p.tail_desc + qa + i0 + lane);
                 uint32_t lo, hi;
                 probe_range(p, d, tile, lo, hi);
-                scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, d.x, base, lane);
+                scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, d.x, base, lane, w_tag);
             }
         }
         __syncwarp();
@@ -963,7 +996,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 if (cell < n_live && (v > thr_s || cell <= tie_cells)) {
                     const uint64_t key = gs_make_key(gs_ord_bits<WT>(Num<WT>::bits(v)), (uint32_t)(base + cell));
                     const uint32_t slot = atomicAdd(w_cnt, 1u);
-                    if (slot < (uint32_t)kWarpBuf) {
+                    if (slot < (uint32_t)WB) {
                         w_key[slot] = key;
                         w_q[slot] = (uint16_t)q;
                     } else {                                             // buffer full: append directly
@@ -974,8 +1007,8 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
         }
         __syncwarp();
-        if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)kFlushAt)
-            batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
+        if (*reinterpret_cast<volatile uint32_t*>(w_cnt) > (uint32_t)BatchGeo<WT>::kFlush)
+            batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane, WB);
     }
     // out of rows in this item.  Every warp observes every phase of the mbarrier (a warp without rows too: a wait for the
     // NEXT phase issued while this one is still pending would be satisfied at once), then reports itself done.
@@ -992,7 +1025,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     }
     __syncwarp();
     }
-    if (filter) batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane);
+    if (filter) batch_flush(p.sink.cand_cnt, p.sink.cand, p.sink.cand_cap, p.q0, w_key, w_q, w_cnt, lane, WB);
     if (kTmem) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
@@ -1351,7 +1384,7 @@ gs_status_t gs_launch_score_term(const gs_index* ix, const gs_qbatch& qb, int64_
         p.n_chunks = (int32_t)((nq + p.chunk - 1) / p.chunk);
         const int64_t grid = (int64_t)ts.count * p.n_chunks;
         if (grid > 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
-        const size_t smem_batch = smem_staged + (size_t)kBWarps * 32 * 8 + (size_t)kCandBuf * 10 + (size_t)(kBWarps + 4) * 4 + 32 + 128;
+        const size_t smem_batch = smem_staged + (ix->wtype == GS_W_F32 ? BatchGeo<GS_W_F32>::kFixed : BatchGeo<GS_W_U8>::kFixed);
         if (group == 0 && ix->Ts == kBT && ix->wtype == GS_W_U8 && use_mma && ix->mma_strips != nullptr &&
             (ix->HX == 0 || qb.x_on) && kMSmem <= (size_t)smem_max && nq <= 65535) {
             // integer impacts: the head contraction on the tensor cores
