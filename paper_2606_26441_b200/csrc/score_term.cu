@@ -407,25 +407,28 @@ __global__ void __launch_bounds__(kWarpsStaged * 32, 1) k_score_term_staged(cons
 // ------------------------------------------------------------------------------------------------
 // Batch kernel (Ts == 512, >= kStagedMinQueries queries, < 2^32 posting slots): same ownership as above — a persistent
 // CTA per doc tile stages the tile's strips once, a warp owns one (query, tile) cell row at a time — with the three
-// per-row phases rebuilt around what the ncu source view of the staged kernel showed (profiles/r01d_term_kernel.md:
+// per-row phases rebuilt around what the ncu source view of the staged kernel showed (profiles/r01d_kernels.md:
 // the tail scatter, 8 % of the multiply-adds, took half of the instructions and 57 % of the stall samples):
 //   * tail: the row's non-empty segments are FLATTENED into one posting stream.  An exclusive scan of the segment
 //     lengths gives every segment its start in the stream; in a round of 32 flat postings a lane finds its segment
 //     with one warp OR-reduction (bit i = "a segment starts at flat position f0+i") and a popcount, fetches
 //     (segment start - stream start, query weight) from a 32-entry per-warp table in shared memory, and loads its
 //     posting: every lane is busy, and the loads of kRounds rounds are in flight together.  The read-modify-writes
-//     of a round are issued segment by segment (two lists may hit the same document; one list never does), so the
-//     order of the additions into a cell is the query's term order: deterministic, no atomics;
+//     of a round resolve same-cell conflicts (two lists may hit the same document; one list never does) either list by
+//     list (integer mode: the order of the additions into a cell is the query's term order) or, fp32, with one tag byte
+//     per cell that picks the lane allowed to update it in this pass (scatter_flat): no atomics, reproducible run to run;
 //   * the probes (query terms -> segment table -> list offsets) of the NEXT TWO queries of the warp are prefetched
 //     (two-stage software pipeline) from the fixed-stride tail32 table;
 //   * head: a lane keeps its 16 documents in registers.  The query's compact strip lists are loaded once, one entry per
 //     lane, and broadcast by shuffle.  fp32: the GS_HOT_STRIPS densest strips of the tile live in TENSOR MEMORY (one
 //     tcgen05.ld.32x32b.x16 per strip feeds eight FFMA2, see tmem_ld16_wait), the other strips in shared memory (one
 //     LDS.128 feeds two FFMA2), the second-tier strips come from global memory.  Integer mode: one IDP4A per cell;
-//   * filter: a cell that reaches the threshold score goes to the warp's candidate buffer in shared memory.
+//   * filter: a hit mask over the lane's 16 cells, then a loop over its set bits: a cell that passes goes to the warp's
+//     candidate buffer in shared memory.
 // Things measured and dropped in round 2 (profiles/r02_kernels.md): a 16-warp x 128-register variant that worked on two
-// rows per warp (one per half-warp in the tail phase, strip loads double-buffered) — 20.2 ms against 16.4 ms; an L2
-// prefetch of the next row's posting segments — 16.9 ms.
+// rows per warp (one per half-warp in the tail phase, strip loads double-buffered) — 20.2 ms against 16.4 ms; L2
+// prefetches (next row's posting segments, next doc tile's strips), second-tier strips in the hot strips' staging rows,
+// deeper unrolling of the strip loops — each slower or within the noise in a same-unit A/B.
 // ------------------------------------------------------------------------------------------------
 constexpr int kBT = 512;          // documents per tile
 // Values kept after the sweeps of rounds 1 and 2 (profiles/r01d_kernels.md, profiles/r02_kernels.md): 24 warps x 80 registers
