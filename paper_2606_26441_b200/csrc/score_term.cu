@@ -479,8 +479,9 @@ __device__ __forceinline__ void tmem_ld16_wait(uint32_t taddr, unsigned long lon
 struct Probe1 { uint32_t wq, off, mode; };                           // query terms (first 32 tail terms, one per lane)
 // + the terms' segments inside the tile.  A lane whose bit is clear in `sparse`: slot range [a, b).  A lane whose bit is
 // set (sparse-mode term): (a, b) = the (mask, seg_l2 index) entry of the tile's 32-tile group, turned into a slot range
-// by resolve_segments when the row is processed (the entry's load stays in flight until then).  Plus tail count,
-// head counts << 16 (as in head_cnt) and the threshold key of the query.
+// by resolve_segments (the batch kernel: after the previous row's head phase, so the entry's load and then the
+// second-level loads are in flight behind other work).  Plus tail count | head counts (probe_query) and the threshold
+// key of the query.
 struct Probe2 { uint32_t a, b, wq, sparse; int32_t cnt_nh; uint64_t thr; };
 
 __device__ __forceinline__ Probe1 probe_terms(const TermParams& p, int64_t b, int lane) {
@@ -696,26 +697,36 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar_s, uint32_t parity) {
 // is free.  The first warp here copies the hot strips shared memory -> tensor memory: one tcgen05.cp.32x128b.warpx4 per
 // (strip, 128 documents) moves 32 rows of 16 bytes and writes them to all four lane quarters; the copies complete on the
 // second mbarrier, which every warp then waits for.  s_tmem: [0] TMEM base, [1..2] copy claimed (per parity).
-template <bool TMEM>
+template <bool TMEM, size_t OFF>
 __device__ __noinline__ void batch_wait_strips(uint32_t mbar_s, uint32_t strip_s, uint32_t* s_tmem, int n_hot_strips, int par, int lane) {
     mbar_wait(mbar_s, (uint32_t)par);
     if (TMEM) {
         const uint32_t mbar2_s = mbar_s + 8u;
-        if (lane == 0 && atomicExch(s_tmem + 1 + par, 1u) == 0u) {
-            s_tmem[1 + (par ^ 1)] = 0u;             // nobody claims the next item before this one's strips have landed
-            const uint32_t t0 = s_tmem[0];
+        uint32_t claimed = 0u;
+        if (lane == 0) claimed = atomicExch(s_tmem + 1 + par, 1u) == 0u ? 1u : 0u;
+        // The claiming warp runs the copy loop as a whole, every value a broadcast of lane 0's (so the compiler keeps the
+        // descriptors in uniform registers: issued from a divergent lane each tcgen05.cp sat in a register-to-uniform
+        // "waterfall" loop and the 128 copies took 8.8 K cycles), one elected lane issuing the copies.
+        if (__shfl_sync(0xFFFFFFFFu, claimed, 0)) {
+            if (lane == 0) s_tmem[1 + (par ^ 1)] = 0u;    // nobody claims the next item before this one's strips have landed
+            const uint32_t t0 = __shfl_sync(0xFFFFFFFFu, s_tmem[0], 0);
+            extern __shared__ __align__(16) unsigned char smem_raw[];
+            const uint32_t ss = (uint32_t)__cvta_generic_to_shared(smem_raw) + (uint32_t)OFF;   // = strip_s, as a constant
+            const int nhs = __shfl_sync(0xFFFFFFFFu, n_hot_strips, 0);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-            for (int h = 0; h < n_hot_strips; ++h)
+            for (int h = 0; h < nhs; ++h)
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
                     // shared-memory matrix descriptor, no swizzle: start address >> 4, leading byte offset (unused: one
                     // 16-byte column), stride byte offset 128 (8 rows of 16 bytes are contiguous) >> 4, version 1
-                    const uint32_t a = strip_s + (uint32_t)(h * (kBT * 4) + r * 512);
+                    const uint32_t a = ss + (uint32_t)(h * (kBT * 4) + r * 512);
                     const unsigned long long d = (unsigned long long)((a & 0x3FFFFu) >> 4) | (1ull << 16) | (8ull << 32) | (1ull << 46);
-                    asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(t0 + (uint32_t)(h * 16 + r * 4)), "l"(d) : "memory");
+                    asm volatile("{ .reg .pred p; elect.sync _|p, 0xFFFFFFFF;\n\t@p tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1; }"
+                                 ::"r"(t0 + (uint32_t)(h * 16 + r * 4)), "l"(d) : "memory");
                 }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar2_s) : "memory");
+            asm volatile("{ .reg .pred p; elect.sync _|p, 0xFFFFFFFF;\n\t@p tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0]; }"
+                         ::"r"(mbar2_s) : "memory");
         }
         __syncwarp();
         mbar_wait(mbar2_s, (uint32_t)par);
@@ -737,8 +748,8 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     constexpr int WB = BatchGeo<WT>::kBuf;                                   // candidate keys the warp buffers
     constexpr size_t kOffQ = kOffKey + (size_t)kBWarps * WB * 8;
     constexpr size_t kOffCnt = kOffQ + (size_t)kBWarps * WB * 2;
-    constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;       // mbarrier (strip copy) | mbarrier (TMEM copy) |
-    constexpr size_t kOffTag = kOffBar + 32;                                // TMEM base address, copy-claimed flags [2] | cell tags
+    constexpr size_t kOffBar = kOffCnt + (size_t)(kBWarps + 4) * 4;       // (32 bytes unused: the barriers are static, s_ctl)
+    constexpr size_t kOffTag = kOffBar + 32;                                // cell tags
     constexpr size_t kOffStrip = (kOffTag + BatchGeo<WT>::kTagBytes + 127) / 128 * 128;   // [kBWarps][kBT] bytes (scatter_flat, fp32)
     A* row = reinterpret_cast<A*>(smem_raw) + (size_t)warp * kBT;
     const uint32_t desc_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffDesc) + (uint32_t)warp * 256u;
@@ -749,9 +760,13 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     uint32_t* s_next = reinterpret_cast<uint32_t*>(smem_raw + kOffCnt) + kBWarps;           // [2]
     uint32_t* s_done = s_next + 2;                                                            // [2]
     W* s_strip = reinterpret_cast<W*>(smem_raw + kOffStrip);
-    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(smem_raw + kOffBar);
+    // mbarrier (strip copy) | mbarrier (TMEM copy) | TMEM base address, copy-claimed flags [2].  Static shared memory: with
+    // these words in the dynamic block ptxas spilled three more values per row, and a spill reload is an L2 round trip
+    // here (227 KB of the SM's 256 KB are shared memory: the streaming loads leave nothing of the L1 for the stack).
+    __shared__ __align__(16) unsigned long long s_ctl[4];
+    const uint32_t mbar_s = (uint32_t)__cvta_generic_to_shared(s_ctl);
     const uint32_t mbar2_s = mbar_s + 8u;
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem_raw + kOffBar + 16);       // [0] TMEM base, [1..2] copy claimed (per parity)
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_ctl + 2);                     // [0] TMEM base, [1..2] copy claimed (per parity)
     constexpr bool kTmem = WT == GS_W_F32;      // hot strips in tensor memory (fp32; the impact strips are a quarter of the bytes)
     // A work item = (doc tile, chunk of queries).  The CTA is persistent: it takes items blockIdx.x, blockIdx.x + gridDim.x, ...
     // The item's strips come in by TMA: one thread issues a 1-D bulk copy per strip (kBT weights, contiguous in the
@@ -766,7 +781,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     };
     if (lane == 0) *w_cnt = 0u;
     if (threadIdx.x == 0) {
-        s_next[0] = s_next[1] = 2u * kBWarps;
+        s_next[0] = s_next[1] = (uint32_t)kBWarps;
         s_done[0] = s_done[1] = 0u;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar_s) : "memory");
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mbar2_s) : "memory");
@@ -793,34 +808,31 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     const int tile = p.ts.first + j * p.ts.stride;
     const int32_t base = tile * kBT;
     bool strips_ready = false;
-    // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with queries
-    // warp and warp + kBWarps of the chunk and claims further ones from a shared-memory counter, two rows ahead of the
-    // row it works on (the probes of the next two rows are in flight).
+    // Queries are handed out dynamically (a row's cost varies with the query's tail lists): a warp starts with query
+    // `warp` of the chunk and claims its next one from a shared-memory counter when it starts a row — ONE row ahead: the
+    // next row's terms are probed during this row's tail phase, its segments during the head phase.  (Claiming three
+    // rows ahead, to have deeper probes, left warps holding up to three unstarted rows at the end of an item while the
+    // others waited: 27 K cycles between the first and the last warp out of an item, measured.)
     const int q_end = min(p.nq, (chunk + 1) * p.chunk);
     int q = chunk * p.chunk + warp;             // row being processed
-    int q_n1 = q + kBWarps;                     // next row (segments probed)
-    int q_n2 = q_end;                           // row after that (terms probed)
-    int q_n3 = q_end;                           // claimed, not yet probed
-    Probe1 s1{0u, 0u, 0xFFFFFFFFu};
+    int q_n1 = q_end;                           // next row
     Probe2 s2{0u, 0u, 0u, 0u, 0, 0ull};
-    if (q < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile); probe_query(p, p.q0 + q, filter, s2); }
-    if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
-    {
-        int c = 0;
-        if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
-        q_n2 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;
+    if (q < q_end) {
+        s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile);
+        probe_query(p, p.q0 + q, filter, s2);
+        resolve_segments(p, s2, tile, lane, s2.a, s2.b);
     }
     const int n_live = (int)min((int64_t)kBT, p.N - (int64_t)base);                    // documents of this tile that exist
-    for (; q < q_end; q = q_n1, q_n1 = q_n2, q_n2 = q_n3) {
+    for (; q < q_end; q = q_n1) {
         const int64_t b = p.q0 + q;
         const Probe2 cur = s2;
-        if (q_n1 < q_end) { s2 = probe_segments(p, s1, tile); probe_query(p, p.q0 + q_n1, filter, s2); }
-        if (q_n2 < q_end) s1 = probe_terms(p, p.q0 + q_n2, lane);
         {
             int c = 0;
             if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
-            q_n3 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;      // used one row later
+            q_n1 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;
         }
+        Probe1 s1{0u, 0u, 0xFFFFFFFFu};
+        if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
         const int nh = (cur.cnt_nh >> 19) & 0x7F, n_hot = (int)((uint32_t)cur.cnt_nh >> 26), cnt = cur.cnt_nh & 0x7FFFF;
         const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
         const uint64_t thr = cur.thr;
@@ -828,11 +840,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
 #pragma unroll
         for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
         __syncwarp();
-        {
-            uint32_t lo, hi;
-            resolve_segments(p, cur, tile, lane, lo, hi);
-            scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane, w_tag);
-        }
+        scatter_flat<WT>(p, row, desc_s, (int)(cur.b - cur.a), cur.a, cur.wq, base, lane, w_tag);   // [a, b): resolved slot range
         if (cnt > GS_TAIL32) {                      // more than 32 tail terms: probed in line
             const int64_t qa = p.q_indptr[b];
             for (int i0 = GS_TAIL32; i0 < cnt; i0 += 32) {
@@ -845,9 +853,10 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
         }
         __syncwarp();
+        if (q_n1 < q_end) { s2 = probe_segments(p, s1, tile); probe_query(p, p.q0 + q_n1, filter, s2); }
 
         if (!strips_ready) {                        // once per warp and item
-            batch_wait_strips<kTmem>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
+            batch_wait_strips<kTmem, kOffStrip>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
             strips_ready = true;
         }
         // head strips: the lane's 16 documents (quads lane, lane+32, lane+64, lane+96) stay in registers
@@ -959,6 +968,10 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
         }
 
+        // the next row's sparse-mode entries have arrived during the head phase: their second-level lookups are issued
+        // now and land during the filter and the next row's zeroing, so the row starts on resolved slot ranges
+        if (q_n1 < q_end) resolve_segments(p, s2, tile, lane, s2.a, s2.b);
+
         if (!filter) {
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
@@ -1015,14 +1028,14 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     }
     // out of rows in this item.  Every warp observes every phase of the mbarrier (a warp without rows too: a wait for the
     // NEXT phase issued while this one is still pending would be satisfied at once), then reports itself done.
-    if (!strips_ready) batch_wait_strips<kTmem>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
+    if (!strips_ready) batch_wait_strips<kTmem, kOffStrip>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
     __syncwarp();
     if (kTmem) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");    // the warp's tensor-memory loads are done
     if (lane == 0) {
         __threadfence_block();
         if (atomicAdd(s_done + par, 1u) == (uint32_t)(kBWarps - 1)) {       // last warp out: the strips buffer is free
             s_done[par] = 0u;
-            s_next[par] = 2u * kBWarps;                                    // for the item after the next
+            s_next[par] = (uint32_t)kBWarps;                                   // for the item after the next
             if (item + (int)gridDim.x < n_items) batch_issue_strips<W>(item_strips(item + (int)gridDim.x), p.N_pad, p.H, strip_s, mbar_s);
         }
     }
