@@ -99,6 +99,14 @@ __global__ void k_ingest(const int64_t* __restrict__ indptr, const int32_t* __re
         __syncwarp();
     }
     if (lane == 0) { tail_cnt[b] = n_tail; head_cnt[b] = (n_hot + n_cold) | (n_hot << 8); xcnt[b] = n_x; }
+    // fourth word of the lane's tail32 entry: the query's counts, so that the batch kernels get them with the term in one
+    // 16-byte load: tail terms (19 bits) | cold head terms << 19 (6 bits) | hot head terms << 25 (6 bits) | bit 31: the
+    // lane's own term is a sparse-mode list (second-level segment lookup)
+    {
+        uint4* e = tail32 + b * GS_TAIL32 + lane;
+        const uint32_t mode = e->z;                 // written above, possibly by another lane (ordered by the __syncwarp)
+        e->w = (uint32_t)n_tail | ((uint32_t)n_cold << 19) | ((uint32_t)n_hot << 25) | (mode == GS_SEG_SPARSE ? 0x80000000u : 0u);
+    }
 }
 
 }  // namespace

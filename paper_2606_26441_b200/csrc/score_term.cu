@@ -476,23 +476,23 @@ __device__ __forceinline__ void tmem_ld16_wait(uint32_t taddr, unsigned long lon
         : "r"(taddr) : "memory");
 }
 
-struct Probe1 { uint32_t wq, off, mode; };                           // query terms (first 32 tail terms, one per lane)
-// + the terms' segments inside the tile.  A lane whose bit is clear in `sparse`: slot range [a, b).  A lane whose bit is
-// set (sparse-mode term): (a, b) = the (mask, seg_l2 index) entry of the tile's 32-tile group, turned into a slot range
-// by resolve_segments (the batch kernel: after the previous row's head phase, so the entry's load and then the
-// second-level loads are in flight behind other work).  Plus tail count | head counts (probe_query) and the threshold
-// key of the query.
-struct Probe2 { uint32_t a, b, wq, sparse; int32_t cnt_nh; uint64_t thr; };
+struct Probe1 { uint32_t wq, off, mode, info; };                     // query terms (first 32 tail terms, one per lane)
+// + the terms' segments inside the tile.  Full-mode term: slot range [a, b).  Sparse-mode term (bit 31 of info):
+// (a, b) = the (mask, seg_l2 index) entry of the tile's 32-tile group, turned into a slot range by resolve_segments (the
+// batch kernel: after the previous row's head phase, so the entry's load and then the second-level loads are in flight
+// behind other work).  info = the query's counts as ingest packs them into the fourth word of the tail32 entry: tail
+// terms (19 bits) | cold head terms << 19 | hot head terms << 25 | the lane's sparse-mode flag << 31 — they come with the
+// term in one 16-byte load (separate loads combined at probe time made the warp wait for them at the probe).
+struct Probe2 { uint32_t a, b, wq; int32_t info; };
 
 __device__ __forceinline__ Probe1 probe_terms(const TermParams& p, int64_t b, int lane) {
     const uint4 e = __ldg(p.tail32 + b * GS_TAIL32 + lane);
-    return Probe1{e.x, e.y, e.z};
+    return Probe1{e.x, e.y, e.z, e.w};
 }
 __device__ __forceinline__ Probe2 probe_segments(const TermParams& p, const Probe1& t, int tile) {
     Probe2 r;
     r.a = r.b = 0u;
-    r.wq = t.wq; r.cnt_nh = 0; r.thr = 0ull;
-    r.sparse = __ballot_sync(0xFFFFFFFFu, t.mode == GS_SEG_SPARSE);
+    r.wq = t.wq; r.info = (int32_t)t.info;
     if (t.mode == GS_SEG_FULL) {
         r.a = __ldg(p.seg_tab + t.off + tile);
         r.b = __ldg(p.seg_tab + t.off + tile + 1);
@@ -502,9 +502,9 @@ __device__ __forceinline__ Probe2 probe_segments(const TermParams& p, const Prob
     }
     return r;
 }
-__device__ __forceinline__ void resolve_segments(const TermParams& p, const Probe2& r, int tile, int lane, uint32_t& lo, uint32_t& hi) {
+__device__ __forceinline__ void resolve_segments(const TermParams& p, const Probe2& r, int tile, uint32_t& lo, uint32_t& hi) {
     lo = r.a; hi = r.b;
-    if ((r.sparse >> lane) & 1u) {
+    if (r.info < 0) {
         const uint32_t bit = 1u << (tile & 31);
         if (lo & bit) {
             const uint32_t idx = hi + (uint32_t)__popc(lo & (bit - 1u));
@@ -515,12 +515,9 @@ __device__ __forceinline__ void resolve_segments(const TermParams& p, const Prob
         }
     }
 }
-__device__ __forceinline__ void probe_query(const TermParams& p, int64_t b, bool filter, Probe2& r) {
-    // tail count (19 bits: ingest rejects longer rows) | head terms << 19 (7 bits) | hot ones << 26 (6 bits)
-    const int hc = __ldg(p.head_cnt + b);
-    r.cnt_nh = __ldg(p.tail_cnt + b) | ((hc & 0xFF) << 19) | ((hc >> 8) << 26);
-    r.thr = filter ? __ldg(p.sink.thr + b) : 0ull;
-}
+__device__ __forceinline__ int info_tail(int32_t info) { return info & 0x7FFFF; }
+__device__ __forceinline__ int info_cold(int32_t info) { return (info >> 19) & 0x3F; }
+__device__ __forceinline__ int info_hot(int32_t info) { return (info >> 25) & 0x3F; }
 
 __device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
     uint2 v;
@@ -816,11 +813,10 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
     const int q_end = min(p.nq, (chunk + 1) * p.chunk);
     int q = chunk * p.chunk + warp;             // row being processed
     int q_n1 = q_end;                           // next row
-    Probe2 s2{0u, 0u, 0u, 0u, 0, 0ull};
+    Probe2 s2{0u, 0u, 0u, 0};
     if (q < q_end) {
         s2 = probe_segments(p, probe_terms(p, p.q0 + q, lane), tile);
-        probe_query(p, p.q0 + q, filter, s2);
-        resolve_segments(p, s2, tile, lane, s2.a, s2.b);
+        resolve_segments(p, s2, tile, s2.a, s2.b);
     }
     const int n_live = (int)min((int64_t)kBT, p.N - (int64_t)base);                    // documents of this tile that exist
     for (; q < q_end; q = q_n1) {
@@ -831,11 +827,11 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (lane == 0) c = (int)atomicAdd(s_next + par, 1u);
             q_n1 = __shfl_sync(0xFFFFFFFFu, c, 0) + chunk * p.chunk;
         }
-        Probe1 s1{0u, 0u, 0xFFFFFFFFu};
+        Probe1 s1{0u, 0u, 0xFFFFFFFFu, 0u};
         if (q_n1 < q_end) s1 = probe_terms(p, p.q0 + q_n1, lane);
-        const int nh = (cur.cnt_nh >> 19) & 0x7F, n_hot = (int)((uint32_t)cur.cnt_nh >> 26), cnt = cur.cnt_nh & 0x7FFFF;
+        const int n_hot = info_hot(cur.info), nh = n_hot + info_cold(cur.info), cnt = info_tail(cur.info);
         const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
-        const uint64_t thr = cur.thr;
+        const uint64_t thr = filter ? __ldg(p.sink.thr + b) : 0ull;    // asked for now, used by the filter (not carried from row to row: registers)
 
 #pragma unroll
         for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
@@ -853,7 +849,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             }
         }
         __syncwarp();
-        if (q_n1 < q_end) { s2 = probe_segments(p, s1, tile); probe_query(p, p.q0 + q_n1, filter, s2); }
+        if (q_n1 < q_end) s2 = probe_segments(p, s1, tile);
 
         if (!strips_ready) {                        // once per warp and item
             batch_wait_strips<kTmem, kOffStrip>(mbar_s, strip_s, s_tmem, n_hot_strips, par, lane);
@@ -970,7 +966,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
 
         // the next row's sparse-mode entries have arrived during the head phase: their second-level lookups are issued
         // now and land during the filter and the next row's zeroing, so the row starts on resolved slot ranges
-        if (q_n1 < q_end) resolve_segments(p, s2, tile, lane, s2.a, s2.b);
+        if (q_n1 < q_end) resolve_segments(p, s2, tile, s2.a, s2.b);
 
         if (!filter) {
 #pragma unroll
@@ -1228,22 +1224,22 @@ __global__ void __launch_bounds__(kMQ * 32, 1) k_score_term_mma(const TermParams
         };
         for (int x = 0; x < min(kMLook, n_groups); ++x) b_ready(G + (uint32_t)x, q_beg + x * kMQ, x == 0, x + 1 == n_groups);
         // probes of the warp's query of the first group (terms -> segment tables), the next group's are asked for one group ahead
-        Probe2 s2{0u, 0u, 0u, 0u, 0, 0ull};
-        if (q_beg + warp < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q_beg + warp, lane), tile); probe_query(p, p.q0 + q_beg + warp, filter, s2); }
+        Probe2 s2{0u, 0u, 0u, 0};
+        if (q_beg + warp < q_end) s2 = probe_segments(p, probe_terms(p, p.q0 + q_beg + warp, lane), tile);
 #pragma unroll 1
         for (int g = 0; g < n_groups; ++g, ++G) {
             const int qg = q_beg + g * kMQ;
             const int q = qg + warp;
             const Probe2 cur = s2;
-            if (q + kMQ < q_end) { s2 = probe_segments(p, probe_terms(p, p.q0 + q + kMQ, lane), tile); probe_query(p, p.q0 + q + kMQ, filter, s2); }
+            if (q + kMQ < q_end) s2 = probe_segments(p, probe_terms(p, p.q0 + q + kMQ, lane), tile);
             // ---- tail: the row of query q
 #pragma unroll
             for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
             __syncwarp();
             if (q < q_end) {
-                const int cnt = cur.cnt_nh & 0x7FFFF;
+                const int cnt = info_tail(cur.info);
                 uint32_t lo, hi;
-                resolve_segments(p, cur, tile, lane, lo, hi);
+                resolve_segments(p, cur, tile, lo, hi);
                 scatter_flat<WT>(p, row, desc_s, (int)(hi - lo), lo, cur.wq, base, lane);
                 if (cnt > GS_TAIL32) {                  // more than 32 tail terms: probed in line
                     const int64_t qa = p.q_indptr[p.q0 + q];
