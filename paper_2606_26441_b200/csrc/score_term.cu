@@ -832,6 +832,16 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
         const int n_hot = info_hot(cur.info), nh = n_hot + info_cold(cur.info), cnt = info_tail(cur.info);
         const int nx = p.xcnt != nullptr ? __ldg(p.xcnt + b) : 0;      // asked for now, used after the tail and head phases
         const uint64_t thr = filter ? __ldg(p.sink.thr + b) : 0ull;    // asked for now, used by the filter (not carried from row to row: registers)
+        // fp32: the query's compact strip lists are loaded once, one entry per lane, and broadcast by shuffle in the head
+        // phase (a load per strip put an L1 round trip in front of every strip); asked for now, so that the head phase
+        // does not start with a wait for them
+        uint2 e_hot = make_uint2(0u, 0u), e_cold = make_uint2(0u, 0u), e_x = make_uint2(0u, 0u);
+        if (WT == GS_W_F32) {
+            const uint2* hl0 = p.head_pair + b * GS_HEAD_MAX;
+            if (lane < n_hot) e_hot = __ldg(hl0 + lane);
+            if (lane < nh - n_hot) e_cold = __ldg(hl0 + (GS_HEAD_MAX - 1 - lane));
+            if (p.xcnt != nullptr) e_x = __ldg(p.xpair + b * GS_XSTRIP_MAX + lane);    // entries past the query's count: unused
+        }
 
 #pragma unroll
         for (int r = 0; r < 4; ++r) reinterpret_cast<int4*>(row)[lane + 32 * r] = make_int4(0, 0, 0, 0);
@@ -865,10 +875,6 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                 const ulonglong2 a2 = reinterpret_cast<const ulonglong2*>(row)[lane + 32 * r];
                 acc[r][0] = a2.x; acc[r][1] = a2.y;
             }
-            // The query's compact strip lists are loaded once, one entry per lane, and broadcast by shuffle: a load per
-            // strip put an L1 round trip in front of every strip (profiles/r02_kernels.md).
-            const uint2 e_hot = lane < n_hot ? __ldg(hl + lane) : make_uint2(0u, 0u);
-            const uint2 e_cold = lane < nh - n_hot ? __ldg(hl + (GS_HEAD_MAX - 1 - lane)) : make_uint2(0u, 0u);
             // hot strips: the lane's 16 documents of a strip in one tensor-memory load
 #pragma unroll 2
             for (int i = 0; i < n_hot; ++i) {
@@ -900,7 +906,6 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
             if (nx > 0) {                          // second-tier strips: same contraction, the strip read from global memory
                 const uint2* xl = p.xpair + b * GS_XSTRIP_MAX;
                 const float* gx = reinterpret_cast<const float*>(p.xstrip) + (size_t)base + 4 * lane;
-                const uint2 e_x = lane < nx ? __ldg(xl + lane) : make_uint2(0u, 0u);
 #pragma unroll 1
                 for (int i = 0; i < nx; ++i) {
                     uint2 e;
