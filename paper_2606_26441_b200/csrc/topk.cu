@@ -231,7 +231,7 @@ constexpr int64_t kRowFusedMax = 1 << 20;
 constexpr int kRowUnroll = 4;
 
 template <int WT>
-__global__ void __launch_bounds__(kRowThreads) k_sel_row(gs_sel_src src, int32_t k, int kp2, int32_t* __restrict__ out_ids,
+__global__ void __launch_bounds__(kRowThreads, 2) k_sel_row(gs_sel_src src, int32_t k, int kp2, int32_t* __restrict__ out_ids,
                                                          uint32_t* __restrict__ out_scores, uint64_t* __restrict__ out_thr) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(kRowThreads) k_sel_row(gs_sel_src src, int32_t
     __shared__ unsigned long long s_prefix;
     __shared__ uint32_t s_krem, s_cnt;
     __shared__ int s_shift, s_done;
+    __shared__ long long s_live;                                               // dense rows: columns [0, s_live) are documents
     const int64_t b = blockIdx.x / C;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t n = src_count(src, b);
@@ -264,16 +265,42 @@ __global__ void __launch_bounds__(kRowThreads) k_sel_row(gs_sel_src src, int32_t
         s_shift = 64;
         s_done = live <= k ? 1 : 0;            // everything is selected: threshold key 0 (no live key is 0)
         s_cnt = 0;
+        s_live = live;                         // (columns are in doc order: only the end of the last tile can lie past the last document)
     }
     __syncthreads();
+    // Dense rows: while the digit lies in the score half of the key (digits never straddle bit 32: 11 + 11 + 10 bits, twice)
+    // an item is its 32 ordered score bits — no doc id, no 64-bit key; the doc half is only looked at to split score ties
+    // (rare) and for the few items the collect pass takes.
+    const bool dense = src.keys == nullptr;
+    const uint32_t* drow = dense ? src.dense + b * src.ld : nullptr;
+    const int64_t d_hi = dense ? min(i_hi, (int64_t)s_live) : 0;
     while (!s_done) {                          // every CTA of the cluster takes the same decisions
         const int shift = s_shift;
         const unsigned long long prefix = s_prefix;
-        const int width = min(GS_SEL_BITS, shift);
+        const int width = min(GS_SEL_BITS, shift > 32 ? shift - 32 : shift);
         const int lo = shift - width;
         const uint64_t himask = shift >= 64 ? 0ull : ~((1ull << shift) - 1ull);
         for (int i = tid; i < GS_SEL_BINS; i += kRowThreads) hist[i] = 0;
         __syncthreads();
+        if (dense && lo >= 32) {
+            const uint32_t pre32 = (uint32_t)(prefix >> 32), hm32 = (uint32_t)(himask >> 32);
+            const int lo32 = lo - 32;
+            for (int64_t base = i_lo; base < d_hi; base += kRowUnroll * kRowThreads) {
+                uint32_t o[kRowUnroll];
+#pragma unroll
+                for (int u = 0; u < kRowUnroll; ++u) {
+                    const int64_t i = base + tid + (int64_t)u * kRowThreads;
+                    o[u] = i < d_hi ? gs_ord_bits<WT>(drow[i]) : 0u;
+                }
+#pragma unroll
+                for (int u = 0; u < kRowUnroll; ++u) {
+                    const bool live = base + tid + (int64_t)u * kRowThreads < d_hi && (o[u] & hm32) == pre32;
+                    const uint32_t digit = live ? ((o[u] >> lo32) & ((1u << width) - 1u)) : 0xFFFFFFFFu;
+                    const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
+                    if (live && lane == __ffs(peers) - 1) atomicAdd(&hist[digit], (uint32_t)__popc(peers));
+                }
+            }
+        } else
         for (int64_t base = i_lo; base < i_hi; base += kRowUnroll * kRowThreads) {   // uniform trip count; loads in flight
             uint64_t key[kRowUnroll];
 #pragma unroll
@@ -338,10 +365,24 @@ __global__ void __launch_bounds__(kRowThreads) k_sel_row(gs_sel_src src, int32_t
     uint32_t* cnt0 = cluster.map_shared_rank(&s_cnt, 0);
     for (int64_t base = i_lo; base < i_hi; base += kRowUnroll * kRowThreads) {
         uint64_t key[kRowUnroll];
+        if (dense) {                           // the full key only of items whose score reaches the threshold's
+            uint32_t o[kRowUnroll];
 #pragma unroll
-        for (int u = 0; u < kRowUnroll; ++u) {
-            const int64_t i = base + tid + (int64_t)u * kRowThreads;
-            key[u] = i < i_hi ? src_key<WT>(src, b, i) : 0ull;
+            for (int u = 0; u < kRowUnroll; ++u) {
+                const int64_t i = base + tid + (int64_t)u * kRowThreads;
+                o[u] = i < d_hi ? gs_ord_bits<WT>(drow[i]) : 0u;
+            }
+#pragma unroll
+            for (int u = 0; u < kRowUnroll; ++u) {
+                const int64_t i = base + tid + (int64_t)u * kRowThreads;
+                key[u] = (i < d_hi && o[u] >= (uint32_t)(thr >> 32)) ? src_key<WT>(src, b, i) : 0ull;
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < kRowUnroll; ++u) {
+                const int64_t i = base + tid + (int64_t)u * kRowThreads;
+                key[u] = i < i_hi ? src_key<WT>(src, b, i) : 0ull;
+            }
         }
 #pragma unroll
         for (int u = 0; u < kRowUnroll; ++u) {
