@@ -296,8 +296,12 @@ __global__ void __launch_bounds__(kRowThreads, 2) k_sel_row(gs_sel_src src, int3
                 for (int u = 0; u < kRowUnroll; ++u) {
                     const bool live = base + tid + (int64_t)u * kRowThreads < d_hi && (o[u] & hm32) == pre32;
                     const uint32_t digit = live ? ((o[u] >> lo32) & ((1u << width) - 1u)) : 0xFFFFFFFFu;
-                    const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
-                    if (live && lane == __ffs(peers) - 1) atomicAdd(&hist[digit], (uint32_t)__popc(peers));
+                    // lanes of a warp mostly share the digit in the first pass (leading score bits) and mostly differ in
+                    // the later ones: one atomic for the warp when all agree, one per lane otherwise
+                    const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, digit, 0);
+                    if (__all_sync(0xFFFFFFFFu, digit == d0)) {
+                        if (lane == 0 && live) atomicAdd(&hist[digit], 32u);
+                    } else if (live) atomicAdd(&hist[digit], 1u);
                 }
             }
         } else
