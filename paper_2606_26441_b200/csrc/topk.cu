@@ -317,8 +317,10 @@ __global__ void __launch_bounds__(kRowThreads, 2) k_sel_row(gs_sel_src src, int3
                 // scores share their leading bits, so a digit's counter is hot: one atomic per distinct digit per warp
                 const bool live = key[u] != 0ull && (key[u] & himask) == prefix;
                 const uint32_t digit = live ? (uint32_t)((key[u] >> lo) & ((1u << width) - 1u)) : 0xFFFFFFFFu;
-                const unsigned peers = __match_any_sync(0xFFFFFFFFu, digit);
-                if (live && lane == __ffs(peers) - 1) atomicAdd(&hist[digit], (uint32_t)__popc(peers));
+                const uint32_t d0 = __shfl_sync(0xFFFFFFFFu, digit, 0);        // as in the dense passes above
+                if (__all_sync(0xFFFFFFFFu, digit == d0)) {
+                    if (lane == 0 && live) atomicAdd(&hist[digit], 32u);
+                } else if (live) atomicAdd(&hist[digit], 1u);
             }
         }
         cluster.sync();
