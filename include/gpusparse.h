@@ -248,6 +248,18 @@ GS_API gs_status_t gs_topk_dense(const void* scores, int32_t wtype, int64_t num_
                           int32_t k, int32_t* out_ids, void* out_scores, void* workspace,
                           size_t workspace_bytes, gs_stream_t stream);
 
+/* gs_topk_dense without a workspace argument and without any allocation, for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the select's scratch lives in a
+ * static device array of GS_TOPK_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it
+ * until the process exits).  Same arguments, results and errors as gs_topk_dense, plus: GS_ERR_OUT_OF_RANGE when the
+ * call's scratch need — gs_topk_workspace_bytes(num_rows, n, k) — exceeds GS_TOPK_STATIC_SCRATCH_BYTES (2.5 MiB: up to
+ * 64 rows at k = GS_MAX_K, 256 rows at k <= 64).  All calls share the array: calls that overlap on
+ * the GPU (different streams, or unordered threads) race; order them on one stream.  Asynchronous on `stream`; calls no
+ * cudaMalloc, cudaFree or allocating library routine. */
+#define GS_TOPK_STATIC_SCRATCH_BYTES 2624000   /* = gs_topk_workspace_bytes(64, n, 4096) */
+GS_API gs_status_t gs_topk_dense_static(const void* scores, int32_t wtype, int64_t num_rows, int64_t n, int64_t ld,
+                                 int32_t k, int32_t* out_ids, void* out_scores, gs_stream_t stream);
+
 /* Exact merge of partial top-k lists (document sharding; §6.7 L322-324 merges on
  * the host, L430 asks for a device-side merge).  `ids` [n_lists][B][k_in] int32 and `scores` [n_lists][B][k_in]
  * (float | int32 per wtype) are DEVICE arrays: list l holds, for every query, the top-k_in of shard l as returned by

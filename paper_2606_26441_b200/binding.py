@@ -25,7 +25,7 @@ EXPORTS = [
     "gs_index_build", "gs_index_info", "gs_index_free", "gs_index_copy_meta", "gs_index_copy_list",
     "gs_index_copy_head_terms",
     "gs_search_workspace_bytes", "gs_search", "gs_search_finish", "gs_search_host", "gs_search_stats", "gs_score_dense",
-    "gs_topk_workspace_bytes", "gs_topk_dense", "gs_merge_topk_workspace_bytes", "gs_merge_topk", "gs_strerror", "gs_version", "gs_abi_version",
+    "gs_topk_workspace_bytes", "gs_topk_dense", "gs_topk_dense_static", "gs_merge_topk_workspace_bytes", "gs_merge_topk", "gs_strerror", "gs_version", "gs_abi_version",
     "gs_last_cuda_error", "gs_last_launch_count", "gs_profile_enable", "gs_profile_read", "gs_kclass_name", "gs_dispatch_model",
 ]
 GS_PROF_CLASSES = 8
@@ -105,6 +105,7 @@ def lib():
         L.gs_score_dense.argtypes = [vp, P(gs_csr_t), P(gs_search_opts_t), vp, i64, vp, sz, vp]
         L.gs_topk_workspace_bytes.argtypes = [i64, i64, i32, P(sz)]
         L.gs_topk_dense.argtypes = [vp, i32, i64, i64, i64, i32, vp, vp, vp, sz, vp]
+        L.gs_topk_dense_static.argtypes = [vp, i32, i64, i64, i64, i32, vp, vp, vp]
         L.gs_merge_topk_workspace_bytes.argtypes = [i32, i64, i32, i32, P(sz)]
         L.gs_merge_topk.argtypes = [i32, i32, i64, i32, i32, vp, vp, P(i64), vp, vp, vp, sz, vp]
         L.gs_strerror.argtypes = [ctypes.c_int]
@@ -386,6 +387,27 @@ def topk_dense(scores, k: int, n: Optional[int] = None, stream=None):
     _check(lib().gs_topk_dense(scores.data_ptr(), wt, rows, n, ld, k, ids.data_ptr(), sc.data_ptr(), ws.data_ptr(),
                                ws.numel(), _stream_ptr(stream)))
     return ids, sc
+
+
+GS_TOPK_STATIC_SCRATCH_BYTES = 2624000
+
+
+def topk_dense_static(scores, k: int, out_ids, out_scores, n: Optional[int] = None, stream=None):
+    """gs_topk_dense_static: as topk_dense, but the library allocates nothing (scratch = a static device array of
+    GS_TOPK_STATIC_SCRATCH_BYTES shared by all calls) and neither does this wrapper: the caller passes the outputs
+    ``out_ids`` [rows, k] int32 and ``out_scores`` [rows, k] (dtype of ``scores``).  Raises GsError(2) beyond the maximum."""
+    torch = _torch()
+    assert scores.is_cuda and scores.dim() == 2 and scores.is_contiguous()
+    rows, ld = scores.shape
+    n = ld if n is None else n
+    wt = GS_W_F32 if scores.dtype == torch.float32 else GS_W_U8
+    if wt == GS_W_U8:
+        assert scores.dtype == torch.int32
+    assert out_ids.is_cuda and out_ids.dtype == torch.int32 and out_ids.shape == (rows, k) and out_ids.is_contiguous()
+    assert out_scores.is_cuda and out_scores.dtype == scores.dtype and out_scores.shape == (rows, k) and out_scores.is_contiguous()
+    _check(lib().gs_topk_dense_static(scores.data_ptr(), wt, rows, n, ld, k, out_ids.data_ptr(), out_scores.data_ptr(),
+                                      _stream_ptr(stream)))
+    return out_ids, out_scores
 
 
 def merge_topk(ids, scores, k_out: int, doc_bases=None, workspace=None, stream=None):

@@ -10,6 +10,7 @@
 #include <cooperative_groups.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "gs_internal.cuh"
 
@@ -524,4 +525,69 @@ gs_status_t gs_launch_select(const gs_sel_src& src, int64_t rows, int32_t k, int
     return src.wtype == GS_W_F32
                ? run_select<GS_W_F32>(src, rows, k, out_ids, out_scores, out_thr, out_keys, out_cnt, out_cap, scratch, s)
                : run_select<GS_W_U8>(src, rows, k, out_ids, out_scores, out_thr, out_keys, out_cnt, out_cap, scratch, s);
+}
+
+// ------------------------------------------------------------------------------------------------
+// gs_topk_dense_static: gs_topk_dense for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that
+// forbid cudaMalloc) — the select's scratch (per-row state, digit histograms, selected keys: what gs_topk_dense takes as
+// `workspace`) lives in a file-scope device array instead.  Every GPU that loads the library holds the array until the
+// process exits, so it is modest: GS_TOPK_STATIC_SCRATCH_BYTES.
+//
+// In host code the array's NAME is a host-side stand-in, not a device address (a kernel handed it would fault or, where the
+// GPU can reach host memory, silently use the wrong memory): the device address comes from cudaGetSymbolAddress, asked once
+// per device with that device current and kept.  All calls share the array and it keeps the last call's contents: the first
+// launch of every call (k_sel_init) re-initialises the state and the histograms of the rows in use, and the selected-key
+// region is only read where this call wrote it, so nothing has to be cleared by the caller — but two calls that overlap on
+// the GPU (different streams, or the same stream from two threads without ordering) race on it.
+// Calls no cudaMalloc / cudaFree / allocating library routine.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_topk_static_scratch[GS_TOPK_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kMaxDevices] = {};      // device address of g_topk_static_scratch, per device
+
+gs_status_t static_scratch(void** out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return GS_ERR_UNSUPPORTED_DEVICE; }
+    if (dev < 0 || dev >= kMaxDevices) return GS_ERR_UNSUPPORTED_DEVICE;
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return GS_ERR_UNSUPPORTED_DEVICE; }
+    if (major != 10) return GS_ERR_UNSUPPORTED_DEVICE;          // the library holds sm_100a code only
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (g_static_ptr[dev] == nullptr) {
+        void* ptr = nullptr;
+        GS_CUDA(cudaGetSymbolAddress(&ptr, g_topk_static_scratch));   // device `dev` is current
+        if (ptr == nullptr) return GS_ERR_CUDA;
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return GS_OK;
+}
+
+bool on_device(const void* p) {
+    if (!p) return false;
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+}  // namespace
+
+extern "C" GS_API gs_status_t gs_topk_dense_static(const void* scores, int32_t wtype, int64_t rows, int64_t n, int64_t ld, int32_t k,
+                                                   int32_t* out_ids, void* out_scores, gs_stream_t stream) {
+    if (!out_ids || !out_scores || rows < 0 || n < 0 || ld < n) return GS_ERR_INVALID_ARG;
+    if (wtype != GS_W_F32 && wtype != GS_W_U8) return GS_ERR_INVALID_ARG;
+    if (k < 1 || k > GS_MAX_K) return GS_ERR_OUT_OF_RANGE;
+    if (rows > 65535 || n >= 0x7FFFFFFFLL) return GS_ERR_OUT_OF_RANGE;
+    // the maximum: the call's scratch need must fit the static array
+    if (gs_select_scratch_bytes(rows, k) > (size_t)GS_TOPK_STATIC_SCRATCH_BYTES) return GS_ERR_OUT_OF_RANGE;
+    void* scratch = nullptr;
+    GS_TRY(static_scratch(&scratch));
+    if (n > 0 && rows > 0 && !on_device(scores)) return GS_ERR_INVALID_ARG;
+    if (!on_device(out_ids) || !on_device(out_scores)) return GS_ERR_INVALID_ARG;
+    gs_tls_launches = 0;
+    gs_sel_src src{};
+    src.dense = (const uint32_t*)scores; src.ld = ld; src.n_cols = n; src.n_docs = n; src.Ts = 0; src.wtype = wtype;
+    return gs_launch_select(src, rows, k, out_ids, out_scores, nullptr, nullptr, nullptr, 0, scratch, (cudaStream_t)stream);
 }
