@@ -126,7 +126,7 @@ typedef struct gs_info {
 #define GS_FLAG_VALIDATE_QUERIES 1u   /* check query ids/dups/finite on device, synchronise, return the error   */
 #define GS_FLAG_FORCE_DENSE_TOPK 2u   /* materialise every score tile and select from it (no threshold filter) */
 #define GS_FLAG_NO_HEAD_STRIPS 4u     /* term-parallel: send every list through the scatter path               */
-#define GS_FLAG_TENSOR_CORE_HEAD 8u   /* integer-impact mode, batches of >= 64 queries, 512-doc tiles: contract the dense strips  */
+#define GS_FLAG_TENSOR_CORE_HEAD 8u   /* integer-impact mode, batches of >= 32 queries, 512-doc tiles: contract the dense strips  */
                                       /* with tcgen05.mma kind::i8 (uint8 x uint8 -> int32 is exact: k_score_term_mma) instead of  */
                                       /* IDP4A on the CUDA cores.  Bit-identical results; measured slower on B200 (16.2 vs 13.9 ms */
                                       /* per 500-query batch at 8.8M docs: the tail scatter dominates), so opt-in.   */

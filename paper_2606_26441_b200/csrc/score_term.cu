@@ -1346,13 +1346,16 @@ gs_status_t launch(const TermParams& p, unsigned grid, size_t smem, bool staged,
 // batch kernel): 8.8M docs 48: 3.03 / 3.19, 64: 3.89 / 3.37, 128: 7.25 / 5.51, 256: 13.7 / 9.49, 500: 25.9 / 16.6;
 // 1M docs 64: 0.61 / 0.62, 96: 0.84 / 0.88, 128: 1.04 / 0.98, 256: 1.87 / 1.53, 500: 3.41 / 2.59 — the fixed cost of a CTA
 // (staging, first-row probes) is amortised over fewer rows when the collection has few doc tiles.
-constexpr int kStagedMinQueries = 128;
-constexpr int kStagedMinQueriesLarge = 64;     // collections of >= kLargeTiles doc tiles
-constexpr int kLargeTiles = 8192;
+// batches of at least this many queries take the batch / staged kernels (one CTA of 32 warps per doc tile and query chunk);
+// measured on B200 after the round-2 cuts of the batch kernel: it wins from one query per warp on, on every collection
+// size (8.8M docs: B = 32 1.94 -> 1.77 ms, config 5 B = 32 9.60 -> 8.63 ms; 1M docs B = 64 0.476 -> 0.442 ms), and loses
+// below (B = 24: 1.45 vs 1.67 ms)
+constexpr int kStagedMinQueries = 32;
 constexpr int kStagedChunk = 512;         // most queries per CTA of the staged / batch kernels
 constexpr int kChunkWaves = 16;   // CTAs per SM a launch aims for before it stops splitting the queries
 static inline bool cta_per_tile(const gs_index* ix, int64_t nq) {
-    return nq >= (ix->ntiles >= kLargeTiles ? kStagedMinQueriesLarge : kStagedMinQueries);
+    (void)ix;
+    return nq >= kStagedMinQueries;
 }
 
 }  // namespace
