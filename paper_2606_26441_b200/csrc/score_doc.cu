@@ -36,7 +36,21 @@
 
 #include "gs_internal.cuh"
 
-#define GS_DOC_PF 2      // chunks of the posting stream in flight per warp (1: 62.3 %, 2: 62.8 % of the copy bandwidth)
+#ifndef GS_DOC_SG
+#define GS_DOC_SG 4      // strip values in flight per thread in the fp32 strip contraction
+#endif
+#ifndef GS_DOC_PF
+#define GS_DOC_PF 1      // chunks of the posting stream in flight per warp ahead of the one being filtered
+#endif
+#ifndef GS_DOC_PFSKIP
+#define GS_DOC_PFSKIP 4
+#endif
+#ifndef GS_DOC_PFDIST
+#define GS_DOC_PFDIST 4
+#endif
+#ifndef GS_DOC_L2PF
+#define GS_DOC_L2PF 24   // L2 prefetch of the next block: 1 = its strip segments, 2 = its posting range
+#endif
 
 namespace {
 
@@ -53,6 +67,7 @@ struct ConstTile {
     uint32_t pair_off;                   // ... and of the shared pairs array
     uint32_t pad[3];
     uint32_t hl[GS_STRIP_MAX];           // compact position -> strip number (0 beyond nh)
+    unsigned long long soff[GS_STRIP_MAX]; // ... and the byte offset of that strip's row in the strip array (hl * N_pad * sizeof(W))
     uint32_t thr_s[kMaxQT];              // threshold as a score (accumulator bits); "accept all" = NaN / INT32_MIN
     unsigned long long thr_key[kMaxQT];  // threshold as a key; queries beyond the tile: all ones
     uint32_t qh[GS_STRIP_MAX * kMaxQT];  // f32: [compact strip][QT] head weights, row stride QT; u8: [strip / 4][QT] words of
@@ -131,7 +146,8 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                                                       const void* __restrict__ weights, const int16_t* __restrict__ head_slot,
                                                       int H, int64_t q0, int64_t nq, int QT, int32_t V, int Wd,
                                                       const uint64_t* __restrict__ thr, unsigned char* __restrict__ scratch,
-                                                      int64_t n_passes, int64_t nnz_cap, const int32_t* __restrict__ status) {
+                                                      int64_t n_passes, int64_t nnz_cap, const int32_t* __restrict__ status,
+                                                      int64_t strip_row_bytes) {
     extern __shared__ uint32_t sm[];                  // bitmap[Wd], prefix[Wd]
     if (*status != 0) return;                         // ingest found a malformed batch (e.g. a non-monotone indptr): nothing is read
     __shared__ uint32_t warp_tot[32];
@@ -183,9 +199,12 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
     if (threadIdx.x == 0) {   // compact list of the strips some query of the tile uses, padded to a multiple of 4
         uint32_t n = 0;
         for (int h = 0; h < H; ++h)
-            if ((s_hmask[h >> 5] >> (h & 31)) & 1u) ct->hl[n++] = (uint32_t)h;
+            if ((s_hmask[h >> 5] >> (h & 31)) & 1u) {
+                ct->soff[n] = (unsigned long long)h * (unsigned long long)strip_row_bytes;
+                ct->hl[n++] = (uint32_t)h;
+            }
         const uint32_t n8 = WT == GS_W_F32 ? ((n + 3u) & ~3u) : ((n + 7u) & ~7u);      // strips per turn of strips_phase
-        for (uint32_t i = n; i < GS_STRIP_MAX; ++i) ct->hl[i] = 0u;      // padding rows carry zero weights
+        for (uint32_t i = n; i < GS_STRIP_MAX; ++i) { ct->hl[i] = 0u; ct->soff[i] = 0ull; }      // padding rows carry zero weights
         ct->nh = n8;
         ct->R = R;
         ct->row_off = row_off;
@@ -281,7 +300,7 @@ template <int QT> struct Geo {
     // stand-in) should fit, because a walk over part of a block leaves the lanes of the other documents idle
     static constexpr int QCAP = QT <= 8 ? 640 : (QT == 16 ? 512 : (QT == 32 ? 768 : 1152));
     static constexpr size_t per_warp = (size_t)QCAP * 8 + (size_t)32 * AST * 4;
-    static __host__ __device__ size_t fixed(int Wd) { return (size_t)Wd * 8; }
+    static __host__ __device__ size_t fixed(int Wd) { return (size_t)Wd * 8 + (size_t)GS_STRIP_MAX * 8; }   // bitmap, prefix, strip offsets
 };
 
 __device__ __forceinline__ uint4 ld_stream4(const uint4* p) { return __ldcs(p); }
@@ -300,8 +319,16 @@ __device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, fl
     return d;
 }
 
+#ifndef GS_DOC_INLINE_STRIPS
+#define GS_DOC_INLINE_STRIPS 1
+#endif
+#if GS_DOC_INLINE_STRIPS
+#define GS_STRIPS_ATTR __forceinline__
+#else
+#define GS_STRIPS_ATTR __noinline__
+#endif
 template <int WT, int QT>
-__device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ myacc,
+__device__ GS_STRIPS_ATTR void strips_phase(typename NumD<WT>::A* __restrict__ myacc,
                                           const typename NumD<WT>::W* __restrict__ sp, int64_t N_pad) {
     using A = typename NumD<WT>::A;
     const int nh = (int)c_tile.nh;
@@ -311,29 +338,65 @@ __device__ __noinline__ void strips_phase(typename NumD<WT>::A* __restrict__ mya
 #pragma unroll
         for (int q = 0; q < QT / 2; ++q)
             asm("mov.b64 %0, {%1, %2};" : "=l"(acc[q]) : "f"(myacc[2 * q]), "f"(myacc[2 * q + 1]));
-        // The strip values of the next kSG strips are loaded before the multiply-adds of the current ones: a strip value is
-        // one DRAM round trip per block of 32 documents, and with 4 in flight that wait is 20 % of the kernel's stall
-        // samples (profiles/r02_kernels.md).  c_tile.hl is padded with valid strip numbers up to a multiple of kSG.
-        constexpr int kSG = 4;
-        float xn[kSG];
+        if constexpr (QT <= 16) {
+            // Fully unrolled over the (at most GS_STRIP_MAX) compact strips with early exits on nh: every weight offset is a
+            // compile-time constant, so the weights arrive by LDCU.128 (four weights = two FFMA2 per uniform load; with a
+            // runtime strip index the compiler issued one LDCU.64 per FFMA2) and a strip's address is base + a 64-bit byte
+            // offset from the constant tile (no multiply).  Two register groups of kSG strip values alternate: the values of
+            // the next group are loaded before the multiply-adds of the current one (a strip value is one DRAM / L2 round
+            // trip per block of 32 documents).  c_tile.soff is padded with offset 0 (a valid row, zero weights).
+            constexpr int kSG = GS_DOC_SG;
+            const char* spb = reinterpret_cast<const char*>(sp);
+            float xa[kSG], xb[kSG];
+            auto ldx = [&](float (&x)[kSG], int i0) {
 #pragma unroll
-        for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[u] * N_pad];
-#pragma unroll 1
-        for (int i0 = 0; i0 < nh; i0 += kSG) {
-            float x[kSG];
+                for (int u = 0; u < kSG; ++u) x[u] = *reinterpret_cast<const float*>(spb + c_tile.soff[i0 + u]);
+            };
+            auto mac = [&](const float (&x)[kSG], int i0) {
 #pragma unroll
-            for (int u = 0; u < kSG; ++u) x[u] = xn[u];
-            if (i0 + kSG < nh) {
+                for (int u = 0; u < kSG; ++u) {
 #pragma unroll
-                for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[i0 + kSG + u] * N_pad];
+                    for (int q = 0; q < QT; q += 2) {
+                        const unsigned long long v = *reinterpret_cast<const unsigned long long*>(&c_tile.qh[(i0 + u) * QT + q]);
+                        acc[q / 2] = fma_f32x2(v, x[u], acc[q / 2]);
+                    }
+                }
+            };
+            ldx(xa, 0);
+#pragma unroll
+            for (int i0 = 0; i0 < GS_STRIP_MAX; i0 += 2 * kSG) {
+                if (i0 >= nh) break;
+                if (i0 + kSG < nh) ldx(xb, i0 + kSG);
+                mac(xa, i0);
+                if (i0 + kSG >= nh) break;
+                if (i0 + 2 * kSG < GS_STRIP_MAX && i0 + 2 * kSG < nh) ldx(xa, i0 + 2 * kSG);
+                mac(xb, i0 + kSG);
             }
+        } else {
+            // The strip values of the next kSG strips are loaded before the multiply-adds of the current ones: a strip value is
+            // one DRAM round trip per block of 32 documents, and with 4 in flight that wait is 20 % of the kernel's stall
+            // samples (profiles/r02_kernels.md).  c_tile.hl is padded with valid strip numbers up to a multiple of kSG.
+            constexpr int kSG = 4;
+            float xn[kSG];
 #pragma unroll
-            for (int u = 0; u < kSG; ++u) {
+            for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[u] * N_pad];
+#pragma unroll 1
+            for (int i0 = 0; i0 < nh; i0 += kSG) {
+                float x[kSG];
 #pragma unroll
-                for (int q = 0; q < QT; q += 4) {
-                    const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(&c_tile.qh[(i0 + u) * QT + q]);
-                    acc[q / 2] = fma_f32x2(v.x, x[u], acc[q / 2]);
-                    acc[q / 2 + 1] = fma_f32x2(v.y, x[u], acc[q / 2 + 1]);
+                for (int u = 0; u < kSG; ++u) x[u] = xn[u];
+                if (i0 + kSG < nh) {
+#pragma unroll
+                    for (int u = 0; u < kSG; ++u) xn[u] = sp[(size_t)c_tile.hl[i0 + kSG + u] * N_pad];
+                }
+#pragma unroll
+                for (int u = 0; u < kSG; ++u) {
+#pragma unroll
+                    for (int q = 0; q < QT; q += 4) {
+                        const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(&c_tile.qh[(i0 + u) * QT + q]);
+                        acc[q / 2] = fma_f32x2(v.x, x[u], acc[q / 2]);
+                        acc[q / 2 + 1] = fma_f32x2(v.y, x[u], acc[q / 2 + 1]);
+                    }
                 }
             }
         }
@@ -390,7 +453,8 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
 
     uint32_t* s_bm = reinterpret_cast<uint32_t*>(smem);                           // [Wd]
     uint32_t* s_pre = s_bm + Wd;                                                  // [Wd]
-    unsigned char* pw = reinterpret_cast<unsigned char*>(s_pre + Wd);
+    unsigned long long* s_soff = reinterpret_cast<unsigned long long*>(s_pre + Wd);   // [GS_STRIP_MAX] copy of c_tile.soff (lane-indexed reads)
+    unsigned char* pw = reinterpret_cast<unsigned char*>(s_soff + GS_STRIP_MAX);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint2* queue = reinterpret_cast<uint2*>(pw + (size_t)warp * G::per_warp);     // [QCAP]
     A* s_acc = reinterpret_cast<A*>(queue + QCAP);                                // [32][AST]
@@ -400,6 +464,7 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     const bool filter = p.sink.thr != nullptr;
     {   // stage the query tile
         for (int i = threadIdx.x; i < 2 * Wd; i += NW * 32) s_bm[i] = p.tile_bm[i];   // bitmap and prefix are adjacent
+        if (threadIdx.x < GS_STRIP_MAX) s_soff[threadIdx.x] = c_tile.soff[threadIdx.x];
         if (sparse_in_smem) {
             for (uint32_t i = threadIdx.x; i < np; i += NW * 32) s_pairs[i] = g_pairs[i];
             for (uint32_t i = threadIdx.x; i < R; i += NW * 32) s_rows[i] = g_rows[i];
@@ -417,8 +482,10 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     const unsigned lt = (1u << lane) - 1u;
     A* myacc = s_acc + lane * AST;
     const int subs_per_tile = p.Ts >> 5;
-    const int64_t n_subs = (int64_t)p.ts.count * subs_per_tile;
-    const int64_t sb_stride = (int64_t)gridDim.x * NW;
+    // 32-bit block, chunk and document numbers in the loop state (the launcher checks the ranges): registers are what
+    // limits the loads in flight here
+    const int n_subs = (int)(p.ts.count * subs_per_tile);
+    const int sb_stride = (int)gridDim.x * NW;
 
     // lane d applies the queued hits of document d (contiguous: the queue is in stream order); one loop over (hit, pair)
     auto walk = [&](int n) {
@@ -453,71 +520,127 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     };
 
     // block -> (start, chunks) of its posting range, or nothing beyond the collection
-    auto block_of = [&](int64_t sb, int64_t& doc0) -> int64_t {
+    auto block_of = [&](int sb, int& doc0) -> int {
         const int64_t tile = p.ts.first + (sb / subs_per_tile) * (int64_t)p.ts.stride;
-        doc0 = tile * p.Ts + (sb % subs_per_tile) * 32;
-        return doc0 < p.N ? (doc0 >> 5) : -1;
+        const int64_t d = tile * p.Ts + (sb % subs_per_tile) * 32;
+        doc0 = (int)d;
+        return d < p.N ? (int)(d >> 5) : -1;
     };
     const uint32_t* __restrict__ wp1 = reinterpret_cast<const uint32_t*>(p.fwd_w);     // u8: 4 weights per word
     const uint4* __restrict__ wp4 = reinterpret_cast<const uint4*>(p.fwd_w);           // f32
     const uint4* __restrict__ tp4 = reinterpret_cast<const uint4*>(p.fwd_terms);
     // chunk c (128 postings) of the index: lane holds postings 4*lane .. 4*lane+3
-    auto load_chunk = [&](int64_t chunk, uint4& t4, uint4& w4) {
-        t4 = ld_stream4(tp4 + chunk * 32 + lane);
+    auto load_chunk = [&](int chunk, uint4& t4, uint4& w4) {
+        t4 = ld_stream4(tp4 + (size_t)(uint32_t)chunk * 32 + lane);
         if (WT == GS_W_F32) {
-            w4 = ld_stream4(wp4 + chunk * 32 + lane);
+            w4 = ld_stream4(wp4 + (size_t)(uint32_t)chunk * 32 + lane);
         } else if (p.fwd_packed) {                 // compressed postings: term | impact << 19 | (doc & 31) << 27
             w4 = make_uint4((t4.x >> 19) & 0xFFu, (t4.y >> 19) & 0xFFu, (t4.z >> 19) & 0xFFu, (t4.w >> 19) & 0xFFu);
             t4 = make_uint4(t4.x & 0xF807FFFFu, t4.y & 0xF807FFFFu, t4.z & 0xF807FFFFu, t4.w & 0xF807FFFFu);
         } else {
-            const uint32_t v = ld_stream1(wp1 + chunk * 32 + lane);
+            const uint32_t v = ld_stream1(wp1 + (size_t)(uint32_t)chunk * 32 + lane);
             w4 = make_uint4(v & 0xFFu, (v >> 8) & 0xFFu, (v >> 16) & 0xFFu, v >> 24);
         }
     };
-
-    int64_t sb = (int64_t)blockIdx.x * NW + warp;
-    int64_t doc0 = 0, c0 = 0, c1 = 0;              // chunk range of the current block
-    uint4 tc = make_uint4(0, 0, 0, 0), wc = tc;      // chunk c of the current block
-#if GS_DOC_PF >= 2
-    uint4 td = tc, wd = tc;                          // chunk c + 1
-#endif
-    if (sb < n_subs) {
-        const int64_t blk = block_of(sb, doc0);
-        if (blk >= 0) {
-            c0 = p.fwd_blk[blk] / GS_FWD_CHUNK;
-            c1 = p.fwd_blk[blk + 1] / GS_FWD_CHUNK;
-            if (c0 < c1) load_chunk(c0, tc, wc);
-#if GS_DOC_PF >= 2
-            if (c0 + 1 < c1) load_chunk(c0 + 1, td, wd);
-#endif
-        } else {
-            c0 = c1 = -1;
+    // block -> first chunk and number of chunks of its posting range (c0 < 0: block beyond the collection)
+    auto range_of = [&](int sbx, int& d0, int& cc0, int& ncc) {
+        cc0 = -1; ncc = 0; d0 = 0;
+        if (sbx >= n_subs) return;
+        const int blk = block_of(sbx, d0);
+        if (blk < 0) return;
+        cc0 = (int)(p.fwd_blk[blk] / GS_FWD_CHUNK);
+        ncc = (int)(p.fwd_blk[blk + 1] / GS_FWD_CHUNK) - cc0;
+    };
+    // L2 prefetch of what the warp reads one block later (no registers, no shared memory: the lines wait in the L2):
+    // the 128-byte strip segments of the next block's documents, one line per lane and turn, and the next block's
+    // posting range as bulk prefetches issued by two lanes.  The loads themselves then find their lines in the L2.
+    auto prefetch_block = [&](int d0, int cc0, int ncc) {
+#if GS_DOC_L2PF & 4
+        {   // the first chunks of the next block only (the start of its stream)
+            const int n4 = min(ncc, GS_DOC_PFSKIP);
+            if (n4 > 0) {
+                if (lane == 0)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)cc0 * 32), "r"(n4 * 512) : "memory");
+                if (WT == GS_W_F32 && lane == 1)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)cc0 * 32), "r"(n4 * 512) : "memory");
+            }
         }
-    }
+#endif
+#if GS_DOC_L2PF & 2
+        if (ncc > 0) {
+            if (lane == 0)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 512) : "memory");
+            if (WT == GS_W_F32) {
+                if (lane == 1)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 512) : "memory");
+            } else if (!p.fwd_packed) {
+                if (lane == 1)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp1 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 128) : "memory");
+            }
+        }
+#endif
+    };
+
+    int sb = (int)blockIdx.x * NW + warp;
+    int doc0 = 0, c0 = -1;                           // first document and first chunk of the current block
+    int nc = 0;                                      // its chunks
+    // three chunk buffers: chunk i of a block lives in buffer i % 3 while it is in flight / being filtered (the chunk loop
+    // is unrolled by three so that no buffer is ever copied to another: the rotation by register moves was a quarter of
+    // the loop's instructions)
+    uint4 tA = make_uint4(0, 0, 0, 0), wA = tA, tB = tA, wB = tA;
+#if GS_DOC_PF >= 2
+    uint4 tC = tA, wC = tA;
+#endif
+    range_of(sb, doc0, c0, nc);
+    if (nc > 0) load_chunk(c0, tA, wA);
+    if (GS_DOC_PF >= 2 && nc > 1) load_chunk(c0 + 1, tB, wB);
     for (; sb < n_subs; sb += sb_stride) {
         // the next block's range, asked for now, needed after the walk
-        const int64_t sbn = sb + sb_stride;
-        int64_t doc0n = 0, blkn = -1, c0n = -1, c1n = -1;
-        if (sbn < n_subs) blkn = block_of(sbn, doc0n);
-        if (blkn >= 0) { c0n = p.fwd_blk[blkn] / GS_FWD_CHUNK; c1n = p.fwd_blk[blkn + 1] / GS_FWD_CHUNK; }
+        int doc0n, c0n, ncn;
+        range_of(sb + sb_stride, doc0n, c0n, ncn);
         if (c0 < 0) {                              // block beyond the collection
-            doc0 = doc0n; c0 = c0n; c1 = c1n;
-            if (c0 >= 0 && c0 < c1) load_chunk(c0, tc, wc);
-#if GS_DOC_PF >= 2
-            if (c0 >= 0 && c0 + 1 < c1) load_chunk(c0 + 1, td, wd);
-#endif
+            doc0 = doc0n; c0 = c0n; nc = ncn;
+            if (nc > 0) load_chunk(c0, tA, wA);
+            if (GS_DOC_PF >= 2 && nc > 1) load_chunk(c0 + 1, tB, wB);
             continue;
         }
+        if (c0n >= 0) prefetch_block(doc0n, c0n, ncn);
+        // the 128-byte strip segments of this block's documents, one line per lane and turn, into the L2 (no registers, no
+        // shared memory): asked for now, read after the walk.  Not a whole block earlier: in one block's time the stream
+        // turns the whole L2 over, and the lines were gone again (1.9 GB of re-reads per pass, measured)
+        auto prefetch_strips = [&]() {
+            for (int i = lane; i < nh; i += 32)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(strips + doc0) + s_soff[i]));
+        };
+#if GS_DOC_L2PF & 1
+        prefetch_strips();
+#endif
+#if GS_DOC_L2PF & 4
+        if (nc > GS_DOC_PFSKIP) {                 // the rest of this block's stream
+            if (lane == 2)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)(c0 + GS_DOC_PFSKIP) * 32), "r"((nc - GS_DOC_PFSKIP) * 512) : "memory");
+            if (WT == GS_W_F32 && lane == 3)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)(c0 + GS_DOC_PFSKIP) * 32), "r"((nc - GS_DOC_PFSKIP) * 512) : "memory");
+        }
+#endif
+#if GS_DOC_L2PF & 8
+        // rolling L2 prefetch of the posting stream: lanes 0..3 ask for the four 128-byte lines of the terms of the chunk
+        // GS_DOC_PFDIST ahead, lanes 4..7 for its fp32 weights
+        const char* pfb;
+        if constexpr (WT == GS_W_F32)
+            pfb = (lane < 4 ? reinterpret_cast<const char*>(tp4) : reinterpret_cast<const char*>(wp4)) + (lane & 3) * 128;
+        else
+            pfb = reinterpret_cast<const char*>(tp4) + (lane & 3) * 128;      // byte weights: the terms only (a fifth of the bytes)
+        constexpr int pf_lanes = WT == GS_W_F32 ? 8 : 4;
+#endif
         for (int i = lane; i < 32 * AST; i += 32) s_acc[i] = A(0);
 
         // ---- tail: the block's postings as one flat range -> bitmap filter -> hit queue -> per-document walk
         int cnt = 0;
-        for (int64_t c = c0; c < c1; ++c) {
-            uint4 tn = make_uint4(0, 0, 0, 0), wn = tn;
-#if GS_DOC_PF >= 2
-            if (c + 2 < c1) load_chunk(c + 2, tn, wn);                       // prefetch, two chunks ahead
-#else
-            if (c + 1 < c1) load_chunk(c + 1, tn, wn);                       // prefetch
+        auto filter_chunk = [&](const uint4& tc, const uint4& wc, int i) {
+#if GS_DOC_L2PF & 8
+            if (lane < pf_lanes && i + GS_DOC_PFDIST < nc)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(pfb + (size_t)(uint32_t)(c0 + i + GS_DOC_PFDIST) * 512));
 #endif
             if (cnt + GS_FWD_CHUNK > QCAP) { walk(cnt); cnt = 0; }
             const uint32_t tw[4] = {tc.x, tc.y, tc.z, tc.w};
@@ -537,21 +660,44 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
                 }
                 cnt += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
+        };
 #if GS_DOC_PF >= 2
-            tc = td; wc = wd; td = tn; wd = wn;
-#else
-            tc = tn; wc = wn;
-#endif
+        for (int i = 0;;) {                          // two chunks in flight ahead of the one being filtered
+            if (i >= nc) break;
+            if (i + 2 < nc) load_chunk(c0 + i + 2, tC, wC);
+            filter_chunk(tA, wA, i);
+            ++i;
+            if (i >= nc) break;
+            if (i + 2 < nc) load_chunk(c0 + i + 2, tA, wA);
+            filter_chunk(tB, wB, i);
+            ++i;
+            if (i >= nc) break;
+            if (i + 2 < nc) load_chunk(c0 + i + 2, tB, wB);
+            filter_chunk(tC, wC, i);
+            ++i;
         }
-        walk(cnt);
-        // first chunk(s) of the next block: in flight during the contraction
-        if (c0n >= 0 && c0n < c1n) load_chunk(c0n, tc, wc);
-#if GS_DOC_PF >= 2
-        if (c0n >= 0 && c0n + 1 < c1n) load_chunk(c0n + 1, td, wd);
+#else
+        for (int i = 0;;) {                          // one chunk in flight ahead of the one being filtered
+            if (i >= nc) break;
+            if (i + 1 < nc) load_chunk(c0 + i + 1, tB, wB);
+            filter_chunk(tA, wA, i);
+            ++i;
+            if (i >= nc) break;
+            if (i + 1 < nc) load_chunk(c0 + i + 1, tA, wA);
+            filter_chunk(tB, wB, i);
+            ++i;
+        }
 #endif
+#if GS_DOC_L2PF & 16
+        prefetch_strips();
+#endif
+        walk(cnt);
+        // first chunks of the next block: in flight during the contraction
+        if (ncn > 0) load_chunk(c0n, tA, wA);
+        if (GS_DOC_PF >= 2 && ncn > 1) load_chunk(c0n + 1, tB, wB);
 
         // ---- head strips: thread = document, QT accumulators in registers, weights as uniform constant operands
-        const int64_t doc = doc0 + lane;
+        const int64_t doc = (int64_t)doc0 + lane;
         if (nh > 0) strips_phase<WT, QT>(myacc, strips + doc, p.N_pad);
         A acc[QT];
 #pragma unroll
@@ -560,7 +706,7 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         // ---- sink: this thread owns the cells (qa + q, doc)
         if (doc < p.N) {
             if (!filter) {
-                uint32_t* out = p.sink.dense + p.q_rel * p.sink.ld + sb * 32 + lane;
+                uint32_t* out = p.sink.dense + p.q_rel * p.sink.ld + (int64_t)sb * 32 + lane;
 #pragma unroll
                 for (int q = 0; q < QT; ++q)
                     if (q < p.nqt) out[(int64_t)q * p.sink.ld] = NumD<WT>::bits(acc[q]);
@@ -579,7 +725,7 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
             }
         }
         __syncwarp();
-        doc0 = doc0n; c0 = c0n; c1 = c1n;
+        doc0 = doc0n; c0 = c0n; nc = ncn;
     }
     };
     if (sparse_in_smem) run(std::true_type{}); else run(std::false_type{});
@@ -676,11 +822,13 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
         if (ix->wtype == GS_W_F32) {
             GS_CUDA(gs_optin_smem(k_build_qtile<GS_W_F32>));
             k_build_qtile<GS_W_F32><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                              QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status);
+                                                              QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status,
+                                                              (int64_t)ix->N_pad * 4);
         } else {
             GS_CUDA(gs_optin_smem(k_build_qtile<GS_W_U8>));
             k_build_qtile<GS_W_U8><<<n_passes, 1024, bsm, s>>>(q->indptr, q->term_ids, q->weights, ix->head_slot, ix->H, q0, nq,
-                                                             QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status);
+                                                             QT, ix->V, Wd, sink.thr, (unsigned char*)scratch, passes_cap, q->nnz, qb.status,
+                                                             (int64_t)ix->N_pad);
         }
         ++gs_tls_launches;
         GS_CUDA(cudaGetLastError());
@@ -693,6 +841,8 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
     p.rows = ss.rows; p.pairs = ss.pairs;
     p.ts = ts; p.sink = sink; p.status = qb.status;
     const int64_t n_subs = (int64_t)ts.count * (ix->Ts / 32);
+    // the kernel keeps block, chunk and document numbers in 32 bits
+    if (n_subs >= (1LL << 31) - (1LL << 20) || ix->N >= (1LL << 31) - 64 || ix->P_fwd / GS_FWD_CHUNK >= (1LL << 31) - 8) return GS_ERR_OUT_OF_RANGE;
     return ix->wtype == GS_W_F32
                ? launch_doc_qt<GS_W_F32>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s)
                : launch_doc_qt<GS_W_U8>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
