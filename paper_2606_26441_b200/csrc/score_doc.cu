@@ -36,26 +36,12 @@
 
 #include "gs_internal.cuh"
 
-#ifndef GS_DOC_SG
-#define GS_DOC_SG 4      // strip values in flight per thread in the fp32 strip contraction
-#endif
-#ifndef GS_DOC_PF
-#define GS_DOC_PF 1      // chunks of the posting stream in flight per warp ahead of the one being filtered
-#endif
-#ifndef GS_DOC_PFSKIP
-#define GS_DOC_PFSKIP 4
-#endif
-#ifndef GS_DOC_PFDIST
-#define GS_DOC_PFDIST 4
-#endif
-#ifndef GS_DOC_L2PF
-#define GS_DOC_L2PF 24   // L2 prefetch of the next block: 1 = its strip segments, 2 = its posting range
-#endif
 
 namespace {
 
 constexpr uint32_t kTermMask = (1u << GS_FWD_DOC_SHIFT) - 1u;
 constexpr int kMaxQT = 64;
+constexpr int kPfDist = 4;   // rolling L2 prefetch of the posting stream: chunks ahead (3, 4, 6 measured alike; 8 and 12 slower)
 
 // What a pass needs with warp-uniform access.  Built in the search workspace by k_build_qtile, copied to
 // c_tile before the pass's launch (stream ordered).  qh is last: a pass copies only its [GS_STRIP_MAX][QT] prefix.
@@ -319,16 +305,8 @@ __device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, fl
     return d;
 }
 
-#ifndef GS_DOC_INLINE_STRIPS
-#define GS_DOC_INLINE_STRIPS 1
-#endif
-#if GS_DOC_INLINE_STRIPS
-#define GS_STRIPS_ATTR __forceinline__
-#else
-#define GS_STRIPS_ATTR __noinline__
-#endif
 template <int WT, int QT>
-__device__ GS_STRIPS_ATTR void strips_phase(typename NumD<WT>::A* __restrict__ myacc,
+__device__ __forceinline__ void strips_body(typename NumD<WT>::A* __restrict__ myacc,
                                           const typename NumD<WT>::W* __restrict__ sp, int64_t N_pad) {
     using A = typename NumD<WT>::A;
     const int nh = (int)c_tile.nh;
@@ -345,7 +323,7 @@ __device__ GS_STRIPS_ATTR void strips_phase(typename NumD<WT>::A* __restrict__ m
             // offset from the constant tile (no multiply).  Two register groups of kSG strip values alternate: the values of
             // the next group are loaded before the multiply-adds of the current one (a strip value is one DRAM / L2 round
             // trip per block of 32 documents).  c_tile.soff is padded with offset 0 (a valid row, zero weights).
-            constexpr int kSG = GS_DOC_SG;
+            constexpr int kSG = 4;
             const char* spb = reinterpret_cast<const char*>(sp);
             float xa[kSG], xb[kSG];
             auto ldx = [&](float (&x)[kSG], int i0) {
@@ -412,28 +390,72 @@ __device__ GS_STRIPS_ATTR void strips_phase(typename NumD<WT>::A* __restrict__ m
 #pragma unroll
         for (int q = 0; q < QT; ++q) acc[q] = myacc[q];
         // integer impacts: the document's bytes of four strips packed into one word, the tile's weights of the same four
-        // strips packed per query (k_build_qtile): one IDP4A per (four strips, query)
-        // the bytes of the next 8 strips are loaded before the IDP4As of the current ones (see the fp32 branch)
-        uint32_t xn[8];
+        // strips packed per query (k_build_qtile): one IDP4A per (four strips, query); the bytes of the next 8 strips are
+        // loaded before the IDP4As of the current ones
+        if constexpr (QT <= 16) {
+            // unrolled like the fp32 branch: constant offsets, strip addresses from c_tile.soff, two alternating groups
+            const char* spb = reinterpret_cast<const char*>(sp);
+            uint32_t xa[8], xb[8];
+            auto ldx = [&](uint32_t (&x)[8], int i0) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[u] * N_pad];
-#pragma unroll 1
-        for (int i0 = 0; i0 < nh; i0 += 8) {
-            const uint32_t xa = xn[0] | (xn[1] << 8) | (xn[2] << 16) | (xn[3] << 24);
-            const uint32_t xb = xn[4] | (xn[5] << 8) | (xn[6] << 16) | (xn[7] << 24);
-            if (i0 + 8 < nh) {
+                for (int u = 0; u < 8; ++u) x[u] = (uint32_t) * reinterpret_cast<const uint8_t*>(spb + c_tile.soff[i0 + u]);
+            };
+            auto mac = [&](const uint32_t (&x)[8], int i0) {
+                const uint32_t lo = x[0] | (x[1] << 8) | (x[2] << 16) | (x[3] << 24);
+                const uint32_t hi = x[4] | (x[5] << 8) | (x[6] << 16) | (x[7] << 24);
 #pragma unroll
-                for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[i0 + 8 + u] * N_pad];
+                for (int q = 0; q < QT; ++q) {
+                    acc[q] = (A)__dp4a(lo, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
+                    acc[q] = (A)__dp4a(hi, c_tile.qh[((i0 >> 2) + 1) * QT + q], (uint32_t)acc[q]);
+                }
+            };
+            ldx(xa, 0);
+#pragma unroll
+            for (int i0 = 0; i0 < GS_STRIP_MAX; i0 += 16) {
+                if (i0 >= nh) break;
+                if (i0 + 8 < nh) ldx(xb, i0 + 8);
+                mac(xa, i0);
+                if (i0 + 8 >= nh) break;
+                if (i0 + 16 < GS_STRIP_MAX && i0 + 16 < nh) ldx(xa, i0 + 16);
+                mac(xb, i0 + 8);
             }
+        } else {
+            uint32_t xn[8];
 #pragma unroll
-            for (int q = 0; q < QT; ++q) {
-                acc[q] = (A)__dp4a(xa, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
-                acc[q] = (A)__dp4a(xb, c_tile.qh[((i0 >> 2) + 1) * QT + q], (uint32_t)acc[q]);
+            for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[u] * N_pad];
+#pragma unroll 1
+            for (int i0 = 0; i0 < nh; i0 += 8) {
+                const uint32_t xa = xn[0] | (xn[1] << 8) | (xn[2] << 16) | (xn[3] << 24);
+                const uint32_t xb = xn[4] | (xn[5] << 8) | (xn[6] << 16) | (xn[7] << 24);
+                if (i0 + 8 < nh) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) xn[u] = (uint32_t)sp[(size_t)c_tile.hl[i0 + 8 + u] * N_pad];
+                }
+#pragma unroll
+                for (int q = 0; q < QT; ++q) {
+                    acc[q] = (A)__dp4a(xa, c_tile.qh[(i0 >> 2) * QT + q], (uint32_t)acc[q]);
+                    acc[q] = (A)__dp4a(xb, c_tile.qh[((i0 >> 2) + 1) * QT + q], (uint32_t)acc[q]);
+                }
             }
         }
 #pragma unroll
         for (int q = 0; q < QT; ++q) myacc[q] = acc[q];
     }
+}
+
+// QT <= 16: in line (unrolled, no call: the loads of the next block's first chunk stay in flight across the contraction
+// instead of being saved around a call).  Larger tiles: a separate function — compiled on its own, the strip loop's index
+// stays in a uniform register and the body stays small in the instruction cache.
+template <int WT, int QT>
+__device__ __noinline__ void strips_call(typename NumD<WT>::A* __restrict__ myacc, const typename NumD<WT>::W* __restrict__ sp,
+                                         int64_t N_pad) {
+    strips_body<WT, QT>(myacc, sp, N_pad);
+}
+template <int WT, int QT>
+__device__ __forceinline__ void strips_phase(typename NumD<WT>::A* __restrict__ myacc, const typename NumD<WT>::W* __restrict__ sp,
+                                             int64_t N_pad) {
+    if constexpr (QT <= 16) strips_body<WT, QT>(myacc, sp, N_pad);
+    else strips_call<WT, QT>(myacc, sp, N_pad);
 }
 
 template <int WT, int QT>
@@ -551,49 +573,16 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         cc0 = (int)(p.fwd_blk[blk] / GS_FWD_CHUNK);
         ncc = (int)(p.fwd_blk[blk + 1] / GS_FWD_CHUNK) - cc0;
     };
-    // L2 prefetch of what the warp reads one block later (no registers, no shared memory: the lines wait in the L2):
-    // the 128-byte strip segments of the next block's documents, one line per lane and turn, and the next block's
-    // posting range as bulk prefetches issued by two lanes.  The loads themselves then find their lines in the L2.
-    auto prefetch_block = [&](int d0, int cc0, int ncc) {
-#if GS_DOC_L2PF & 4
-        {   // the first chunks of the next block only (the start of its stream)
-            const int n4 = min(ncc, GS_DOC_PFSKIP);
-            if (n4 > 0) {
-                if (lane == 0)
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)cc0 * 32), "r"(n4 * 512) : "memory");
-                if (WT == GS_W_F32 && lane == 1)
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)cc0 * 32), "r"(n4 * 512) : "memory");
-            }
-        }
-#endif
-#if GS_DOC_L2PF & 2
-        if (ncc > 0) {
-            if (lane == 0)
-                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 512) : "memory");
-            if (WT == GS_W_F32) {
-                if (lane == 1)
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 512) : "memory");
-            } else if (!p.fwd_packed) {
-                if (lane == 1)
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp1 + (size_t)(uint32_t)cc0 * 32), "r"(ncc * 128) : "memory");
-            }
-        }
-#endif
-    };
-
     int sb = (int)blockIdx.x * NW + warp;
     int doc0 = 0, c0 = -1;                           // first document and first chunk of the current block
     int nc = 0;                                      // its chunks
-    // three chunk buffers: chunk i of a block lives in buffer i % 3 while it is in flight / being filtered (the chunk loop
-    // is unrolled by three so that no buffer is ever copied to another: the rotation by register moves was a quarter of
-    // the loop's instructions)
+    // two chunk buffers: chunk i of a block lives in buffer i % 2 while it is in flight / being filtered (the chunk loop is
+    // unrolled by two so that no buffer is ever copied to another: the rotation by register moves was a quarter of the
+    // loop's instructions).  A third buffer (two chunks in flight) spills at 64 registers and measured slower (69.7 vs
+    // 57.5 ms per 500-query batch); 24 or 28 warps with 80 / 72 registers and two chunks in flight: 64.4 / 62.0 ms
     uint4 tA = make_uint4(0, 0, 0, 0), wA = tA, tB = tA, wB = tA;
-#if GS_DOC_PF >= 2
-    uint4 tC = tA, wC = tA;
-#endif
     range_of(sb, doc0, c0, nc);
     if (nc > 0) load_chunk(c0, tA, wA);
-    if (GS_DOC_PF >= 2 && nc > 1) load_chunk(c0 + 1, tB, wB);
     for (; sb < n_subs; sb += sb_stride) {
         // the next block's range, asked for now, needed after the walk
         int doc0n, c0n, ncn;
@@ -601,47 +590,31 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         if (c0 < 0) {                              // block beyond the collection
             doc0 = doc0n; c0 = c0n; nc = ncn;
             if (nc > 0) load_chunk(c0, tA, wA);
-            if (GS_DOC_PF >= 2 && nc > 1) load_chunk(c0 + 1, tB, wB);
             continue;
         }
-        if (c0n >= 0) prefetch_block(doc0n, c0n, ncn);
         // the 128-byte strip segments of this block's documents, one line per lane and turn, into the L2 (no registers, no
-        // shared memory): asked for now, read after the walk.  Not a whole block earlier: in one block's time the stream
-        // turns the whole L2 over, and the lines were gone again (1.9 GB of re-reads per pass, measured)
+        // shared memory): asked for before the walk, read after it.  Not a whole block earlier: in one block's time the
+        // stream turns the whole L2 over, and the lines were gone again (1.9 GB of re-reads per pass, measured); at the
+        // block's start: 57.5 ms per 500-query batch against 54.9 here
         auto prefetch_strips = [&]() {
             for (int i = lane; i < nh; i += 32)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(strips + doc0) + s_soff[i]));
         };
-#if GS_DOC_L2PF & 1
-        prefetch_strips();
-#endif
-#if GS_DOC_L2PF & 4
-        if (nc > GS_DOC_PFSKIP) {                 // the rest of this block's stream
-            if (lane == 2)
-                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(tp4 + (size_t)(uint32_t)(c0 + GS_DOC_PFSKIP) * 32), "r"((nc - GS_DOC_PFSKIP) * 512) : "memory");
-            if (WT == GS_W_F32 && lane == 3)
-                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(wp4 + (size_t)(uint32_t)(c0 + GS_DOC_PFSKIP) * 32), "r"((nc - GS_DOC_PFSKIP) * 512) : "memory");
-        }
-#endif
-#if GS_DOC_L2PF & 8
         // rolling L2 prefetch of the posting stream: lanes 0..3 ask for the four 128-byte lines of the terms of the chunk
-        // GS_DOC_PFDIST ahead, lanes 4..7 for its fp32 weights
+        // kPfDist ahead, lanes 4..7 for its fp32 weights
         const char* pfb;
         if constexpr (WT == GS_W_F32)
             pfb = (lane < 4 ? reinterpret_cast<const char*>(tp4) : reinterpret_cast<const char*>(wp4)) + (lane & 3) * 128;
         else
             pfb = reinterpret_cast<const char*>(tp4) + (lane & 3) * 128;      // byte weights: the terms only (a fifth of the bytes)
         constexpr int pf_lanes = WT == GS_W_F32 ? 8 : 4;
-#endif
         for (int i = lane; i < 32 * AST; i += 32) s_acc[i] = A(0);
 
         // ---- tail: the block's postings as one flat range -> bitmap filter -> hit queue -> per-document walk
         int cnt = 0;
         auto filter_chunk = [&](const uint4& tc, const uint4& wc, int i) {
-#if GS_DOC_L2PF & 8
-            if (lane < pf_lanes && i + GS_DOC_PFDIST < nc)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(pfb + (size_t)(uint32_t)(c0 + i + GS_DOC_PFDIST) * 512));
-#endif
+            if (lane < pf_lanes && i + kPfDist < nc)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(pfb + (size_t)(uint32_t)(c0 + i + kPfDist) * 512));
             if (cnt + GS_FWD_CHUNK > QCAP) { walk(cnt); cnt = 0; }
             const uint32_t tw[4] = {tc.x, tc.y, tc.z, tc.w};
             const uint32_t ww[4] = {wc.x, wc.y, wc.z, wc.w};
@@ -661,22 +634,6 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
                 cnt += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
         };
-#if GS_DOC_PF >= 2
-        for (int i = 0;;) {                          // two chunks in flight ahead of the one being filtered
-            if (i >= nc) break;
-            if (i + 2 < nc) load_chunk(c0 + i + 2, tC, wC);
-            filter_chunk(tA, wA, i);
-            ++i;
-            if (i >= nc) break;
-            if (i + 2 < nc) load_chunk(c0 + i + 2, tA, wA);
-            filter_chunk(tB, wB, i);
-            ++i;
-            if (i >= nc) break;
-            if (i + 2 < nc) load_chunk(c0 + i + 2, tB, wB);
-            filter_chunk(tC, wC, i);
-            ++i;
-        }
-#else
         for (int i = 0;;) {                          // one chunk in flight ahead of the one being filtered
             if (i >= nc) break;
             if (i + 1 < nc) load_chunk(c0 + i + 1, tB, wB);
@@ -687,14 +644,10 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
             filter_chunk(tB, wB, i);
             ++i;
         }
-#endif
-#if GS_DOC_L2PF & 16
         prefetch_strips();
-#endif
         walk(cnt);
         // first chunks of the next block: in flight during the contraction
         if (ncn > 0) load_chunk(c0n, tA, wA);
-        if (GS_DOC_PF >= 2 && ncn > 1) load_chunk(c0n + 1, tB, wB);
 
         // ---- head strips: thread = document, QT accumulators in registers, weights as uniform constant operands
         const int64_t doc = (int64_t)doc0 + lane;
