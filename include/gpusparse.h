@@ -179,10 +179,10 @@ GS_API gs_status_t gs_index_copy_head_terms(const gs_index_t* index, int32_t cap
  * q̄·L̄ postings per query, the document-parallel kernel streams all N·k̄ postings per pass, and the crossover is where the
  * work ratio meets the ratio of the effective rates.  On B200 both sides were measured over N in {20K .. 1M} documents,
  * B in {1 .. 256} queries of 25 .. 4000 terms (profiles/r02_dispatch_sweep.md); the forms below predict
- * the faster path on 62 of the 64 grid points (the two misses cost 7 %):
- *   term: 0.10 ms + max(1, B*tiles / 9472 warp slots) * (nnz/B) * 0.5 us * (1 + 0.6*min(1, N/1e6))
- *         (a cell row costs ~0.5 us per query term: one segment-table probe per (query, term, doc tile));
- *   doc : 0.13 ms + ceil(B/QT) * stream_bytes / 4.0 TB/s + nnz * 0.1 us * (1 + 2.7*N/1e6)
+ * the faster path on 63 of the 64 grid points (the miss costs 6 %):
+ *   term: 0.10 ms + max(1, B*tiles / 9472 warp slots) * (nnz/B) * 0.6 us * (1 + 1.8*min(1, N/1e6))
+ *         (a cell row costs ~0.6 us per query term: one segment-table probe per (query, term, doc tile));
+ *   doc : 0.13 ms + ceil(B/QT) * stream_bytes / 4.7 TB/s + nnz * 0.1 us * (1 + 2.7*N/1e6)
  *         (one pass over the forward index per tile of QT = 8 (B <= 8) or 16 queries, plus the hit walk).
  * Host arithmetic only (no device call, no handle): num_docs, tile_docs and stream_bytes (forward index + head strips,
  * gs_info_t.bytes_forward + the head share of bytes_head) describe the index; B and nnz the query batch.  Returns

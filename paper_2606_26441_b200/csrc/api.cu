@@ -391,14 +391,15 @@ int32_t gs_dispatch_model(int64_t num_docs, int32_t tile_docs, int64_t stream_by
                           double* out_doc_ms) {
     const double N = (double)std::max<int64_t>(num_docs, 0), Bq = (double)std::max<int64_t>(B, 1), terms = (double)std::max<int64_t>(nnz, 0);
     const double tiles = std::ceil(N / (double)std::max(tile_docs, 1));
-    // term-parallel: cell rows = B * tiles over 148 SMs x 64 warp slots; a row costs ~0.5 us per query term (one
-    // segment-table probe per (query, term, doc tile) plus the postings it finds), a little more on long lists
+    // term-parallel: cell rows = B * tiles over 148 SMs x 64 warp slots; a row costs ~0.6 us per query term (one
+    // segment-table probe per (query, term, doc tile) plus the postings it finds), up to 2.8x that on long lists
     const double waves = std::max(1.0, Bq * tiles / 9472.0);
-    const double t_term = 0.10 + waves * (terms / Bq) * 0.5e-3 * (1.0 + 0.6 * std::min(1.0, N / 1e6));
-    // document-parallel: one pass over the forward index per tile of QT queries at ~4.0 TB/s, plus the hit walk
+    const double t_term = 0.10 + waves * (terms / Bq) * 0.6e-3 * (1.0 + 1.8 * std::min(1.0, N / 1e6));
+    // document-parallel: one pass over the forward index per tile of QT queries at ~4.7 TB/s, plus the hit walk
+    // (constants re-fitted to the sweep of the reworked kernels, profiles/r02_dispatch_sweep.csv)
     const double qt = B <= 8 ? 8.0 : 16.0;
     const double passes = std::ceil(Bq / qt);
-    const double t_doc = 0.13 + passes * ((double)std::max<int64_t>(stream_bytes_, 0) / 4.0e9) + terms * 0.1e-3 * (1.0 + 2.7 * N / 1e6);
+    const double t_doc = 0.13 + passes * ((double)std::max<int64_t>(stream_bytes_, 0) / 4.7e9) + terms * 0.1e-3 * (1.0 + 2.7 * N / 1e6);
     if (out_term_ms) *out_term_ms = t_term;
     if (out_doc_ms) *out_doc_ms = t_doc;
     return t_doc < t_term ? GS_ALGO_DOC_PARALLEL : GS_ALGO_TERM_PARALLEL;
