@@ -363,6 +363,15 @@ __global__ void __launch_bounds__(kRowThreads, 2) k_sel_row(gs_sel_src src, int3
         }
         __syncthreads();
     }
+    // Threshold-only call (the sample select of a search: no ids, no scores): once the score half of the key is resolved,
+    // the prefix itself — selected digits, zeros below — is the answer.  The keys >= prefix are exactly the k selected
+    // ones, so it bounds the k-th key from below and differs from it in doc-id bits only; the filter that uses it
+    // (key >= threshold) lets the same sample cells pass.  Skips the collect pass, two cluster barriers and the sort
+    // (a third of this launch at one row).  The loop ran (more than k live keys) whenever s_shift has left 64.
+    if (out_ids == nullptr && out_thr != nullptr && s_shift <= 32) {
+        if (rank == 0 && tid == 0) out_thr[b] = s_prefix;
+        return;                                // no CTA reads another's shared memory after the loop's last cluster barrier
+    }
     // collect the keys >= threshold (exactly min(k, live) of them: all keys are distinct) in CTA 0, sort, decode
     const uint64_t thr = s_prefix;
     if (rank == 0)
