@@ -68,6 +68,7 @@ struct TermParams {
     gs_tileset ts;
     gs_sink sink;
     int32_t vec4;                               // dense sink rows are 16-byte aligned
+    int32_t pf_rows;                            // small-batch kernel: few rows in flight -> each asks the L2 for its strips at its start
 };
 
 // Slot range [lo, hi) of the postings of a tail term (descriptor d: weight bits, table offset, table mode, -) inside doc
@@ -172,6 +173,40 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
     const int quads = Ts >> 2;
     for (int dq = lane; dq < quads; dq += 32) reinterpret_cast<int4*>(row)[dq] = make_int4(0, 0, 0, 0);
     __syncwarp();
+    if (!STAGED && p.pf_rows) {
+        // A launch of few rows (the threshold sample of a small batch: 136 rows at B = 1) is pure latency: the head phase
+        // below reads a row's strip segments strip by strip, ~26 exposed round trips per row.  Ask the L2 for all of
+        // them now (one 128-byte line per lane and turn, no registers): they arrive under the tail scatter.  Only for
+        // such launches: with thousands of rows in flight (26 KB each) the prefetched lines exceed the L2 and are gone
+        // before their use (single-query filter launch: 0.138 -> 0.160 ms, profiles/r02_kernels.md).
+        const int L = (Ts * (int)sizeof(W) + 127) >> 7;                    // lines per strip segment
+        if ((L & (L - 1)) == 0 && L <= 32) {
+            const int sh = 31 - __clz(L), spw = 32 >> sh;                   // strips per warp turn
+            const int hc0 = p.H > 0 ? p.head_cnt[b] : 0;
+            const int nh0 = hc0 & 0xFF, n_hot0 = hc0 >> 8;
+            const uint2* hl0 = p.head_pair + b * GS_HEAD_MAX;
+            const char* g0 = reinterpret_cast<const char*>(reinterpret_cast<const W*>(p.head_strip) + base) + ((lane & (L - 1)) << 7);
+            for (int s0 = 0; s0 < nh0; s0 += spw) {
+                const int si = s0 + (lane >> sh);
+                if (si < nh0) {
+                    const uint2 e = head_entry(hl0, si, n_hot0);
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(g0 + (size_t)e.x * (size_t)p.N_pad * sizeof(W)));
+                }
+            }
+            if (XS) {
+                const int nx0 = p.xcnt[b];
+                const uint2* xl0 = p.xpair + b * GS_XSTRIP_MAX;
+                const char* x0 = reinterpret_cast<const char*>(reinterpret_cast<const W*>(p.xstrip) + base) + ((lane & (L - 1)) << 7);
+                for (int s0 = 0; s0 < nx0; s0 += spw) {
+                    const int si = s0 + (lane >> sh);
+                    if (si < nx0) {
+                        const uint2 e = __ldg(xl0 + si);
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(x0 + (size_t)e.x * (size_t)p.N_pad * sizeof(W)));
+                    }
+                }
+            }
+        }
+    }
 
     // scatter the tail lists of the query: segment of each list inside this tile, 32 terms probed at once.  The
     // non-empty segments are applied one after the other (two lists may hit the same document), but the first 32
@@ -1319,6 +1354,9 @@ __global__ void __launch_bounds__(kMQ * 32, 1) k_score_term_mma(const TermParams
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem0), "n"(512));
 }
 
+// launches of at most this many cell rows prefetch their strips into the L2 at row start (process_item); 1024 and 4096
+// measured alike: single-query search 0.1375 -> 0.1336 ms of scoring, Zipf-1.3 collection 0.832 -> 0.811, integer 0.107 -> 0.103
+constexpr int64_t kPfRowsMax = 1024;
 int norm_warps(int w) { return w <= 0 ? kWarpsDefault : std::min(w, kWarpsMax); }
 
 template <int WT, bool XS>
@@ -1330,7 +1368,9 @@ gs_status_t launch_x(const TermParams& p, unsigned grid, size_t smem, bool stage
     } else {
         GS_CUDA(gs_optin_smem(k_score_term<WT, XS>));
         GsProfScope ps(GS_K_SCORE_TERM, s);
-        k_score_term<WT, XS><<<grid, p.warps * 32, smem, s>>>(p);
+        TermParams pp = p;
+        pp.pf_rows = (int64_t)p.ts.count * p.nq <= kPfRowsMax ? 1 : 0;
+        k_score_term<WT, XS><<<grid, p.warps * 32, smem, s>>>(pp);
     }
     ++gs_tls_launches;
     GS_CUDA(cudaGetLastError());
