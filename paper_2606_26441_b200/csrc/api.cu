@@ -173,7 +173,10 @@ Plan make_plan(const gs_index* ix, int64_t B, int64_t nnz, int32_t k, const gs_s
         p.group = o->query_group;
         p.qtile = o->doc_query_tile;
     }
-    if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : 16;   // doc-parallel: queries per pass; 16 is the largest tile that stays HBM bound
+    // doc-parallel, queries per pass: 16 is the largest tile that stays HBM bound in fp32; the integer
+    // kernel is issue bound at every size and a pass of 32 queries costs it less than two of 16 (44.5 vs 54.2 ms per
+    // 500-query batch at 8.8M docs)
+    if (p.qtile <= 0) p.qtile = B <= 8 ? 8 : (ix->wtype == GS_W_U8 && B >= 32 ? 32 : 16);
     p.use_head = !(p.flags & GS_FLAG_NO_HEAD_STRIPS);
     // Threshold sample = 1/2^shift of the doc tiles.  The select phases read the sample (N/2^shift cells per query) and
     // the candidates (about k*2^shift per query), so the balance is 2^shift ~ sqrt(N/k); the candidate lists
