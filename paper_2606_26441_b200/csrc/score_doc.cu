@@ -19,7 +19,8 @@
 //   * every other posting sits in a "tail" block CSR: one row pointer per aligned block of 32
 //     documents, the block's postings one flat range padded to 128, the term word carrying the
 //     document's position in the block.  A warp owns a block and streams its range with 128-bit
-//     loads (next chunk prefetched, next block's first chunk prefetched across the contraction),
+//     loads (one 1 KB chunk in flight in registers — the next block's first chunk across the
+//     contraction —, the chunk four ahead asked for from the L2 by prefetch.global.L2),
 //     tests each term against a V-bit bitmap of the tile's tail terms (shared memory) and compacts
 //     the hits, in stream order, into a per-warp queue (one ballot prefix per 128 postings).  Then
 //     lane d walks the hits of document d (contiguous in the queue: a binary search finds them) in
@@ -29,6 +30,12 @@
 // Each (query, doc) cell is produced by exactly one thread in a fixed order — zero atomics,
 // deterministic.  The query tiles (bitmap + popcount prefix, row table, head weights, thresholds)
 // are built once per search by k_build_qtile.
+//
+// What bounds it (profiles/r02_kernels.md, last sections): 32 warps x 64 registers per SM.  A second chunk in
+// flight, eight strip values in flight, fewer warps with more registers, batched candidate atomics: each
+// measured slower (spills, or too few warps).  The latency the registers cannot cover is covered from the
+// L2 instead — prefetches a few microseconds ahead, not a block ahead: at 4.7 TB/s the stream replaces the
+// whole 126 MB L2 within one block's time.
 #include <algorithm>
 #include <cstddef>
 #include <mutex>
@@ -189,7 +196,7 @@ __global__ void __launch_bounds__(1024) k_build_qtile(const int64_t* __restrict_
                 ct->soff[n] = (unsigned long long)h * (unsigned long long)strip_row_bytes;
                 ct->hl[n++] = (uint32_t)h;
             }
-        const uint32_t n8 = WT == GS_W_F32 ? ((n + 3u) & ~3u) : ((n + 7u) & ~7u);      // strips per turn of strips_phase
+        const uint32_t n8 = WT == GS_W_F32 ? ((n + 3u) & ~3u) : ((n + 7u) & ~7u);      // strips per turn of the strip contraction
         for (uint32_t i = n; i < GS_STRIP_MAX; ++i) { ct->hl[i] = 0u; ct->soff[i] = 0ull; }      // padding rows carry zero weights
         ct->nh = n8;
         ct->R = R;
@@ -293,10 +300,11 @@ __device__ __forceinline__ uint4 ld_stream4(const uint4* p) { return __ldcs(p); 
 __device__ __forceinline__ uint32_t ld_stream1(const uint32_t* p) { return __ldcs(p); }
 
 // Dense strip contraction of one document (thread = document): acc[q] += x[h][doc] * Q[h][q] over the strips the
-// tile uses.  A separate (not inlined) function: compiled on its own, the strip loop's index stays in a uniform
-// register, so every weight is fetched by a uniform constant load (LDCU c[3][UR+imm]) and used as the uniform
-// operand of the FFMA/IMAD itself, and the body (4 x QT multiply-adds) stays small in the instruction cache.
-// The accumulators travel through the lane's own row of the shared-memory tile (conflict-free).
+// tile uses; every weight is fetched by a uniform constant load and used as the uniform operand of the FFMA2 / IDP4A
+// itself.  Tiles of up to 16 queries: fully unrolled and in line (strips_body below).  Larger tiles: a separate
+// function (strips_call) — compiled on its own, the strip loop's index stays in a uniform register (LDCU
+// c[3][UR+imm]), the body (4 x QT multiply-adds) stays small in the instruction cache, and the accumulators travel
+// through the lane's own row of the shared-memory tile (conflict-free).
 __device__ __forceinline__ unsigned long long fma_f32x2(unsigned long long a, float x, unsigned long long c) {
     // (a.lo * x + c.lo, a.hi * x + c.hi): one FFMA2, each half an IEEE fp32 fma (same result as two fmaf)
     unsigned long long d, xx;
