@@ -175,6 +175,19 @@ def test_doc_parallel_long_rows(gs, qtile):
     assert np.all(np.abs(S.astype(np.float64) - A) <= np.maximum(4e-5 * np.abs(A), 1e-6))
     ids, sc = gpu_search(gs, ix, queries, 10, algo="doc", doc_query_tile=qtile)
     assert ids.shape == (B, 10) and np.all(ids >= 0)
+    # the top-10 against the oracle's, with the same widened relative bound: structure, values, set, order
+    o_ids, o_sc = oracle.search(R_q, R_d, 10)
+    for b in range(B):
+        t = A[b, ids[b]]
+        bound = lambda x: np.maximum(4e-5 * np.abs(x), 1e-6)
+        assert len(set(ids[b].tolist())) == 10 and np.all(np.diff(sc[b]) <= 0)
+        eq = np.nonzero(np.diff(sc[b]) == 0)[0]
+        assert np.all(ids[b][eq] < ids[b][eq + 1])
+        assert np.all(np.abs(sc[b].astype(np.float64) - t) <= bound(t))
+        tau = o_sc[b][9]
+        assert np.all(np.isin(o_ids[b][o_sc[b] > tau + 2 * bound(tau)], ids[b])), "a clearly-top-k document is missing"
+        assert np.all(t >= tau - 2 * bound(tau)), "a returned document is clearly below the k-th score"
+        assert np.all(t[:-1] >= t[1:] - 2 * bound(t[1:])), "returned order contradicts true scores"
     ix.close()
 
 
@@ -308,10 +321,19 @@ def test_signed_weights_and_negative_zero(gs, algo):
         # cancellation makes |score| small relative to the summands: compare with an absolute bound from the summand sizes
         for b in range(q.rows):
             t = oracle.score_pairs(R_q, R_d, np.full(k, b, np.int64), ids[b].astype(np.int64))
-            assert np.all(np.abs(sc[b] - t) <= 1e-5 * 30 * 16), "score error"
+            atol = 1e-5 * 30 * 16
+            assert np.all(np.abs(sc[b] - t) <= atol), "score error"
             assert np.all(np.diff(sc[b]) <= 0) and len(set(ids[b].tolist())) == k
             eq = np.nonzero(np.diff(sc[b]) == 0)[0]
             assert np.all(ids[b][eq] < ids[b][eq + 1])
+            # the top-k SET against the oracle's (same rule as parity.check_f32_row, with the absolute bound): every
+            # document clearly above the oracle's k-th score is returned, nothing returned is clearly below it, and the
+            # returned order does not contradict the true scores
+            tau = o_sc[b][k - 1]
+            must = o_ids[b][o_sc[b] > tau + 2 * atol]
+            assert np.all(np.isin(must, ids[b])), "a clearly-top-k document is missing"
+            assert np.all(t >= tau - 2 * atol), "a returned document is clearly below the k-th score"
+            assert np.all(t[:-1] >= t[1:] - 2 * atol), "returned order contradicts true scores"
     ix.close()
 
 
