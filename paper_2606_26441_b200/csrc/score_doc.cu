@@ -803,7 +803,7 @@ gs_status_t gs_launch_score_doc(const gs_index* ix, const gs_csr_t* q, const gs_
     p.ts = ts; p.sink = sink; p.status = qb.status;
     const int64_t n_subs = (int64_t)ts.count * (ix->Ts / 32);
     // the kernel keeps block, chunk and document numbers in 32 bits
-    if (n_subs >= (1LL << 31) - (1LL << 20) || ix->N >= (1LL << 31) - 64 || ix->P_fwd / GS_FWD_CHUNK >= (1LL << 31) - 8) return GS_ERR_OUT_OF_RANGE;
+    if (n_subs >= (1LL << 31) - (1LL << 20) || ix->N_pad + ix->Ts >= (1LL << 31) || ix->P_fwd / GS_FWD_CHUNK >= (1LL << 31) - 8) return GS_ERR_OUT_OF_RANGE;
     return ix->wtype == GS_W_F32
                ? launch_doc_qt<GS_W_F32>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s)
                : launch_doc_qt<GS_W_U8>(QT, p, (const unsigned char*)scratch, Wd, n_subs, n_passes, q0, nq, sms, smem_max, s);
