@@ -560,10 +560,16 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
     const uint4* __restrict__ wp4 = reinterpret_cast<const uint4*>(p.fwd_w);           // f32
     const uint4* __restrict__ tp4 = reinterpret_cast<const uint4*>(p.fwd_terms);
     // chunk c (128 postings) of the index: lane holds postings 4*lane .. 4*lane+3
-    auto load_chunk = [&](int chunk, uint4& t4, uint4& w4) {
-        t4 = ld_stream4(tp4 + (size_t)(uint32_t)chunk * 32 + lane);
+    auto load_chunk = [&](int chunk, uint4& t4, uint4& w4, bool pf = false) {
+        const uint4* tptr = tp4 + (size_t)(uint32_t)chunk * 32 + lane;
+        t4 = ld_stream4(tptr);
+        // rolling L2 prefetch: a lane whose 16 bytes start a 128-byte line (lanes 0, 8, 16, 24) asks for the same line of
+        // the chunk kPfDist - 1 further on — the load's own address plus a constant, no address arithmetic of its own
+        if (pf) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(tptr) + (kPfDist - 1) * 512));
         if (WT == GS_W_F32) {
-            w4 = ld_stream4(wp4 + (size_t)(uint32_t)chunk * 32 + lane);
+            const uint4* wptr = wp4 + (size_t)(uint32_t)chunk * 32 + lane;
+            if (pf) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(wptr) + (kPfDist - 1) * 512));
+            w4 = ld_stream4(wptr);
         } else if (p.fwd_packed) {                 // compressed postings: term | impact << 19 | (doc & 31) << 27
             w4 = make_uint4((t4.x >> 19) & 0xFFu, (t4.y >> 19) & 0xFFu, (t4.z >> 19) & 0xFFu, (t4.w >> 19) & 0xFFu);
             t4 = make_uint4(t4.x & 0xF807FFFFu, t4.y & 0xF807FFFFu, t4.z & 0xF807FFFFu, t4.w & 0xF807FFFFu);
@@ -608,21 +614,14 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
             for (int i = lane; i < nh; i += 32)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(strips + doc0) + s_soff[i]));
         };
-        // rolling L2 prefetch of the posting stream: lanes 0..3 ask for the four 128-byte lines of the terms of the chunk
-        // kPfDist ahead, lanes 4..7 for its fp32 weights
-        const char* pfb;
-        if constexpr (WT == GS_W_F32)
-            pfb = (lane < 4 ? reinterpret_cast<const char*>(tp4) : reinterpret_cast<const char*>(wp4)) + (lane & 3) * 128;
-        else
-            pfb = reinterpret_cast<const char*>(tp4) + (lane & 3) * 128;      // byte weights: the terms only (a fifth of the bytes)
-        constexpr int pf_lanes = WT == GS_W_F32 ? 8 : 4;
+        // rolling L2 prefetch of the posting stream (load_chunk): the lanes whose 16 bytes start a 128-byte line ask for
+        // the same line of the chunk kPfDist ahead of the one being filtered
+        const bool pf_lane = (lane & 7) == 0;
         for (int i = lane; i < 32 * AST; i += 32) s_acc[i] = A(0);
 
         // ---- tail: the block's postings as one flat range -> bitmap filter -> hit queue -> per-document walk
         int cnt = 0;
-        auto filter_chunk = [&](const uint4& tc, const uint4& wc, int i) {
-            if (lane < pf_lanes && i + kPfDist < nc)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(pfb + (size_t)(uint32_t)(c0 + i + kPfDist) * 512));
+        auto filter_chunk = [&](const uint4& tc, const uint4& wc) {
             if (cnt + GS_FWD_CHUNK > QCAP) { walk(cnt); cnt = 0; }
             const uint32_t tw[4] = {tc.x, tc.y, tc.z, tc.w};
             const uint32_t ww[4] = {wc.x, wc.y, wc.z, wc.w};
@@ -644,12 +643,12 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
         };
         for (int i = 0;;) {                          // one chunk in flight ahead of the one being filtered
             if (i >= nc) break;
-            if (i + 1 < nc) load_chunk(c0 + i + 1, tB, wB);
-            filter_chunk(tA, wA, i);
+            if (i + 1 < nc) load_chunk(c0 + i + 1, tB, wB, pf_lane && i + kPfDist < nc);
+            filter_chunk(tA, wA);
             ++i;
             if (i >= nc) break;
-            if (i + 1 < nc) load_chunk(c0 + i + 1, tA, wA);
-            filter_chunk(tB, wB, i);
+            if (i + 1 < nc) load_chunk(c0 + i + 1, tA, wA, pf_lane && i + kPfDist < nc);
+            filter_chunk(tB, wB);
             ++i;
         }
         prefetch_strips();
