@@ -121,7 +121,7 @@ __global__ void k_finalize_stats(StatsBlock* sb, const uint32_t* cand_cnt, int64
     __syncthreads();
     unsigned long long local = 0;
     for (int64_t b = threadIdx.x; b < B; b += blockDim.x) {
-        const uint32_t c = cand_cnt ? cand_cnt[b] : 0u;
+        const uint32_t c = cand_cnt ? cand_cnt[b * GS_CNT_STRIDE] : 0u;
         local += c;
         if (cand_cnt && (int64_t)c > cap) overflow_list[atomicAdd(&n_ov, 1)] = (int32_t)b;
     }
@@ -239,7 +239,7 @@ Carve carve_ws(const gs_index* ix, const Plan& p, int64_t B, int64_t nnz, int32_
     c.qb.xpair = (uint2*)take((size_t)B * GS_XSTRIP_MAX * 8);
     c.qb.xcnt = (int32_t*)take((size_t)B * 4);
     c.thr = (uint64_t*)take((size_t)B * 8);
-    c.cand_cnt = (uint32_t*)take((size_t)B * 4);
+    c.cand_cnt = (uint32_t*)take((size_t)B * 4 * GS_CNT_STRIDE);
     c.overflow_list = (int32_t*)take((size_t)B * 4);
     c.sel_scratch = take(gs_select_scratch_bytes(B, k));
     c.doc_scratch = p.algo == GS_ALGO_DOC_PARALLEL ? take(gs_score_doc_scratch_bytes_ex(ix, p.qtile, B, nnz)) : nullptr;
@@ -335,7 +335,7 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     // ---- 2. filter: all tiles, emit key >= bound
     {
         GsProfScope ps(GS_K_MISC, s);
-        k_zero_u32<<<(unsigned)((B + 255) / 256), 256, 0, s>>>(c.cand_cnt, B);
+        k_zero_u32<<<(unsigned)((B * GS_CNT_STRIDE + 255) / 256), 256, 0, s>>>(c.cand_cnt, B * GS_CNT_STRIDE);
     }
     ++gs_tls_launches;
     {
@@ -347,7 +347,7 @@ gs_status_t search_impl(const gs_index* ix, const gs_csr_t* q, int32_t k, const 
     // ---- 3. final select over the candidate lists
     {
         gs_sel_src src{};
-        src.keys = c.cand; src.cap = p.cand_cap; src.counts = c.cand_cnt; src.wtype = ix->wtype;
+        src.keys = c.cand; src.cap = p.cand_cap; src.counts = c.cand_cnt; src.cnt_stride = GS_CNT_STRIDE; src.wtype = ix->wtype;
         GS_TRY(gs_launch_select(src, B, k, out_ids, out_scores, nullptr, nullptr, nullptr, 0, c.sel_scratch, s));
     }
     {

@@ -176,12 +176,16 @@ struct gs_tileset {
     int32_t stride = 1;      // tile j of the set is doc tile first + j*stride
     int32_t count = 0;       // number of tiles in the set
 };
+// Candidate counters sit one per 128-byte line.  A document-parallel pass adds to the counters of its 16 queries once per
+// passing cell (2 M atomics per pass at 8.8M docs): packed into one line they all queue at one L2 slice, and the pass time
+// then depended on where the workspace happened to lie (15.0 vs 20.3 ms per 128-query search for workspaces 2 MB apart).
+#define GS_CNT_STRIDE 32
 struct gs_sink {
     uint32_t* dense = nullptr;
     int64_t ld = 0;
     const uint64_t* thr = nullptr;       // [B] threshold keys (filter mode when non-null)
     uint64_t* cand = nullptr;            // [B][cand_cap]
-    uint32_t* cand_cnt = nullptr;        // [B]
+    uint32_t* cand_cnt = nullptr;        // [B * GS_CNT_STRIDE]: query b's counter is cand_cnt[b * GS_CNT_STRIDE]
     int64_t cand_cap = 0;
 };
 
@@ -230,6 +234,7 @@ struct gs_sel_src {
     const uint64_t* keys = nullptr;
     int64_t cap = 0;
     const uint32_t* counts = nullptr;
+    int32_t cnt_stride = 1;    // row b's count is counts[b * cnt_stride]
     int32_t wtype = 0;
 };
 size_t gs_select_scratch_bytes(int64_t rows, int32_t k);

@@ -677,7 +677,7 @@ __global__ void __launch_bounds__(Geo<QT>::NW * 32, 1) k_score_doc(const DocPara
                         const uint64_t key = gs_make_key(gs_ord_bits<WT>(NumD<WT>::bits(acc[q])), (uint32_t)doc);
                         if (q < p.nqt && key >= c_tile.thr_key[q]) {
                             const int64_t b = p.qa + q;
-                            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                            const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b * GS_CNT_STRIDE], 1u);
                             if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                         }
                     }

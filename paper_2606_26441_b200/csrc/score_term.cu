@@ -379,7 +379,7 @@ __device__ __forceinline__ void process_item(const TermParams& p, typename Num<W
         }
         const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
         uint32_t pos = 0;
-        if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b], total);
+        if (lane == 0) pos = atomicAdd(&p.sink.cand_cnt[b * GS_CNT_STRIDE], total);
         pos = __shfl_sync(0xFFFFFFFFu, pos, 0) + incl - mine;
         while (mask) {
             const int bit = __ffs(mask) - 1;
@@ -688,7 +688,7 @@ __device__ __noinline__ void batch_flush(uint32_t* cand_cnt, uint64_t* cand, int
         const int end = later ? __ffs((int)later) - 1 : n_valid;          // one past the run's last lane
         const int64_t bb = q0 + (valid ? (int64_t)qi : 0);
         uint32_t pos = 0;
-        if (head) pos = atomicAdd(&cand_cnt[bb], (uint32_t)(end - lane));
+        if (head) pos = atomicAdd(&cand_cnt[bb * GS_CNT_STRIDE], (uint32_t)(end - lane));
         pos = __shfl_sync(0xFFFFFFFFu, pos, start & 31) + (uint32_t)(lane - start);
         if (valid && (int64_t)pos < cand_cap) cand[bb * cand_cap + pos] = w_key[i];
     }
@@ -1052,7 +1052,7 @@ __global__ void __launch_bounds__(kBWarps * 32, 1) k_score_term_batch(const Term
                         w_key[slot] = key;
                         w_q[slot] = (uint16_t)q;
                     } else {                                             // buffer full: append directly
-                        const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                        const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b * GS_CNT_STRIDE], 1u);
                         if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                     }
                 }
@@ -1334,7 +1334,7 @@ __global__ void __launch_bounds__(kMQ * 32, 1) k_score_term_mma(const TermParams
                                 w_key[slot] = key;
                                 w_q[slot] = (uint16_t)qq;
                             } else {                                         // buffer full: append directly
-                                const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b], 1u);
+                                const uint32_t pos = atomicAdd(&p.sink.cand_cnt[b * GS_CNT_STRIDE], 1u);
                                 if ((int64_t)pos < p.sink.cand_cap) p.sink.cand[b * p.sink.cand_cap + pos] = key;
                             }
                         }

@@ -32,7 +32,7 @@ struct SelState {
 };
 
 __device__ __forceinline__ int64_t src_count(const gs_sel_src& s, int64_t b) {
-    return s.keys ? (int64_t)min((uint64_t)s.counts[b], (uint64_t)s.cap) : s.n_cols;
+    return s.keys ? (int64_t)min((uint64_t)s.counts[b * s.cnt_stride], (uint64_t)s.cap) : s.n_cols;
 }
 // key of item i of row b, or 0 when the item does not exist (column beyond the last document)
 template <int WT>
